@@ -1,0 +1,111 @@
+/* bse.h - C ABI of the B200-native screened-exchange hot path of the low-rank BSE method
+ * (arxiv 2409.15116, "WEST-BSE").  Citations are PAPER.md line numbers.
+ *
+ * What the library computes
+ *   bse_build_tau : overlap screen of occupied-orbital pairs (eq. 16) and, for every
+ *                   surviving pair (v<=v'), the screened Coulomb pair integral
+ *                       tau_vv'(r) = int W(r,r') u_v(r') u_v'(r') dr'              (eq. 6)
+ *                   with W = v_c + v_c^{1/2} chibar v_c^{1/2} applied through the PDEP low-rank form
+ *                       chibar = sum_a |phi_a> lambda_a/(1-lambda_a) <phi_a|       (eq. 9-11)
+ *   bse_apply_k1x : out[b,v] = P_c sum_{v'} tau_vv' a[b,v'],  P_c x = x - sum_w u_w <u_w|x>
+ *                                                               (eq. 5 and PAPER.md:67; the paper's K^1d)
+ *
+ * Conventions (normative)
+ *   grid n1 x n2 x n3 (this version: n1 = n2 = n3 = n even, cubic cell of edge L, else BSE_EUNSUPPORTED),
+ *   linear index (i1*n + i2)*n + i3;  r = (L/n) i;  G = (2 pi/L) m;  Hartree atomic units.
+ *   sphere S = { m : |m|^2 <= floor(2 ecut (L/2pi)^2 (1+1e-12)) };  R = floor(sqrt(max)) must be < n/2.
+ *   half sphere H = { m in S : m3>0 } U { m3=0, m2>0 } U { m3=m2=0, m1>=0 }, sorted by ascending
+ *   ((m1 mod n) n + (m2 mod n)) n + (m3 mod n);  Npw_h = |H|.  PW arrays hold c(G) on H, interleaved
+ *   (re,im), with f(r) = sum_{G in S} c(G) e^{+iG.r}, c(-G) = conj c(G), c(0) real.
+ *   v_c(G) = 4 pi/|G|^2, v_c(0) := 0.  phi_a normalised sum_S |phi_a(G)|^2 = 1, phi_a(0) = 0.
+ *   Everything is fp64.
+ *
+ * Ownership: the caller owns every array it passes.  With device pointers (default) `u` and `phi` are
+ *   BORROWED: they must stay alive and unmodified until bse_destroy.  With BSE_PTR_HOST the library copies
+ *   them to device memory it owns during bse_create.  `out` must not alias `a`.  The library owns the pair
+ *   list, the tau store and all workspaces.
+ * Errors: every call returns a status; nothing throws or exits across the ABI.  There is NO CPU fallback:
+ *   without a CUDA device every compute entry point returns BSE_ECUDA.
+ * Asynchrony: work is enqueued on the cudaStream_t passed at create (NULL = default stream); calls that
+ *   return host data synchronise that stream.  bse_build_tau synchronises once (pair count read-back).
+ */
+#ifndef BSE_H
+#define BSE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct bse_handle bse_handle;
+
+enum { BSE_OK = 0, BSE_EINVAL = -1, BSE_ENOMEM = -2, BSE_ECUDA = -3, BSE_ESTATE = -4, BSE_EUNSUPPORTED = -5 };
+
+/* flags of bse_create */
+#define BSE_TAU_REAL   0x0u   /* tau_vv'(r) stored on the real-space grid, [P][N] doubles (default)          */
+#define BSE_TAU_PW     0x1u   /* tau_vv'(G) stored on H, [P][Npw_h] complex; inverse FFT inside the apply     */
+#define BSE_TAU_STREAM 0x2u   /* nothing stored: tau rebuilt in pair batches inside every bse_apply_k1x       */
+#define BSE_TAU_MASK   0x3u
+#define BSE_VEC_REAL   0x0u   /* a/out = [B][Nv][N] real (default)                                            */
+#define BSE_VEC_PW     0x4u   /* a/out = [B][Nv][Npw_h] complex on H ("of length N_pw")         */
+#define BSE_PTR_HOST   0x8u   /* u and phi passed to bse_create are HOST pointers (copied to the device)      */
+
+/* Create a problem instance.  Builds the sphere/stick tables, twiddles and v_c^{1/2} on the host and uploads
+ * them; launches no heavy work.
+ *   grid[3]   n1,n2,n3 (i3 fastest)                cell[9]  row-major lattice vectors (bohr)
+ *   ecut      Ha, sphere |G|^2/2 <= ecut           Nv, u    [Nv][N] real, orthonormal: dV sum_r u_v u_w = delta
+ *   Npdep,phi [Npdep][Npw_h] complex interleaved on H   lambda [Npdep] HOST pointer, every lambda < 1
+ *   eta       overlap threshold of eq. 16: pair kept iff O_vv' >= eta; diagonal always kept
+ *   stream    cudaStream_t (as void*) or NULL
+ * Errors: BSE_EINVAL (null pointer, non-positive size, lambda >= 1, eta < 0, sphere does not fit: R >= n/2,
+ * Npdep > 2(Npw_h-1)), BSE_EUNSUPPORTED (non-cubic cell or grid, odd n, radix other than 2,3,5),
+ * BSE_ENOMEM, BSE_ECUDA. */
+int bse_create(bse_handle **h, const int grid[3], const double cell[9], double ecut,
+               int Nv, const double *u, int Npdep, const double *phi, const double *lambda,
+               double eta, unsigned flags, void *stream);
+
+/* Screen (eq. 16) -> pair list; then tau for every listed pair unless BSE_TAU_STREAM.  May be called again
+ * (rebuilds).  Errors: BSE_ENOMEM before any work is launched if the tau store does not fit. */
+int bse_build_tau(bse_handle *h);
+
+/* out[b,v] = P_c sum_v' tau_vv' a[b,v'] for B trial blocks.  a, out: DEVICE pointers, layout per
+ * BSE_VEC_* flag.  BSE_ESTATE if bse_build_tau has not run. */
+int bse_apply_k1x(bse_handle *h, const double *a, double *out, int B);
+
+/* Same with HOST pointers: copies a to the device, applies, copies out back, synchronises (the end-to-end
+ * call bench.py times as `e2e`). */
+int bse_apply_k1x_host(bse_handle *h, const double *a_host, double *out_host, int B);
+
+int bse_destroy(bse_handle *h);
+
+/* ---- read-only accessors (parity tests, input construction) ---- */
+int bse_npw_half(const bse_handle *h, long long *npw_h);
+int bse_gvectors(const bse_handle *h, int *mill /* HOST [Npw_h][3] */);
+int bse_num_pairs(const bse_handle *h, long long *P);
+int bse_get_pairs(const bse_handle *h, int *pairs /* HOST [P][2], lexicographic, v<=v' */);
+int bse_get_overlap(const bse_handle *h, double *O /* HOST [Nv][Nv], eq. 16 */);
+/* tau of pairs [first, first+count) into a DEVICE buffer; layout BSE_TAU_REAL ([count][N] doubles) or
+ * BSE_TAU_PW ([count][Npw_h] complex).  Works in every storage mode (recomputes if needed). */
+int bse_get_tau(bse_handle *h, long long first, long long count, double *dst, unsigned layout);
+
+/* ---- measurement helpers ---- */
+/* Per-stage device time (CUDA events on the library's stream).  enable != 0 switches recording on (adds a
+ * host sync per call).  Stage indices: BSE_ST_*; ms and launches are arrays of BSE_ST_COUNT, accumulated since
+ * the last bse_profile_reset. */
+enum { BSE_ST_SCREEN = 0, BSE_ST_PAIRLIST, BSE_ST_FWD_PLANE, BSE_ST_FWD_STICK, BSE_ST_PROJECT, BSE_ST_BACKPROJECT,
+       BSE_ST_INV_STICK, BSE_ST_INV_PLANE, BSE_ST_ACCUM, BSE_ST_PC_OVERLAP, BSE_ST_PC_UPDATE, BSE_ST_COUNT };
+int bse_profile_enable(bse_handle *h, int enable);
+int bse_profile_reset(bse_handle *h);
+int bse_profile_get(const bse_handle *h, double *ms /* [BSE_ST_COUNT] */, long long *launches /* [BSE_ST_COUNT] */);
+const char *bse_stage_name(int stage);
+
+/* FP64 peak probe: runs a dependent-free DMMA (mma.sync m8n8k4 f64) chain and a DFMA chain on every SM and
+ * returns the achieved TFLOP/s of each (the roofline denominators for the dense contractions). */
+int bse_probe_fp64_peak(double *dmma_tflops, double *dfma_tflops, void *stream);
+
+const char *bse_last_error(void);
+const char *bse_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BSE_H */

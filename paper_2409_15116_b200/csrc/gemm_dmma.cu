@@ -1,0 +1,246 @@
+// FP64 tensor-core (DMMA, mma.sync.m8n8k4.f64) GEMMs for the dense contractions of the path:
+//   a1  screen          M_vw   = sum_r u_v^2 u_w^2                       (eq. 16)   dot form, split-K
+//   a5  PDEP projection c_{a,p}= 2 sum_{H\0} Re(conj phi_a x_p)          (eq. 11)   dot form, split-K
+//   a7  back-projection y_p(G) = sum_a phi_a(G) f_a c_{a,p}, fused a8    (eq. 9, 11)              NN form
+//   a11 P_c             S = dV acc u^T (dot form), out = acc - S u (NN)
+// tcgen05.mma has no f64 kind on sm_100a, so the FP64 tensor path is the warp-level DMMA; operands are staged
+// with cp.async (LDGSTS) through a 3-stage shared-memory ring.  CTA tile 64 x 64 x 16, 4 warps of 32 x 32.
+#include "bse_internal.h"
+
+namespace {
+
+constexpr int BM = 64, BN = 64, BK = 16, STAGES = 3, THREADS = 128;
+constexpr int LDK = BK + 4;    // K-major tile row stride (doubles): conflict-free fragment reads
+constexpr int LDN = BN + 4;    // N-major tile row stride
+constexpr int A_TILE = BM * LDK;
+constexpr int B_TILE_K = BN * LDK;
+constexpr int B_TILE_N = BK * LDN;
+
+// 16-byte cp.async that reads only `sz` (0, 8 or 16) bytes from global and zero-fills the rest
+__device__ __forceinline__ void cp_async16(void *smem, const void *gmem, int sz) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s), "l"(gmem), "r"(sz));
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int N>
+__device__ __forceinline__ void cp_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N)); }
+
+__device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n"
+                 : "+d"(c0), "+d"(c1)
+                 : "d"(a), "d"(b));
+}
+
+// load a K-major tile: rows [r0, r0+64) of a [rows][K] matrix, k in [k0, k0+16) -> smem [64][LDK]
+__device__ __forceinline__ void load_tile_k(double *sm, const double *g, long long ld, int rows, int r0,
+                                            long long k0, long long kend) {
+    // 64 rows x 8 chunks of 16 B = 512 chunks, 128 threads -> 4 each
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int c = threadIdx.x + i * THREADS;
+        const int r = c >> 3, kc = (c & 7) * 2;
+        const long long left = kend - (k0 + kc);
+        const bool ok = (r0 + r < rows) && (left > 0);
+        const double *src = ok ? g + (long long)(r0 + r) * ld + k0 + kc : g;
+        cp_async16(sm + r * LDK + kc, src, ok ? (left >= 2 ? 16 : 8) : 0);
+    }
+}
+// load an N-major tile: k rows [k0,k0+16) of a [K][N] matrix, columns [c0, c0+64) -> smem [16][LDN]
+__device__ __forceinline__ void load_tile_n(double *sm, const double *g, long long ld, long long cols, long long c0,
+                                            int k0, int kend) {
+    // 16 rows x 32 chunks = 512 chunks
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int c = threadIdx.x + i * THREADS;
+        const int r = c >> 5, cc = (c & 31) * 2;
+        const long long left = cols - (c0 + cc);
+        const bool ok = (k0 + r < kend) && (left > 0);
+        const double *src = ok ? g + (long long)(k0 + r) * ld + c0 + cc : g;
+        cp_async16(sm + r * LDN + cc, src, ok ? (left >= 2 ? 16 : 8) : 0);
+    }
+}
+
+// BN_MAJOR = false: B is [N][K] (dot form).  true: B is [K][N] (NN form).
+// EPI_PARTIAL: store raw accumulators to part[z][M][Ntot]  (split-K, K range per blockIdx.z)
+// EPI_TAU    : C[m][n] = cs2[n>>1] * (Xin[m][n] + acc)
+// EPI_SUB    : C[m][n] = C[m][n] - acc
+template <bool BN_MAJOR, int EPI, bool SQA, bool SQB>
+__global__ void __launch_bounds__(THREADS)
+dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restrict__ B, long long ldb, int M,
+             long long Ntot, long long K, long long kchunk, double *__restrict__ C, long long ldc,
+             const double *__restrict__ Xin, const double *__restrict__ cs2) {
+    extern __shared__ __align__(16) double sm[];
+    double *As = sm;
+    double *Bs = sm + STAGES * A_TILE;
+    constexpr int B_TILE = BN_MAJOR ? B_TILE_N : B_TILE_K;
+
+    const int m0 = blockIdx.y * BM;
+    const long long n0 = (long long)blockIdx.x * BN;
+    const long long kbeg = (long long)blockIdx.z * kchunk;
+    const long long kend = (kbeg + kchunk < K) ? kbeg + kchunk : K;
+    const int nk = (int)((kend - kbeg + BK - 1) / BK);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wm = (warp >> 1) * 32, wn = (warp & 1) * 32;
+    const int lr = lane >> 2, lc = lane & 3;
+
+    double acc[4][4][2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    auto issue = [&](int kt) {
+        if (kt < nk) {
+            const int st = kt % STAGES;
+            const long long k0 = kbeg + (long long)kt * BK;
+            load_tile_k(As + st * A_TILE, A, lda, M, m0, k0, kend);
+            if (BN_MAJOR) load_tile_n(Bs + st * B_TILE, B, ldb, Ntot, n0, (int)k0, (int)kend);
+            else load_tile_k(Bs + st * B_TILE, B, ldb, (int)Ntot, (int)n0, k0, kend);
+        }
+        cp_commit();
+    };
+    issue(0);
+    issue(1);
+    for (int kt = 0; kt < nk; ++kt) {
+        cp_wait<STAGES - 2>();
+        __syncthreads();
+        issue(kt + STAGES - 1);
+        const double *as = As + (kt % STAGES) * A_TILE;
+        const double *bs = Bs + (kt % STAGES) * B_TILE;
+#pragma unroll
+        for (int kk = 0; kk < BK; kk += 4) {
+            double af[4], bf[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                af[i] = as[(wm + i * 8 + lr) * LDK + kk + lc];
+                if (SQA) af[i] *= af[i];
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                bf[j] = BN_MAJOR ? bs[(kk + lc) * LDN + wn + j * 8 + lr] : bs[(wn + j * 8 + lr) * LDK + kk + lc];
+                if (SQB) bf[j] *= bf[j];
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dmma(acc[i][j][0], acc[i][j][1], af[i], bf[j]);
+        }
+    }
+    cp_wait<0>();
+
+    // epilogue: thread holds C[row = lr][col = 2*lc, 2*lc+1] of each 8x8 tile
+    double *Cout = C;
+    if (EPI == EPI_PARTIAL) Cout = C + (long long)blockIdx.z * M * ldc;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int m = m0 + wm + i * 8 + lr;
+        if (m >= M) continue;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const long long nn = n0 + wn + j * 8 + 2 * lc;
+            if (nn >= Ntot) continue;     // Ntot even for every caller that reaches the vector store below
+            double v0 = acc[i][j][0], v1 = acc[i][j][1];
+            double *dst = Cout + (long long)m * ldc + nn;
+            if (EPI == EPI_TAU) {
+                const double2 x = *reinterpret_cast<const double2 *>(Xin + (long long)m * ldc + nn);
+                const double sc = cs2[nn >> 1];
+                v0 = sc * (x.x + v0);
+                v1 = sc * (x.y + v1);
+            } else if (EPI == EPI_SUB) {
+                const double2 x = *reinterpret_cast<const double2 *>(dst);
+                v0 = x.x - v0;
+                v1 = x.y - v1;
+            }
+            if (EPI == EPI_PARTIAL) {          // ldc may be odd here: scalar stores
+                dst[0] = v0;
+                if (nn + 1 < Ntot) dst[1] = v1;
+            } else if (nn + 1 < Ntot) {
+                *reinterpret_cast<double2 *>(dst) = make_double2(v0, v1);
+            } else {
+                dst[0] = v0;
+            }
+        }
+    }
+}
+
+// C[m][n] = alpha * colscale[n] * sum_z part[z][m][n], fixed order (deterministic)
+__global__ void splitk_reduce_kernel(const double *__restrict__ part, int splits, long long MN, int N,
+                                     double *__restrict__ C, long long ldc, double alpha,
+                                     const double *__restrict__ colscale) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= MN) return;
+    double s = 0.0;
+    for (int z = 0; z < splits; ++z) s += part[(long long)z * MN + i];
+    s *= alpha;
+    const long long m = i / N;
+    const int n = (int)(i - m * N);
+    if (colscale) s *= colscale[n];
+    C[m * ldc + n] = s;
+}
+
+constexpr int SMEM_DOT = STAGES * (A_TILE + B_TILE_K) * 8;
+constexpr int SMEM_NN = STAGES * (A_TILE + B_TILE_N) * 8;
+
+template <typename KernelT>
+int prep(KernelT k, int smem) {
+    BSE_CUDA(cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    return BSE_OK;
+}
+
+}  // namespace
+
+int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb, int M, int N, long long K,
+                 bool squareA, bool squareB, double *part, size_t part_bytes, double *C, long long ldc,
+                 double alpha, const double *colscale, cudaStream_t s) {
+    if (M <= 0 || N <= 0) return BSE_OK;
+    const int tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
+    const long long ksteps = (K + BK - 1) / BK;
+    long long splits = (2LL * 148 + (long long)tm * tn - 1) / ((long long)tm * tn);
+    if (splits > ksteps / 8) splits = ksteps / 8;
+    if (splits < 1) splits = 1;
+    const long long cap = (long long)(part_bytes / ((size_t)M * N * 8));
+    if (cap < 1) { bse_set_error("bse_gemm_dot: split-K workspace too small"); return BSE_ENOMEM; }
+    if (splits > cap) splits = cap;
+    long long kchunk = ((ksteps + splits - 1) / splits) * BK;
+    splits = (K + kchunk - 1) / kchunk;
+    dim3 grid(tn, tm, (unsigned)splits);
+    int rc;
+    if (squareA && squareB) {
+        auto k = dgemm_kernel<false, EPI_PARTIAL, true, true>;
+        if ((rc = prep(k, SMEM_DOT))) return rc;
+        k<<<grid, THREADS, SMEM_DOT, s>>>(A, lda, B, ldb, M, N, K, kchunk, part, N, nullptr, nullptr);
+    } else {
+        auto k = dgemm_kernel<false, EPI_PARTIAL, false, false>;
+        if ((rc = prep(k, SMEM_DOT))) return rc;
+        k<<<grid, THREADS, SMEM_DOT, s>>>(A, lda, B, ldb, M, N, K, kchunk, part, N, nullptr, nullptr);
+    }
+    BSE_CUDA(cudaGetLastError());
+    const long long MN = (long long)M * N;
+    splitk_reduce_kernel<<<(unsigned)((MN + 255) / 256), 256, 0, s>>>(part, (int)splits, MN, N, C, ldc, alpha, colscale);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, int M, long long N, int K, int epi,
+                const double *Xin, const double *colscale2, double *C, long long ldc, cudaStream_t s) {
+    if (M <= 0 || N <= 0) return BSE_OK;
+    const int tm = (M + BM - 1) / BM;
+    const long long tn = (N + BN - 1) / BN;
+    dim3 grid((unsigned)tn, tm, 1);
+    int rc;
+    if (epi == EPI_TAU) {
+        auto k = dgemm_kernel<true, EPI_TAU, false, false>;
+        if ((rc = prep(k, SMEM_NN))) return rc;
+        k<<<grid, THREADS, SMEM_NN, s>>>(A, lda, B, ldb, M, N, K, K, C, ldc, Xin, colscale2);
+    } else if (epi == EPI_SUB) {
+        auto k = dgemm_kernel<true, EPI_SUB, false, false>;
+        if ((rc = prep(k, SMEM_NN))) return rc;
+        k<<<grid, THREADS, SMEM_NN, s>>>(A, lda, B, ldb, M, N, K, K, C, ldc, nullptr, nullptr);
+    } else {
+        bse_set_error("bse_gemm_nn: bad epilogue");
+        return BSE_EINVAL;
+    }
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}

@@ -1,0 +1,214 @@
+"""GPU parity: CUDA path (through the C ABI) vs the CPU oracle, element by element, same seeded inputs.
+
+Bar (BASELINE.json north_star): surviving-pair list bit-exact; tau and K1x output within 1e-10 relative L2.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import bse_oracle as orc                      # noqa: E402
+from paper_2409_15116_b200 import workloads as wl         # noqa: E402
+
+TOL = 1e-10
+
+
+def _bse():
+    from paper_2409_15116_b200 import bse
+    return bse
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(np.asarray(b)))
+
+
+class Gpu:
+    """Device-resident inputs + handle for one workload."""
+
+    def __init__(self, w, flags=0):
+        bse = _bse()
+        self.bse, self.w = bse, w
+        dev = torch.device("cuda:0")
+        self.u = torch.from_numpy(w.u).to(dev)
+        phi = np.ascontiguousarray(w.phi).view(np.float64)          # interleaved (re, im)
+        self.phi = torch.from_numpy(phi).to(dev)
+        self.h = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, self.u, w.phi.shape[0], self.phi, w.lam, w.eta, flags)
+
+    def build(self):
+        self.bse.bse_build_tau(self.h)
+        torch.cuda.synchronize()
+        return self.bse.bse_get_pairs(self.h)
+
+    def tau_r(self, first, count):
+        dst = torch.empty((count, self.w.N), dtype=torch.float64, device="cuda:0")
+        self.bse.bse_get_tau(self.h, first, count, dst, self.bse.BSE_TAU_REAL)
+        torch.cuda.synchronize()
+        return dst.cpu().numpy()
+
+    def tau_g(self, first, count):
+        npw_h = self.bse.bse_npw_half(self.h)
+        dst = torch.empty((count, npw_h, 2), dtype=torch.float64, device="cuda:0")
+        self.bse.bse_get_tau(self.h, first, count, dst, self.bse.BSE_TAU_PW)
+        torch.cuda.synchronize()
+        return dst.cpu().numpy().view(np.complex128)[..., 0]
+
+    def apply(self, a):
+        a_d = torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+        out = torch.empty_like(a_d)
+        self.bse.bse_apply_k1x(self.h, a_d, out, a.shape[0])
+        torch.cuda.synchronize()
+        return out.cpu().numpy()
+
+    def close(self):
+        self.bse.bse_destroy(self.h)
+
+
+def _check_full(w, flags=0, check_g=True):
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    pairs_ref, O = orc.screen_pairs(w.u, w.eta)
+    assert orc.screen_margin(O, w.eta) > 1e-9, "workload violates the screen guard band (S10)"
+    g = Gpu(w, flags)
+    try:
+        assert np.array_equal(g.bse.bse_gvectors(g.h), w.mill)
+        pairs = g.build()
+        assert pairs.dtype == np.int32 and np.array_equal(pairs, pairs_ref)          # bit-exact list
+        O_gpu = g.bse.bse_get_overlap(g.h, w.Nv)
+        assert np.abs(O_gpu - O).max() < 1e-12
+        tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs_ref, want="r")
+        tau = g.tau_r(0, len(pairs))
+        assert rel(tau, tau_ref) <= TOL
+        worst = max(rel(tau[p], tau_ref[p]) for p in range(len(pairs)))
+        assert worst <= 10 * TOL
+        if check_g:
+            tg_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs_ref, want="G")
+            assert rel(g.tau_g(0, len(pairs)), tg_ref) <= TOL
+        a = w.a_real()
+        out_ref = orc.apply_k1x_real(tab, w.u, pairs_ref, tau_ref, a)
+        out = g.apply(a)
+        assert rel(out, out_ref) <= TOL
+        # P_c did its job on the GPU result: <u_w|out> = 0
+        ov = tab.dV * np.einsum("wr,bvr->bvw", w.u, out)
+        assert np.abs(ov).max() < 1e-11 * np.abs(out).max() * tab.N ** 0.5
+        return out
+    finally:
+        g.close()
+
+
+def test_cfg1_full_all_modes():
+    w = wl.make(1)
+    bse = _bse()
+    o0 = _check_full(w, bse.BSE_TAU_REAL)
+    o1 = _check_full(w, bse.BSE_TAU_PW, check_g=False)
+    o2 = _check_full(w, bse.BSE_TAU_STREAM, check_g=False)
+    assert rel(o1, o0) < 1e-12 and rel(o2, o0) < 1e-12
+
+
+@pytest.mark.parametrize("n,L,ecut,Nv,Npdep,B,eta", [
+    (12, 9.0, 3.0, 5, 7, 3, 0.05),        # odd Nv / Npdep / B, radix 4*3, screened
+    (20, 12.0, 4.0, 6, 9, 1, 0.0),        # radix 5
+    (30, 14.0, 5.0, 4, 16, 2, 0.02),      # radices 2,3,5
+    (24, 10.0, 8.0, 9, 33, 16, 0.9),      # big threshold: (nearly) only diagonal pairs, B = 16
+])
+def test_small_shapes_and_edges(n, L, ecut, Nv, Npdep, B, eta):
+    cfg = wl.Config("edge", L, n, Nv, Npdep, ecut, 1.3, 0.8, 3.0, eta, B, "random", seed=100 + n)
+    w = wl.make(cfg=cfg)
+    _check_full(w)
+
+
+def test_cfg2_reduced_full_check():
+    # config-2 grid and sphere (64^3, 15895 PWs, several GEMM tiles and a ragged K tail), fewer orbitals
+    w = wl.make(2, Nv=12, Npdep=40, B=2)
+    for flags in (0, _bse().BSE_TAU_PW, _bse().BSE_TAU_STREAM):
+        _check_full(w, flags, check_g=(flags == 0))
+
+
+def _sampled_check(w, n_pairs, rows, flags=0):
+    """Full-size config: bit-exact list; tau on sampled pairs; K1x on sampled rows v (all blocks)."""
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    pairs_ref, O = orc.screen_pairs(w.u, w.eta)
+    assert orc.screen_margin(O, w.eta) > 1e-9
+    g = Gpu(w, flags)
+    try:
+        pairs = g.build()
+        assert np.array_equal(pairs, pairs_ref)
+        P = len(pairs)
+        rng = np.random.default_rng(5)
+        sample = sorted(set(rng.choice(P, size=min(n_pairs, P), replace=False).tolist()) | {0, P - 1})
+        phiS = tab.expand_H_to_S(w.phi)
+        for p in sample:
+            v, x = pairs[p]
+            ref = orc.tau_r(tab, w.u[v], w.u[x], phiS, w.lam)
+            assert rel(g.tau_r(p, 1)[0], ref) <= TOL
+        a = w.a_real()
+        out = g.apply(a)
+        index = {(int(v), int(x)): p for p, (v, x) in enumerate(pairs)}
+        for v in rows:
+            acc = np.zeros((a.shape[0], tab.N))
+            for x in range(w.Nv):
+                key = (min(v, x), max(v, x))
+                if key in index:
+                    t = orc.tau_r(tab, w.u[key[0]], w.u[key[1]], phiS, w.lam)
+                    acc += t[None, :] * a[:, x, :]
+            ref = np.array([orc.p_c_real(tab, w.u, acc[b]) for b in range(a.shape[0])])
+            assert rel(out[:, v, :], ref) <= TOL
+        return P
+    finally:
+        g.close()
+
+
+def test_cfg2_full_size_sampled():
+    w = wl.make(2)
+    P = _sampled_check(w, n_pairs=6, rows=[0, 37])
+    assert 64 <= P < 2080
+
+
+def test_error_paths():
+    bse = _bse()
+    w = wl.make(cfg=wl.Config("e", 9.0, 12, 4, 6, 3.0, 1.3, 0.8, 3.0, 0.0, 2, "random", seed=3))
+    g = Gpu(w)
+    try:
+        a = torch.zeros((1, w.Nv, w.N), dtype=torch.float64, device="cuda:0")
+        with pytest.raises(bse.BseError) as e:
+            bse.bse_apply_k1x(g.h, a, torch.empty_like(a), 1)
+        assert e.value.code == bse.BSE_ESTATE
+        g.build()
+        with pytest.raises(bse.BseError) as e:
+            bse.bse_apply_k1x(g.h, a, a, 1)
+        assert e.value.code == bse.BSE_EINVAL
+    finally:
+        g.close()
+    lam_bad = w.lam.copy()
+    lam_bad[0] = 1.0
+    u = torch.from_numpy(w.u).cuda()
+    phi = torch.from_numpy(np.ascontiguousarray(w.phi).view(np.float64)).cuda()
+    for kwargs, code in [
+        (dict(lam=lam_bad), bse.BSE_EINVAL),
+        (dict(ecut=40.0), bse.BSE_EINVAL),                 # sphere does not fit
+        (dict(eta=-1.0), bse.BSE_EINVAL),
+        (dict(grid=[12, 12, 10]), bse.BSE_EUNSUPPORTED),
+        (dict(flags=bse.BSE_VEC_PW), bse.BSE_EUNSUPPORTED),
+    ]:
+        args = dict(grid=[w.n] * 3, ecut=w.ecut, lam=w.lam, eta=0.0, flags=0)
+        args.update(kwargs)
+        with pytest.raises(bse.BseError) as e:
+            bse.bse_create(args["grid"], w.cell, args["ecut"], w.Nv, u, w.phi.shape[0], phi, args["lam"], args["eta"], args["flags"])
+        assert e.value.code == code
+
+
+def test_host_pointer_entry_points():
+    bse = _bse()
+    w = wl.make(cfg=wl.Config("h", 9.0, 12, 4, 6, 3.0, 1.3, 0.8, 3.0, 0.0, 2, "random", seed=4))
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    phi = np.ascontiguousarray(w.phi).view(np.float64)
+    h = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, w.u, w.phi.shape[0], phi, w.lam, w.eta, bse.BSE_PTR_HOST)
+    try:
+        bse.bse_build_tau(h)
+        pairs = bse.bse_get_pairs(h)
+        a = np.ascontiguousarray(w.a_real())
+        out = np.empty_like(a)
+        bse.bse_apply_k1x_host(h, a, out, a.shape[0])
+        tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs, want="r")
+        assert rel(out, orc.apply_k1x_real(tab, w.u, pairs, tau_ref, a)) <= TOL
+    finally:
+        bse.bse_destroy(h)
