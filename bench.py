@@ -1,0 +1,367 @@
+#!/usr/bin/env python
+"""bench.py - throughput of the screened-exchange hot path on B200 (one line of JSON on stdout).
+
+A "step" = one pass of the whole hot path over one synthetic workload: bse_build_tau (screen, pair list,
+tau for every surviving pair) followed by bse_apply_k1x on the config's B trial blocks.
+  value  = screened pair integrals / s  (P / device time of bse_build_tau, screen included), inputs resident in HBM
+  k1x    = K1x applies / s              (B / device time of bse_apply_k1x)
+  e2e    = the same two through the C ABI with HOST buffers (pinned): H2D of u, phi, a and D2H of out inside
+           the timed region.
+  roofline     = the dominant kernel (largest share of the step) against the measured HBM / FP64 peak
+  cpu_baseline = the CPU oracle (oracle/bse_oracle.py, as it stands) on a bounded sample of the same workload
+
+`--impl reference` times the oracle alone on the host cores (rank 0 only).
+Multi-GPU: the path has no exchange step at this scope ("replicas only"): with --gpus N every rank
+runs an independent replica of the workload; value = pairs of all ranks / max-over-ranks time ("weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "screened pair integrals/s (tau build incl. screen; K1x applies/s beside it), fp64, B200"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i] == "Active"})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def stage_model(w, P, B, npw_h, NS):
+    """Algorithmic flops and compulsory HBM bytes per stage for one step."""
+    n, N, Nv, Npd = w.n, w.N, w.Nv, w.phi.shape[0]
+    z = 16 * n * NS
+    g = 16 * npw_h
+    fft_plane = 2.5 * n * n * np.log2(n) * n + 5 * n * np.log2(n) * (w_cols(w)) * n     # rows (real) + kept columns
+    fft_stick = 5 * n * np.log2(n) * NS
+    return {
+        "screen_syrk": dict(flops=Nv * (Nv + 1) * N, bytes=8 * Nv * N, bound="tensor"),
+        "pair_list": dict(flops=0, bytes=8 * Nv * Nv, bound="hbm"),
+        "fwd_plane": dict(flops=P * fft_plane, bytes=P * (8 * N + z), bound="hbm"),
+        "fwd_stick": dict(flops=P * fft_stick, bytes=P * (z + g), bound="hbm"),
+        "pdep_project": dict(flops=2 * P * Npd * 2 * npw_h, bytes=P * g + Npd * g, bound="tensor"),
+        "pdep_backproject": dict(flops=2 * P * Npd * 2 * npw_h, bytes=2 * P * g + Npd * g, bound="tensor"),
+        "inv_stick": dict(flops=P * fft_stick, bytes=P * (g + z), bound="hbm"),
+        "inv_plane": dict(flops=P * fft_plane, bytes=P * (z + 8 * N), bound="hbm"),
+        "k1x_accumulate": dict(flops=2 * B * N * (2 * P - Nv), bytes=8 * N * (P + 2 * B * Nv), bound="hbm"),
+        "pc_overlap": dict(flops=2 * B * Nv * Nv * N, bytes=8 * N * (B * Nv + Nv), bound="tensor"),
+        "pc_update": dict(flops=2 * B * Nv * Nv * N, bytes=8 * N * (2 * B * Nv + Nv), bound="tensor"),
+    }
+
+
+def w_cols(w):
+    from paper_2409_15116_b200 import workloads as wl
+    return int(np.floor(np.sqrt(wl.msq_max(w.L, w.ecut)))) + 1
+
+
+def oracle_sample(w, n_pairs, seconds_cap=30.0):
+    """Time the oracle, as it stands, on a bounded sample: screen on the full u, then tau for n_pairs pairs."""
+    import psutil
+    from oracle import bse_oracle as orc
+    proc = psutil.Process()
+    c0 = proc.cpu_times()
+    t0 = time.perf_counter()
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    pairs, _ = orc.screen_pairs(w.u, w.eta)
+    t_screen = time.perf_counter() - t0
+    phiS = tab.expand_H_to_S(w.phi)
+    rng = np.random.default_rng(11)
+    sel = rng.choice(len(pairs), size=min(n_pairs, len(pairs)), replace=False)
+    t1 = time.perf_counter()
+    done = 0
+    taus = {}
+    for p in sel:
+        v, x = pairs[p]
+        taus[int(p)] = orc.tau_r(tab, w.u[v], w.u[x], phiS, w.lam)
+        done += 1
+        if time.perf_counter() - t1 > seconds_cap:
+            break
+    t_tau = time.perf_counter() - t1
+    # one K1x output row for one block: accumulate the sampled taus + P_c (bounded)
+    t2 = time.perf_counter()
+    a0 = np.zeros(tab.N)
+    for p, t in taus.items():
+        a0 += t * w.u[pairs[p][1]]
+    orc.p_c_real(tab, w.u, a0)
+    t_row = time.perf_counter() - t2
+    wall = time.perf_counter() - t0
+    c1 = proc.cpu_times()
+    cores = max(1, int(round(((c1.user - c0.user) + (c1.system - c0.system)) / wall)))
+    per_pair = t_tau / max(done, 1)
+    P = len(pairs)
+    est_build = t_screen + per_pair * P
+    return dict(pairs_per_s=P / est_build, per_pair_s=per_pair, screen_s=t_screen, sampled=done, P=P, cores=cores,
+                row_s=t_row)
+
+
+def run_reference(args, rank):
+    if rank != 0:
+        return
+    from paper_2409_15116_b200 import workloads as wl
+    w = wl.make(args.config)
+    vals = []
+    info = None
+    per_step_pairs = 3
+    for i in range(args.warmup + args.steps):
+        info = oracle_sample(w, per_step_pairs, seconds_cap=20.0)
+        if i >= args.warmup:
+            vals.append(info["pairs_per_s"])
+    v = float(np.mean(vals))
+    sample = (f"per step: eq.16 screen on the full u + tau for {per_step_pairs} of {info['P']} surviving pairs, "
+              f"extrapolated per pair")
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "pairs/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * info["P"] / v, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.config - 1}] (cfg{args.config})"},
+            "cpu_baseline": {"value": v, "unit": "pairs/s", "cores": info["cores"], "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": "pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-based); 2 = configs[1]")
+    ap.add_argument("--tau", default="real", choices=["real", "pw", "stream"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2409_15116_b200 import bse, workloads as wl
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = wl.make(args.config)
+    B = w.a_pw.shape[0]
+    a_host = torch.from_numpy(np.ascontiguousarray(w.a_real())).pin_memory()
+    u_host = torch.from_numpy(w.u).pin_memory()
+    phi_host = torch.from_numpy(np.ascontiguousarray(w.phi).view(np.float64)).pin_memory()
+    out_host = torch.empty_like(a_host).pin_memory()
+    u_d, phi_d, a_d = u_host.to(dev), phi_host.to(dev), a_host.to(dev)
+    out_d = torch.empty_like(a_d)
+    flags = {"real": bse.BSE_TAU_REAL, "pw": bse.BSE_TAU_PW, "stream": bse.BSE_TAU_STREAM}[args.tau]
+    stream = torch.cuda.current_stream().cuda_stream
+    h = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u_d, w.phi.shape[0], phi_d, w.lam, w.eta, flags, stream)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    def step(timed):
+        flush.fill_(1)                                                  # L2 flush, outside the timed events
+        e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        e0.record()
+        bse.bse_build_tau(h)
+        e1.record()
+        bse.bse_apply_k1x(h, a_d, out_d, B)
+        e2.record()
+        if timed:
+            e2.synchronize()
+            return e0.elapsed_time(e1), e1.elapsed_time(e2)
+        return None
+
+    for _ in range(args.warmup):
+        step(False)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    bse.bse_profile_reset(h)
+    t_build, t_apply = [], []
+    wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        tb, ta = step(True)
+        t_build.append(tb)
+        t_apply.append(ta)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    wall = time.perf_counter() - wall0
+    clocks = sampler.stop() if rank == 0 else None
+    prof_counts = bse.bse_profile_get(h)
+    P = bse.bse_num_pairs(h)
+    tb_ms, ta_ms = float(np.mean(t_build)), float(np.mean(t_apply))
+    if world > 1:
+        t = torch.tensor([tb_ms, ta_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        tb_ms, ta_ms = t.tolist()
+    launches = sum(prof_counts[s][1] * k for s, k in zip(bse.STAGES, bse.KERNELS_PER_STAGE))
+
+    # ---- per-stage device times (CUDA events on the library's stream, one extra profiled pass per step) ----
+    bse.bse_profile_enable(h, True)
+    bse.bse_profile_reset(h)
+    nprof = max(3, min(args.steps, 5))
+    for _ in range(nprof):
+        step(False)
+    torch.cuda.synchronize()
+    prof = bse.bse_profile_get(h)
+    bse.bse_profile_enable(h, False)
+    npw_h = bse.bse_npw_half(h)
+    NS = None
+    # NS (number of half sticks) recomputed here from the sphere definition for the byte model
+    R = w_cols(w) - 1
+    mx = wl.msq_max(w.L, w.ecut)
+    NS = sum(1 for m2 in range(-R, R + 1) for m3 in range(0, R + 1)
+             if m2 * m2 + m3 * m3 <= mx and not (m3 == 0 and m2 < 0))
+    model = stage_model(w, P, B, npw_h, NS)
+    hbm_gbs, peak_src = load_peaks()
+    dmma_tf, dfma_tf = bse.bse_probe_fp64_peak(stream)
+    stages = {}
+    for s in bse.STAGES:
+        ms = prof[s][0] / nprof
+        m = model[s]
+        t_f = m["flops"] / (dmma_tf * 1e12 if m["bound"] == "tensor" else dfma_tf * 1e12)
+        t_b = m["bytes"] / (hbm_gbs * 1e9)
+        stages[s] = {"ms": round(ms, 4), "launches_per_step": prof[s][1] / nprof * bse.KERNELS_PER_STAGE[bse.STAGES.index(s)],
+                     "gflop": round(m["flops"] / 1e9, 3), "mbytes": round(m["bytes"] / 1e6, 2),
+                     "roof_ms": round(1e3 * max(t_f, t_b), 4),
+                     "frac": round(max(t_f, t_b) * 1e3 / ms, 4) if ms > 0 else None}
+    top = max(bse.STAGES, key=lambda s: stages[s]["ms"])
+    mt = model[top]
+    ms_top = stages[top]["ms"]
+    n_launch_top = max(1.0, prof[top][1] / nprof)
+    t_f = mt["flops"] / (dmma_tf * 1e12)
+    t_b = mt["bytes"] / (hbm_gbs * 1e9)
+    if mt["bound"] == "tensor" and t_f >= t_b:
+        roof = {"bound": "tensor", "achieved": mt["flops"] / (ms_top * 1e-3) / 1e12, "peak": dmma_tf, "unit": "TFLOP/s",
+                "peak_source": "fp64 DMMA chain measured live by bse_probe_fp64_peak (bf16-derived alternative in DESIGN.md)"}
+    else:
+        roof = {"bound": "hbm", "achieved": mt["bytes"] / (ms_top * 1e-3) / 1e9, "peak": hbm_gbs, "unit": "GB/s",
+                "peak_source": peak_src}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["kernel"] = top
+    roof["launches_per_step"] = n_launch_top
+    roof["ms_per_launch"] = ms_top / n_launch_top
+    roof["traffic"] = None
+    tot_f = sum(m["flops"] for m in model.values())
+    tot_b = sum(m["bytes"] for m in model.values())
+    pipe_roof_ms = 1e3 * max(tot_f / (dmma_tf * 1e12), tot_b / (hbm_gbs * 1e9))
+    pipeline = {"roof_ms": round(pipe_roof_ms, 4), "measured_ms": round(tb_ms + ta_ms, 4),
+                "frac": round(pipe_roof_ms / (tb_ms + ta_ms), 4), "gflop": round(tot_f / 1e9, 2),
+                "mbytes": round(tot_b / 1e6, 1), "fp64_dmma_tflops": round(dmma_tf, 2), "fp64_dfma_tflops": round(dfma_tf, 2)}
+
+    # ---- end to end through the C ABI with host (pinned) buffers ----
+    e2e_build, e2e_apply = [], []
+    for i in range(2 + 3):
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        hh = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u_host, w.phi.shape[0], phi_host, w.lam, w.eta,
+                            flags | bse.BSE_PTR_HOST, stream)
+        bse.bse_build_tau(hh)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        bse.bse_apply_k1x_host(hh, a_host, out_host, B)
+        t2 = time.perf_counter()
+        bse.bse_destroy(hh)
+        if i >= 2:
+            e2e_build.append(t1 - t0)
+            e2e_apply.append(t2 - t1)
+    e2e_b, e2e_a = float(np.mean(e2e_build)), float(np.mean(e2e_apply))
+    if world > 1:
+        t = torch.tensor([e2e_b, e2e_a], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_b, e2e_a = t.tolist()
+    h2d = u_host.numel() * 8 + phi_host.numel() * 8 + a_host.numel() * 8
+    d2h = out_host.numel() * 8 + 8
+
+    bse.bse_destroy(h)
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1 or (not args.no_cpu_baseline and rank == 0 and args.gpus == 1):
+        info = oracle_sample(w, 40, seconds_cap=20.0)
+        cpu = {"value": info["pairs_per_s"], "unit": "pairs/s", "cores": info["cores"], "kind": "oracle",
+               "sample": f"eq.16 screen on the full u ({info['screen_s']:.1f} s) + tau for {info['sampled']} of {info['P']} "
+                         f"surviving pairs ({info['per_pair_s']:.3f} s/pair), extrapolated to all pairs",
+               "k1x_row_s": info["row_s"]}
+
+    line = {
+        "metric": METRIC, "value": world * P / (tb_ms * 1e-3), "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": tb_ms + ta_ms, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] (cfg{args.config}): grid {w.n}^3, Nv={w.Nv}, "
+                               f"Npdep={w.phi.shape[0]}, Npw_h={npw_h}, eta={w.eta}, P={P} surviving pairs, B={B}",
+                   "tau_storage": args.tau, "vec_layout": "real", "parallelism": "replicas" if world > 1 else "1gpu",
+                   "l2": "512 MB buffer written between timed steps (L2 flush); inputs also exceed L2"},
+        "k1x_applies_per_s": world * B / (ta_ms * 1e-3), "build_ms": tb_ms, "apply_ms": ta_ms, "pairs": P,
+        "gpu_launches": int(launches), "wall_s_timed_region": wall,
+        "clocks": clocks,
+        "e2e": {"value": world * P / e2e_b, "unit": "pairs/s", "k1x_applies_per_s": world * B / e2e_a,
+                "build_ms": 1e3 * e2e_b, "apply_ms": 1e3 * e2e_a, "h2d_bytes_per_step": int(h2d),
+                "d2h_bytes_per_step": int(d2h),
+                "what": "bse_create(BSE_PTR_HOST: H2D of u, phi) + bse_build_tau, then bse_apply_k1x_host (H2D a, D2H out); pinned host buffers"},
+        "roofline": roof, "pipeline_roofline": pipeline, "stages": stages, "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
