@@ -376,21 +376,25 @@ extern "C" int bse_build_tau(bse_handle *h) {
     { StageTimer t(h, BSE_ST_PAIRLIST);
       if ((rc = bse_launch_pairlist(h))) return rc; }
     const unsigned mode = h->flags & BSE_TAU_MASK;
-    cudaFree(h->tau_r); h->tau_r = nullptr;
-    cudaFree(h->tau_g); h->tau_g = nullptr;
     if (mode != BSE_TAU_STREAM) {
         const size_t need = (mode == BSE_TAU_REAL) ? (size_t)h->P * h->N * 8 : (size_t)h->P * h->fft.npw_h * 16;
-        size_t free_b = 0, total_b = 0;
-        cudaMemGetInfo(&free_b, &total_b);
-        if (need + ((size_t)256 << 20) > free_b) {
-            char msg[160];
-            snprintf(msg, sizeof msg, "tau store needs %.2f GB, %.2f GB free: use BSE_TAU_PW or BSE_TAU_STREAM",
-                     need / 1e9, free_b / 1e9);
-            bse_set_error(msg);
-            return BSE_ENOMEM;
+        if (need > h->tau_bytes) {            // grow-only store: a rebuild with the same list allocates nothing
+            cudaFree(h->tau_r); h->tau_r = nullptr;
+            cudaFree(h->tau_g); h->tau_g = nullptr;
+            h->tau_bytes = 0;
+            size_t free_b = 0, total_b = 0;
+            cudaMemGetInfo(&free_b, &total_b);
+            if (need + ((size_t)256 << 20) > free_b) {
+                char msg[160];
+                snprintf(msg, sizeof msg, "tau store needs %.2f GB, %.2f GB free: use BSE_TAU_PW or BSE_TAU_STREAM",
+                         need / 1e9, free_b / 1e9);
+                bse_set_error(msg);
+                return BSE_ENOMEM;
+            }
+            if (mode == BSE_TAU_REAL) BSE_CUDA(cudaMalloc(&h->tau_r, need));
+            else BSE_CUDA(cudaMalloc(&h->tau_g, need));
+            h->tau_bytes = need;
         }
-        if (mode == BSE_TAU_REAL) BSE_CUDA(cudaMalloc(&h->tau_r, std::max<size_t>(need, 8)));
-        else BSE_CUDA(cudaMalloc(&h->tau_g, std::max<size_t>(need, 16)));
         for (long long p0 = 0; p0 < h->P; p0 += h->Pb) {
             const int cnt = (int)std::min<long long>(h->Pb, h->P - p0);
             if (mode == BSE_TAU_REAL) rc = run_pair_batch(h, p0, cnt, h->T, h->tau_r + p0 * h->N);

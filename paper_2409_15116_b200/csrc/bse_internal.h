@@ -63,6 +63,7 @@ struct bse_handle {
     // tau store
     double *tau_r = nullptr;         // [P][N]
     double2 *tau_g = nullptr;        // [P][npw_h]
+    size_t tau_bytes = 0;            // capacity of the store (grow-only)
     // workspaces (sized for a pair batch)
     long long Pb = 0;                // pair-batch capacity
     double2 *Z = nullptr;            // [Pb][n][NS]

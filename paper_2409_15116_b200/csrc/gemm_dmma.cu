@@ -184,7 +184,13 @@ constexpr int SMEM_NN = STAGES * (A_TILE + B_TILE_N) * 8;
 
 template <typename KernelT>
 int prep(KernelT k, int smem) {
+    // all instantiations share one function-pointer type, so remember the pointers already prepared
+    static const void *done[16];
+    static int ndone = 0;
+    for (int i = 0; i < ndone; ++i)
+        if (done[i] == (const void *)k) return BSE_OK;
     BSE_CUDA(cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    if (ndone < 16) done[ndone++] = (const void *)k;
     return BSE_OK;
 }
 
