@@ -54,39 +54,12 @@ int build_fft_plan(bse_handle *h) {
     FftPlan &pl = h->fft;
     const int n = h->n;
     pl.n = n;
-    pl.ld = n + 1;
-    // radix list: 4s first, then 2, 3, 5
-    int rem = n, np = 0;
-    while (rem % 4 == 0) { pl.radix[np++] = 4; rem /= 4; }
-    while (rem % 2 == 0) { pl.radix[np++] = 2; rem /= 2; }
-    while (rem % 3 == 0) { pl.radix[np++] = 3; rem /= 3; }
-    while (rem % 5 == 0) { pl.radix[np++] = 5; rem /= 5; }
-    if (rem != 1 || np > BSE_MAX_RADIX_PASSES) {
-        bse_set_error("grid size must factor into 2, 3, 5");
-        return BSE_EUNSUPPORTED;
-    }
-    pl.npass = np;
-    for (int i = np; i < BSE_MAX_RADIX_PASSES; ++i) pl.radix[i] = 1;
-    // position <-> frequency after the in-place DIF passes
-    std::vector<int> rev(n), pos(n);
-    for (int p = 0; p < n; ++p) {
-        int k = 0, mult = 1, Lc = n, q = p;
-        for (int i = 0; i < np; ++i) {
-            const int m = Lc / pl.radix[i];
-            const int d = q / m;
-            q -= d * m;
-            k += d * mult;
-            mult *= pl.radix[i];
-            Lc = m;
-        }
-        rev[p] = k;
-        pos[k] = p;
-    }
+    int rc;
+    if ((rc = bse_fft_select(pl))) return rc;
     const int msq = h->msq_max;
     const int R = (int)std::floor(std::sqrt((double)msq) + 1e-9);
     pl.R = R;
     pl.W = R + 1;
-    const int W = pl.W, ld = pl.ld;
     // half sphere H in the normative order
     struct M3 { int m1, m2, m3; long long key; };
     std::vector<M3> H;
@@ -105,63 +78,44 @@ int build_fft_plan(bse_handle *h) {
     std::vector<int> hidx((size_t)D * D * D, -1);
     auto hid = [&](int m1, int m2, int m3) -> int & { return hidx[((size_t)(m1 + R) * D + (m2 + R)) * D + (m3 + R)]; };
     h->mill.resize(H.size() * 3);
-    std::vector<double> vc12(H.size()), vc12n(H.size());
+    std::vector<double> vc12(H.size()), vc12n(H.size()), inv2n(H.size());
     const double twopi_L = 2.0 * M_PI / h->L;
     for (size_t i = 0; i < H.size(); ++i) {
         hid(H[i].m1, H[i].m2, H[i].m3) = (int)i;
         h->mill[3 * i] = H[i].m1; h->mill[3 * i + 1] = H[i].m2; h->mill[3 * i + 2] = H[i].m3;
         const int q = H[i].m1 * H[i].m1 + H[i].m2 * H[i].m2 + H[i].m3 * H[i].m3;
         vc12[i] = q == 0 ? 0.0 : std::sqrt(4.0 * M_PI) / (twopi_L * std::sqrt((double)q));
-        vc12n[i] = vc12[i] / (double)h->N;
+        vc12n[i] = vc12[i] / (2.0 * (double)h->N);
+        inv2n[i] = 1.0 / (2.0 * (double)h->N);
     }
-    // half sticks ordered by (m2 mod n, m3)
-    struct St { int m2, m3; long long key; };
+    // half sticks ordered by (t2 = m2 mod n, m3): stick index = soff[t2] + m3 for wmin[t2] <= m3 <= wmax[t2]
+    std::vector<int> soff(n, 0), wmax(n, -1), wmin(n, 0);
+    struct St { int m2, m3; };
     std::vector<St> sticks;
-    for (int m2 = -R; m2 <= R; ++m2)
-        for (int m3 = 0; m3 <= R; ++m3) {
-            if (m2 * m2 + m3 * m3 > msq) continue;
-            if (m3 == 0 && m2 < 0) continue;
-            sticks.push_back({m2, m3, (long long)((m2 + n) % n) * n + m3});
-        }
-    std::sort(sticks.begin(), sticks.end(), [](const St &a, const St &b) { return a.key < b.key; });
-    pl.NS = (int)sticks.size();
-    std::vector<int> kkf(2 * W), kki(2 * W);
-    for (int k = 0; k < W; ++k) {
-        const int mk = (k == 0) ? n / 2 : n - k;
-        kkf[k] = pos[k]; kkf[W + k] = pos[mk];
-        kki[k] = k;      kki[W + k] = mk;
+    for (int t2 = 0; t2 < n; ++t2) {
+        const int m2 = t2 < n / 2 ? t2 : t2 - n;
+        if (std::abs(m2) > R || 2 * t2 == n) continue;
+        const int lo = m2 < 0 ? 1 : 0;
+        int hi = -1;
+        for (int m3 = 0; m3 <= R; ++m3)
+            if (m2 * m2 + m3 * m3 <= msq) hi = m3;
+        wmin[t2] = lo;
+        wmax[t2] = hi;
+        soff[t2] = (int)sticks.size() - lo;
+        for (int m3 = lo; m3 <= hi; ++m3) sticks.push_back({m2, m3});
     }
-    std::vector<int> soff_f(pl.NS), soff_i(pl.NS), soff_m(pl.NS), fmap((size_t)pl.NS * n), imap((size_t)pl.NS * n);
+    pl.NS = (int)sticks.size();
+    std::vector<int> hmapT((size_t)n * pl.NS, -1);
     for (int s = 0; s < pl.NS; ++s) {
         const int m2 = sticks[s].m2, m3 = sticks[s].m3;
-        const int t2 = (m2 + n) % n;
-        const int tf = pos[t2];
-        soff_f[s] = (tf >> 1) * ld + kkf[(tf & 1) * W + m3];
-        soff_i[s] = (t2 >> 1) * ld + kki[(t2 & 1) * W + m3];
-        soff_m[s] = -1;
-        if (m3 == 0 && m2 > 0) {
-            const int tm = n - m2;
-            soff_m[s] = (tm >> 1) * ld + kki[(tm & 1) * W + 0];
-        }
-        for (int t = 0; t < n; ++t) {
-            // forward: position t holds frequency rev[t]
-            {
-                const int f = rev[t];
-                const int m1 = f < n / 2 ? f : f - n;
-                int v = -1;
-                if (std::abs(m1) <= R && m1 * m1 + m2 * m2 + m3 * m3 <= msq) v = hid(m1, m2, m3);
-                fmap[(size_t)s * n + t] = v;
+        for (int t1 = 0; t1 < n; ++t1) {
+            const int m1 = t1 < n / 2 ? t1 : t1 - n;
+            int v = -1;
+            if (2 * t1 != n && std::abs(m1) <= R && m1 * m1 + m2 * m2 + m3 * m3 <= msq) {
+                v = hid(m1, m2, m3);
+                if (v < 0) v = -2 - hid(-m1, -m2, -m3);      // only the (0,0) stick, m1 < 0
             }
-            // inverse: position t = m1 mod n (natural order input)
-            {
-                const int m1 = t < n / 2 ? t : t - n;
-                int v = -1;
-                if (std::abs(m1) <= R && m1 * m1 + m2 * m2 + m3 * m3 <= msq) {
-                    v = hid(m1, m2, m3);
-                    if (v < 0) v = -2 - hid(-m1, -m2, -m3);      // only the (0,0) stick, m1 < 0
-                }
-                imap[(size_t)s * n + t] = v;
-            }
+            hmapT[(size_t)t1 * pl.NS + s] = v;
         }
     }
     std::vector<double2> tw(n);
@@ -169,26 +123,20 @@ int build_fft_plan(bse_handle *h) {
         const long double ang = -2.0L * 3.14159265358979323846264338327950288L * (long double)t / (long double)n;
         tw[t] = make_double2((double)cosl(ang), (double)sinl(ang));
     }
-    int rc;
     if ((rc = upload(pl.tw, tw))) return rc;
-    if ((rc = upload(pl.pos, pos))) return rc;
-    if ((rc = upload(pl.rev, rev))) return rc;
-    if ((rc = upload(pl.kk_fwd, kkf))) return rc;
-    if ((rc = upload(pl.kk_inv, kki))) return rc;
-    if ((rc = upload(pl.stick_off_fwd, soff_f))) return rc;
-    if ((rc = upload(pl.stick_off_inv, soff_i))) return rc;
-    if ((rc = upload(pl.stick_off_mir, soff_m))) return rc;
-    if ((rc = upload(pl.fmap, fmap))) return rc;
-    if ((rc = upload(pl.imap, imap))) return rc;
+    if ((rc = upload(pl.soff, soff))) return rc;
+    if ((rc = upload(pl.wmax, wmax))) return rc;
+    if ((rc = upload(pl.wmin, wmin))) return rc;
+    if ((rc = upload(pl.hmapT, hmapT))) return rc;
     if ((rc = upload(pl.vc12, vc12))) return rc;
     if ((rc = upload(pl.vc12n, vc12n))) return rc;
+    if ((rc = upload(pl.inv2n, inv2n))) return rc;
     return BSE_OK;
 }
 
 void free_plan(FftPlan &pl) {
-    cudaFree(pl.tw); cudaFree(pl.pos); cudaFree(pl.rev); cudaFree(pl.kk_fwd); cudaFree(pl.kk_inv);
-    cudaFree(pl.stick_off_fwd); cudaFree(pl.stick_off_inv); cudaFree(pl.stick_off_mir);
-    cudaFree(pl.fmap); cudaFree(pl.imap); cudaFree(pl.vc12); cudaFree(pl.vc12n);
+    cudaFree(pl.tw); cudaFree(pl.soff); cudaFree(pl.wmax); cudaFree(pl.wmin); cudaFree(pl.hmapT);
+    cudaFree(pl.vc12); cudaFree(pl.vc12n); cudaFree(pl.inv2n);
 }
 
 inline long long ldD(const bse_handle *h) { return (h->Npdep + 1) & ~1; }
@@ -296,10 +244,6 @@ extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cel
     if (2 * R >= h->n) { bse_set_error("sphere does not fit the grid (R >= n/2)"); return fail(BSE_EINVAL); }
     if ((rc = build_fft_plan(h))) return fail(rc);
     if ((long long)Npdep > 2 * (h->fft.npw_h - 1)) { bse_set_error("Npdep > 2 (Npw_h - 1)"); return fail(BSE_EINVAL); }
-    if (bse_fft_smem_bytes_plane(h->fft) > 227 * 1024) {
-        bse_set_error("grid plane does not fit in shared memory");
-        return fail(BSE_EUNSUPPORTED);
-    }
     const long long K2 = 2 * h->fft.npw_h;
     if (flags & BSE_PTR_HOST) {
         if (cudaMalloc(&h->u_owned, (size_t)Nv * h->N * 8) != cudaSuccess ||

@@ -7,33 +7,26 @@
 
 #include "../../include/bse.h"
 
-#define BSE_MAX_RADIX_PASSES 12
-
 // ---------------------------------------------------------------------------------------------------------
-// FFT plan: one length n for all three axes (cubic grid).  In-place decimation-in-frequency passes over
-// shared memory; after all passes position p of a line holds frequency rev[p]  (pos[rev[p]] = p).
+// FFT plan: one length n = R1 * R2 for all three axes (cubic grid); two register-butterfly passes per axis
+// (fft_kernels.cuh).  Sticks = (m2, m3) columns of the sphere's disk with m3 > 0 or (m3 == 0 and m2 >= 0), ordered
+// by (m2 mod n, m3).
 struct FftPlan {
-    int n = 0;           // points per axis
-    int ld = 0;          // padded line length in shared memory (complex elements), n + 1
-    int npass = 0;
-    int radix[BSE_MAX_RADIX_PASSES];
+    int n = 0, R1 = 0, R2 = 0;
     int R = 0;           // floor(sqrt(msq_max))
     int W = 0;           // kept m3 columns in the plane pass: m3 = 0..R  -> W = R + 1
-    int NS = 0;          // number of half sticks (m2, m3): m3 > 0 or (m3 == 0 and m2 >= 0), inside the disk
+    int NS = 0;          // number of half sticks
     long long npw_h = 0;
+    const void *ops = nullptr;    // bsefft::FftOps of this n
     // device tables
     double2 *tw = nullptr;        // [n]   exp(-2 pi i t / n)
-    int *pos = nullptr;           // [n]   position of frequency k after the DIF passes
-    int *rev = nullptr;           // [n]   frequency held at position p
-    int *kk_fwd = nullptr;        // [2][W] column slot of (row parity, m3) in the forward plane pass
-    int *kk_inv = nullptr;        // [2][W] same for the inverse plane pass
-    int *stick_off_fwd = nullptr; // [NS]  smem offset of stick (m2,m3) after the forward plane pass
-    int *stick_off_inv = nullptr; // [NS]  smem offset where stick (m2,m3) is loaded in the inverse plane pass
-    int *stick_off_mir = nullptr; // [NS]  smem offset of the mirrored (-m2, 0) entry, -1 if none
-    int *fmap = nullptr;          // [NS][n] forward stick pass: (stick, position t) -> index in H or -1
-    int *imap = nullptr;          // [NS][n] inverse stick pass: (stick, t = m1 mod n) -> h, -1 (zero), or -2-h (conj)
+    int *soff = nullptr;          // [n]   stick index of (t2 = m2 mod n, m3) is soff[t2] + m3
+    int *wmax = nullptr;          // [n]   largest m3 with a stick at t2, -1 if none
+    int *wmin = nullptr;          // [n]   smallest stored m3 at t2 (1 for m2 < 0)
+    int *hmapT = nullptr;         // [n][NS] (t1 = m1 mod n, stick) -> h in H, -1 outside, -2-h conj of entry h
     double *vc12 = nullptr;       // [npw_h] sqrt(4 pi)/|G|, 0 at G = 0
-    double *vc12n = nullptr;      // [npw_h] vc12 / N   (forward FFT normalisation folded in)
+    double *vc12n = nullptr;      // [npw_h] vc12 / (2N)  (forward normalisation and the untangling 1/2 folded in)
+    double *inv2n = nullptr;      // [npw_h] 1 / (2N)     (forward transform without the Coulomb factor, PW wrapper)
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -95,7 +88,8 @@ int bse_cuda_fail(cudaError_t e, const char *what);
 
 // ---- kernels' host launchers (each returns a BSE_* status) -------------------------------------------------
 // fft_kernels.cu
-int bse_fft_smem_bytes_plane(const FftPlan &pl);
+int bse_fft_select(FftPlan &pl);     // sets R1, R2, ops for pl.n; BSE_EUNSUPPORTED if there is no kernel for n
+// fields: [.][N]; pairs == nullptr: plain transform of field p0+p.  scale: [npw_h] table applied in the stick pass.
 int bse_launch_fwd_plane(const FftPlan &pl, const double *fields, const int2 *pairs, long long p0, int count,
                          long long N, double2 *Z, cudaStream_t s);
 int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2 *X, const double *scale,

@@ -1,0 +1,438 @@
+// Batched, pruned 3-D FFT kernels (fp64), templated on the two-pass factorisation n = R1 * R2 (R2 even).
+//
+// Steps a2, a3, a4, a9 (and the a12 wrappers) of SURVEY.md 8(a)  ("FFTs within a band group"; eq. 6/9/10):
+//   forward:  rho_p(r) = u_v(r) u_w(r)  --plane pass-->  Z[p][i1][stick]  --stick pass-->  x_p(G) on H
+//   inverse:  tau_p(G) on H  --stick pass-->  Z[p][i1][stick]  --plane pass-->  tau_p(r)
+//
+// Every 1-D transform of length n is two in-place decimation-in-frequency passes whose butterflies (sizes R1, R2 <= 16)
+// live in registers (fft_codelets.cuh), so a line crosses shared memory twice:
+//   pass 1: thread (line, j)   takes elements e = j + q R2 (q < R1), R1-point DFT, times w_n^{jq}, back to the same places
+//   pass 2: thread (line, blk) takes elements e = blk R2 + q (q < R2), R2-point DFT; place blk R2 + k2 then holds
+//           frequency blk + R1 k2.
+// Logical element e of a line sits at shared-memory slot natslot(e) = (e / R2) (R2+1) + e % R2 (odd group stride: the
+// strided accesses of pass 2 and of the column passes are bank-conflict free).
+//
+// Plane pass (one CTA = one n x n plane of fixed i1, two real rows packed per complex line):
+//   forward  P1 rows pass 1 straight from global memory (pair product fused: rho never exists in HBM)
+//            P2 rows pass 2, only frequencies |m3| <= R are written back
+//            P3 columns pass 1 with the two-row untangling fused into its load (columns m3 = 0..R only)
+//            P4 columns pass 2 straight to global memory: only the (m2, m3) sticks inside the sphere's disk leave the SM
+//   inverse  I1 columns pass 1 straight from the sticks in global memory, I2 columns pass 2 + tangling of row pairs,
+//            I3 rows pass 1 (zero padding by predicate), I4 rows pass 2 straight to global memory.
+// Stick pass (one CTA = TS sticks of one pair, all i1): S1 from global, S2 to global with the v_c^{1/2}/N scaling and the
+// gather to the half sphere H (forward) / scatter from H (inverse) fused.
+#pragma once
+#include "bse_internal.h"
+#include "fft_codelets.cuh"
+
+namespace bsefft {
+
+struct PlanDev {
+    int R, W, NS;
+    const double2 *tw;      // [n] exp(-2 pi i t / n)
+    const int *soff;        // [n] stick index of (t2, m3) is soff[t2] + m3
+    const int *wmax;        // [n] largest m3 of a stick at t2 = m2 mod n, -1 if none
+    const int *wmin;        // [n] smallest m3 stored (1 for m2 < 0: the (m2<0, m3=0) sticks are mirrors)
+    const int *hmapT;       // [n][NS] (t1 = m1 mod n, stick) -> h in H, -1 outside the sphere, -2-h: conj of entry h
+};
+
+template <int R1, int R2>
+struct Geo {
+    static constexpr int n = R1 * R2;
+    static constexpr int R2p = R2 + 1;
+    static constexpr int LD = R1 * R2p + ((R2 % 8) ? ((R2 - R1 * R2p) % 8 + 8) % 8 : 0);   // plane line stride (complex)
+    static constexpr int LDS = (R1 * R2p) | 1;                                            // stick line stride
+    static constexpr int TS = 16;                                                          // sticks per CTA
+    static __host__ __device__ constexpr int natslot(int e) { return (e / R2) * R2p + e % R2; }
+    static __host__ __device__ constexpr int fwdslot(int k) { return (k % R1) * R2p + k / R1; }
+    static constexpr int plane_smem = (n / 2) * LD * 16 + n * 16 + 3 * n * 4;
+    static constexpr int stick_smem = TS * LDS * 16 + n * 16;
+};
+
+// shared memory carve-up of the plane kernels: C[(n/2)*LD] | tw[n] | soff[n] | wmax[n] | wmin[n]
+template <int R1, int R2>
+__device__ __forceinline__ void plane_tables(unsigned char *smem, const PlanDev &P, double2 *&C, double2 *&tw,
+                                             int *&soff, int *&wmax, int *&wmin) {
+    using G = Geo<R1, R2>;
+    constexpr int n = G::n;
+    C = reinterpret_cast<double2 *>(smem);
+    tw = C + (size_t)(n / 2) * G::LD;
+    soff = reinterpret_cast<int *>(tw + n);
+    wmax = soff + n;
+    wmin = wmax + n;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        tw[i] = P.tw[i]; soff[i] = P.soff[i]; wmax[i] = P.wmax[i]; wmin[i] = P.wmin[i];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// forward plane pass.  grid = (n planes, count).  fields: [.][N]; pair (v,w) = pairs[p0+p], or when pairs == nullptr
+// the single field p0+p (no product: forward wrapper of the PW layout, step a12).
+// Output carries a factor 2 (the 1/2 of the two-row untangling is folded into the stick pass's scale).
+template <int R1, int R2>
+__global__ void __launch_bounds__(512)
+fwd_plane_kernel(PlanDev P, const double *__restrict__ fields, const int2 *__restrict__ pairs, long long p0,
+                 long long N, double2 *__restrict__ Z) {
+    using G = Geo<R1, R2>;
+    constexpr int n = G::n, LD = G::LD, R2p = G::R2p;
+    extern __shared__ __align__(16) unsigned char smem[];
+    double2 *C, *tw; int *soff, *wmax, *wmin;
+    plane_tables<R1, R2>(smem, P, C, tw, soff, wmax, wmin);
+    const int i1 = blockIdx.x;
+    const long long p = blockIdx.y;
+    const double *fv, *fw = nullptr;
+    if (pairs) {
+        const int2 vw = pairs[p0 + p];
+        fv = fields + (long long)vw.x * N + (long long)i1 * n * n;
+        fw = fields + (long long)vw.y * N + (long long)i1 * n * n;
+    } else {
+        fv = fields + (p0 + p) * N + (long long)i1 * n * n;
+    }
+    __syncthreads();
+    // P1 (a2 + rows pass 1)
+    for (int task = threadIdx.x; task < (n / 2) * R2; task += blockDim.x) {
+        const int l = task / R2, j = task - l * R2;
+        const double *ra = fv + (2 * l) * n + j, *rb = ra + n;
+        double2 x[R1];
+#pragma unroll
+        for (int q = 0; q < R1; ++q) x[q] = make_double2(ra[q * R2], rb[q * R2]);
+        if (fw) {
+            const double *wa = fw + (2 * l) * n + j, *wb = wa + n;
+#pragma unroll
+            for (int q = 0; q < R1; ++q) { x[q].x *= wa[q * R2]; x[q].y *= wb[q * R2]; }
+        }
+        Dft<R1, -1>::run(x);
+        twiddle_powers<R1>(x, tw[j]);
+#pragma unroll
+        for (int q = 0; q < R1; ++q) C[l * LD + q * R2p + j] = x[q];
+    }
+    __syncthreads();
+    // P2 (rows pass 2): frequency k = blk + R1 k2 lands in slot blk R2p + k2 = fwdslot(k)
+    const int R = P.R, W = P.W;
+    for (int task = threadIdx.x; task < (n / 2) * R1; task += blockDim.x) {
+        const int l = task / R1, blk = task - l * R1;
+        double2 *c = C + l * LD + blk * R2p;
+        double2 x[R2];
+#pragma unroll
+        for (int q = 0; q < R2; ++q) x[q] = c[q];
+        Dft<R2, -1>::run(x);
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) {
+            const int k = blk + R1 * k2;
+            if (k <= R || k >= n - R) c[k2] = x[k2];
+        }
+    }
+    __syncthreads();
+    // P3 (untangle rows 2l / 2l+1 + columns pass 1), columns m3 = 0..R; two DFTs per thread (rows j = 2jp, 2jp+1)
+    for (int task = threadIdx.x; task < W * (R2 / 2); task += blockDim.x) {
+        const int jp = task / W, m3 = task - jp * W;
+        const int sa = G::fwdslot(m3), sb = G::fwdslot(m3 ? n - m3 : n / 2);
+        double2 xa[R1], xb[R1];
+#pragma unroll
+        for (int q = 0; q < R1; ++q) {
+            const int l = jp + q * (R2 / 2);
+            const double2 za = C[l * LD + sa];
+            if (m3 == 0) {
+                xa[q] = make_double2(2.0 * za.x, 0.0);
+                xb[q] = make_double2(2.0 * za.y, 0.0);
+            } else {
+                const double2 zb = C[l * LD + sb];
+                xa[q] = make_double2(za.x + zb.x, za.y - zb.y);       // za + conj(zb)      = 2 A[m3]
+                xb[q] = make_double2(za.y + zb.y, zb.x - za.x);       // (za - conj(zb))/i  = 2 B[m3]
+            }
+        }
+        Dft<R1, -1>::run(xa);
+        Dft<R1, -1>::run(xb);
+        twiddle_powers<R1>(xa, tw[2 * jp]);
+        twiddle_powers<R1>(xb, tw[2 * jp + 1]);
+#pragma unroll
+        for (int q = 0; q < R1; ++q) {
+            const int l = jp + q * (R2 / 2);
+            C[l * LD + sa] = xa[q];
+            C[l * LD + sb] = xb[q];
+        }
+    }
+    __syncthreads();
+    // P4 (columns pass 2): only sticks inside the disk leave the SM
+    double2 *z = Z + (p * n + i1) * (long long)P.NS;
+    for (int task = threadIdx.x; task < W * R1; task += blockDim.x) {
+        const int blk = task / W, m3 = task - blk * W;
+        const int sa = G::fwdslot(m3), sb = G::fwdslot(m3 ? n - m3 : n / 2);
+        double2 x[R2];
+#pragma unroll
+        for (int q = 0; q < R2; ++q) x[q] = C[(blk * (R2 / 2) + (q >> 1)) * LD + ((q & 1) ? sb : sa)];
+        Dft<R2, -1>::run(x);
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) {
+            const int t2 = blk + R1 * k2;
+            if (m3 <= wmax[t2] && m3 >= wmin[t2]) z[soff[t2] + m3] = x[k2];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// inverse plane pass.  grid = (n planes, count).  Z[p][i1][NS] -> out[p][N] real.
+template <int R1, int R2>
+__global__ void __launch_bounds__(512)
+inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out) {
+    using G = Geo<R1, R2>;
+    constexpr int n = G::n, LD = G::LD, R2p = G::R2p;
+    extern __shared__ __align__(16) unsigned char smem[];
+    double2 *C, *tw; int *soff, *wmax, *wmin;
+    plane_tables<R1, R2>(smem, P, C, tw, soff, wmax, wmin);
+    const int i1 = blockIdx.x;
+    const long long p = blockIdx.y;
+    const int R = P.R, W = P.W;
+    const double2 *z = Z + (p * n + i1) * (long long)P.NS;
+    __syncthreads();
+    // I1 (columns pass 1 from the sticks; (m2<0, m3=0) is the conjugate of (-m2, 0))
+    for (int task = threadIdx.x; task < W * R2; task += blockDim.x) {
+        const int j = task / W, m3 = task - j * W;
+        const int na = G::natslot(m3), nb = G::natslot(m3 ? n - m3 : n / 2);
+        double2 x[R1];
+#pragma unroll
+        for (int q = 0; q < R1; ++q) {
+            const int t2 = j + q * R2;
+            double2 v = make_double2(0.0, 0.0);
+            if (m3 <= wmax[t2]) {
+                if (m3 >= wmin[t2]) v = z[soff[t2] + m3];
+                else { v = z[soff[n - t2]]; v.y = -v.y; }
+            }
+            x[q] = v;
+        }
+        Dft<R1, +1>::run(x);
+        twiddle_powers<R1>(x, cconj(tw[j]));
+#pragma unroll
+        for (int q = 0; q < R1; ++q) {
+            const int e = j + q * R2;
+            C[(e >> 1) * LD + ((e & 1) ? nb : na)] = x[q];
+        }
+    }
+    __syncthreads();
+    // I2 (columns pass 2 + tangle): Z_l[k] = A[k] + i B[k], Z_l[n-k] = conj(A[k]) + i conj(B[k])
+    for (int task = threadIdx.x; task < W * R1; task += blockDim.x) {
+        const int blk = task / W, m3 = task - blk * W;
+        const int na = G::natslot(m3), nb = G::natslot(m3 ? n - m3 : n / 2);
+        double2 x[R2];
+#pragma unroll
+        for (int q = 0; q < R2; ++q) x[q] = C[(blk * (R2 / 2) + (q >> 1)) * LD + ((q & 1) ? nb : na)];
+        Dft<R2, +1>::run(x);
+#pragma unroll
+        for (int t = 0; t < R2 / 2; ++t) {
+            const double2 a = x[2 * t], b = x[2 * t + 1];
+            double2 *c = C + (blk * (R2 / 2) + t) * LD;
+            if (m3 == 0) {
+                c[na] = make_double2(a.x, b.x);
+            } else {
+                c[na] = make_double2(a.x - b.y, a.y + b.x);
+                c[nb] = make_double2(a.x + b.y, b.x - a.y);
+            }
+        }
+    }
+    __syncthreads();
+    // I3 (rows pass 1; frequencies outside |m3| <= R are zero by predicate, never read)
+    for (int task = threadIdx.x; task < (n / 2) * R2; task += blockDim.x) {
+        const int l = task / R2, j = task - l * R2;
+        double2 *c = C + l * LD + j;
+        double2 x[R1];
+#pragma unroll
+        for (int q = 0; q < R1; ++q) {
+            const int e = j + q * R2;
+            x[q] = (e <= R || e >= n - R) ? c[q * R2p] : make_double2(0.0, 0.0);
+        }
+        Dft<R1, +1>::run(x);
+        twiddle_powers<R1>(x, cconj(tw[j]));
+#pragma unroll
+        for (int q = 0; q < R1; ++q) c[q * R2p] = x[q];
+    }
+    __syncthreads();
+    // I4 (rows pass 2 to global): line l packs the rows held at column places 2l, 2l+1 (place p holds row p/R2 + R1 (p%R2))
+    double *o = out + p * N + (long long)i1 * n * n;
+    for (int task = threadIdx.x; task < (n / 2) * R1; task += blockDim.x) {
+        const int l = task / R1, blk = task - l * R1;
+        const double2 *c = C + l * LD + blk * R2p;
+        double2 x[R2];
+#pragma unroll
+        for (int q = 0; q < R2; ++q) x[q] = c[q];
+        Dft<R2, +1>::run(x);
+        const int pa = 2 * l, pb = 2 * l + 1;
+        double *oa = o + (pa / R2 + R1 * (pa % R2)) * n + blk;
+        double *ob = o + (pb / R2 + R1 * (pb % R2)) * n + blk;
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) { oa[R1 * k2] = x[k2].x; ob[R1 * k2] = x[k2].y; }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// stick passes.  grid = (ceil(NS/TS), count), 256 threads.  smem: C[TS*LDS] | tw[n]
+template <int R1, int R2>
+__global__ void __launch_bounds__(256)
+fwd_stick_kernel(PlanDev P, const double2 *__restrict__ Z, double2 *__restrict__ X, long long npw_h,
+                 const double *__restrict__ scale) {
+    using G = Geo<R1, R2>;
+    constexpr int n = G::n, LDS = G::LDS, R2p = G::R2p, TS = G::TS;
+    extern __shared__ __align__(16) unsigned char smem[];
+    double2 *C = reinterpret_cast<double2 *>(smem);
+    double2 *tw = C + TS * LDS;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) tw[i] = P.tw[i];
+    const int NS = P.NS;
+    const int s0 = blockIdx.x * TS;
+    const long long p = blockIdx.y;
+    const double2 *z = Z + p * n * (long long)NS;
+    __syncthreads();
+    for (int task = threadIdx.x; task < TS * R2; task += blockDim.x) {
+        const int j = task / TS, sl = task - j * TS;
+        const int s = s0 + sl;
+        if (s >= NS) continue;
+        double2 x[R1];
+#pragma unroll
+        for (int q = 0; q < R1; ++q) x[q] = z[(long long)(j + q * R2) * NS + s];
+        Dft<R1, -1>::run(x);
+        twiddle_powers<R1>(x, tw[j]);
+#pragma unroll
+        for (int q = 0; q < R1; ++q) C[sl * LDS + q * R2p + j] = x[q];
+    }
+    __syncthreads();
+    // a4: x(G) = scale(G) * rho(G), gathered to H  (scale = v_c^{1/2}/(2N) for tau, 1/(2N) for the PW wrapper)
+    double2 *xo = X + p * npw_h;
+    for (int task = threadIdx.x; task < TS * R1; task += blockDim.x) {
+        const int blk = task / TS, sl = task - blk * TS;
+        const int s = s0 + sl;
+        if (s >= NS) continue;
+        double2 x[R2];
+#pragma unroll
+        for (int q = 0; q < R2; ++q) x[q] = C[sl * LDS + blk * R2p + q];
+        Dft<R2, -1>::run(x);
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) {
+            const int hh = P.hmapT[(blk + R1 * k2) * NS + s];
+            if (hh >= 0) {
+                const double sc = scale[hh];
+                xo[hh] = make_double2(x[k2].x * sc, x[k2].y * sc);
+            }
+        }
+    }
+}
+
+template <int R1, int R2>
+__global__ void __launch_bounds__(256)
+inv_stick_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, double2 *__restrict__ Z) {
+    using G = Geo<R1, R2>;
+    constexpr int n = G::n, LDS = G::LDS, R2p = G::R2p, TS = G::TS;
+    extern __shared__ __align__(16) unsigned char smem[];
+    double2 *C = reinterpret_cast<double2 *>(smem);
+    double2 *tw = C + TS * LDS;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) tw[i] = P.tw[i];
+    const int NS = P.NS;
+    const int s0 = blockIdx.x * TS;
+    const long long p = blockIdx.y;
+    const double2 *tg = T + p * npw_h;
+    __syncthreads();
+    for (int task = threadIdx.x; task < TS * R2; task += blockDim.x) {
+        const int j = task / TS, sl = task - j * TS;
+        const int s = s0 + sl;
+        if (s >= NS) continue;
+        double2 x[R1];
+#pragma unroll
+        for (int q = 0; q < R1; ++q) {
+            const int code = P.hmapT[(j + q * R2) * NS + s];
+            double2 v = make_double2(0.0, 0.0);
+            if (code >= 0) v = tg[code];
+            else if (code <= -2) { v = tg[-2 - code]; v.y = -v.y; }
+            x[q] = v;
+        }
+        Dft<R1, +1>::run(x);
+        twiddle_powers<R1>(x, cconj(tw[j]));
+#pragma unroll
+        for (int q = 0; q < R1; ++q) C[sl * LDS + q * R2p + j] = x[q];
+    }
+    __syncthreads();
+    double2 *z = Z + p * n * (long long)NS;
+    for (int task = threadIdx.x; task < TS * R1; task += blockDim.x) {
+        const int blk = task / TS, sl = task - blk * TS;
+        const int s = s0 + sl;
+        if (s >= NS) continue;
+        double2 x[R2];
+#pragma unroll
+        for (int q = 0; q < R2; ++q) x[q] = C[sl * LDS + blk * R2p + q];
+        Dft<R2, +1>::run(x);
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) z[(long long)(blk + R1 * k2) * NS + s] = x[k2];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// host launchers for one factorisation; collected in a table by fft_kernels.cu
+struct FftOps {
+    int n, R1, R2, plane_smem;
+    int (*fwd_plane)(const PlanDev &, const double *, const int2 *, long long, int, long long, double2 *, cudaStream_t);
+    int (*inv_plane)(const PlanDev &, const double2 *, int, long long, double *, cudaStream_t);
+    int (*fwd_stick)(const PlanDev &, const double2 *, int, double2 *, long long, const double *, cudaStream_t);
+    int (*inv_stick)(const PlanDev &, const double2 *, int, long long, double2 *, cudaStream_t);
+};
+
+inline int plane_threads(int tasks) {
+    const int iters = (tasks + 511) / 512;
+    const int t = ((tasks + iters - 1) / iters + 31) / 32 * 32;
+    return t < 64 ? 64 : t;
+}
+
+template <int R1, int R2>
+struct Launch {
+    using G = Geo<R1, R2>;
+    static int set_smem(const void *fn, int bytes) {
+        if (bytes > 48 * 1024) BSE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+        return BSE_OK;
+    }
+    static int fwd_plane(const PlanDev &P, const double *fields, const int2 *pairs, long long p0, int count, long long N,
+                         double2 *Z, cudaStream_t s) {
+        int rc = set_smem((const void *)fwd_plane_kernel<R1, R2>, G::plane_smem);
+        if (rc) return rc;
+        const int threads = plane_threads((G::n / 2) * R2);
+        for (int c0 = 0; c0 < count; c0 += 65535) {
+            const int c = count - c0 < 65535 ? count - c0 : 65535;
+            fwd_plane_kernel<R1, R2><<<dim3(G::n, c), threads, G::plane_smem, s>>>(
+                P, fields, pairs, p0 + c0, N, Z + (long long)c0 * G::n * P.NS);
+        }
+        BSE_CUDA(cudaGetLastError());
+        return BSE_OK;
+    }
+    static int inv_plane(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s) {
+        int rc = set_smem((const void *)inv_plane_kernel<R1, R2>, G::plane_smem);
+        if (rc) return rc;
+        const int threads = plane_threads((G::n / 2) * R2);
+        for (int c0 = 0; c0 < count; c0 += 65535) {
+            const int c = count - c0 < 65535 ? count - c0 : 65535;
+            inv_plane_kernel<R1, R2><<<dim3(G::n, c), threads, G::plane_smem, s>>>(
+                P, Z + (long long)c0 * G::n * P.NS, N, out + (long long)c0 * N);
+        }
+        BSE_CUDA(cudaGetLastError());
+        return BSE_OK;
+    }
+    static int fwd_stick(const PlanDev &P, const double2 *Z, int count, double2 *X, long long npw_h, const double *scale,
+                         cudaStream_t s) {
+        int rc = set_smem((const void *)fwd_stick_kernel<R1, R2>, G::stick_smem);
+        if (rc) return rc;
+        for (int c0 = 0; c0 < count; c0 += 65535) {
+            const int c = count - c0 < 65535 ? count - c0 : 65535;
+            fwd_stick_kernel<R1, R2><<<dim3((P.NS + G::TS - 1) / G::TS, c), 256, G::stick_smem, s>>>(
+                P, Z + (long long)c0 * G::n * P.NS, X + (long long)c0 * npw_h, npw_h, scale);
+        }
+        BSE_CUDA(cudaGetLastError());
+        return BSE_OK;
+    }
+    static int inv_stick(const PlanDev &P, const double2 *T, int count, long long npw_h, double2 *Z, cudaStream_t s) {
+        int rc = set_smem((const void *)inv_stick_kernel<R1, R2>, G::stick_smem);
+        if (rc) return rc;
+        for (int c0 = 0; c0 < count; c0 += 65535) {
+            const int c = count - c0 < 65535 ? count - c0 : 65535;
+            inv_stick_kernel<R1, R2><<<dim3((P.NS + G::TS - 1) / G::TS, c), 256, G::stick_smem, s>>>(
+                P, T + (long long)c0 * npw_h, npw_h, Z + (long long)c0 * G::n * P.NS);
+        }
+        BSE_CUDA(cudaGetLastError());
+        return BSE_OK;
+    }
+    static FftOps ops() { return FftOps{G::n, R1, R2, G::plane_smem, fwd_plane, inv_plane, fwd_stick, inv_stick}; }
+};
+
+}  // namespace bsefft
