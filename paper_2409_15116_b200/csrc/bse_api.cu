@@ -171,16 +171,24 @@ int ensure_tau_batch(bse_handle *h) {
     return BSE_OK;
 }
 
-int p_c_project(bse_handle *h, double *out, int B) {
-    // out currently holds acc.  S = dV acc u^T (split-K dot GEMM), out -= S u (NN GEMM)   (PAPER.md:67)
-    const long long rows = (long long)B * h->Nv;
+int ensure_sov(bse_handle *h, long long rows) {
     const long long lds = ldS(h);
     if (h->Sov_elems < (size_t)(rows * lds)) {
         cudaFree(h->Sov);
         h->Sov = nullptr;
+        h->Sov_elems = 0;
         BSE_CUDA(cudaMalloc(&h->Sov, (size_t)(rows * lds) * 8));
         h->Sov_elems = (size_t)(rows * lds);
     }
+    return BSE_OK;
+}
+
+int p_c_project(bse_handle *h, double *out, int B) {
+    // out currently holds acc.  S = dV acc u^T (split-K dot GEMM), out -= S u (NN GEMM)   (PAPER.md:67)
+    const long long rows = (long long)B * h->Nv;
+    const long long lds = ldS(h);
+    int rc0;
+    if ((rc0 = ensure_sov(h, rows))) return rc0;
     long long mc = rows;
     const long long per_row = (long long)h->Nv * 8 * 2;
     if (rows * per_row > (long long)h->part_bytes) mc = std::max<long long>(64, (long long)(h->part_bytes / per_row) / 64 * 64);
@@ -197,6 +205,123 @@ int p_c_project(bse_handle *h, double *out, int B) {
     return BSE_OK;
 }
 
+
+// u_w(G) on H for the PW layout (a12): forward transform of every orbital, no pair product, scale 1/(2N) -> uG;
+// uGw = Omega * wt(G) * uG with wt = 2 (G != 0), (1, 0) on (re, im) of G = 0, so that the half-sphere real dot product
+// sum_k uGw[w][k] x[k] equals <u_w|x> = Omega sum_{G in S} conj(u_w(G)) x(G)   (S14).
+int ensure_u_pw(bse_handle *h) {
+    if (h->uG) return BSE_OK;
+    const FftPlan &pl = h->fft;
+    const size_t bytes = (size_t)h->Nv * pl.npw_h * 16;
+    BSE_CUDA(cudaMalloc(&h->uG, bytes));
+    BSE_CUDA(cudaMalloc(&h->uGw, bytes));
+    int rc;
+    for (long long v0 = 0; v0 < h->Nv; v0 += h->Pb) {
+        const int cnt = (int)std::min<long long>(h->Pb, h->Nv - v0);
+        { StageTimer t(h, BSE_ST_FWD_PLANE);
+          if ((rc = bse_launch_fwd_plane(pl, h->u, nullptr, v0, cnt, h->N, h->Z, h->stream))) return rc; }
+        { StageTimer t(h, BSE_ST_FWD_STICK);
+          if ((rc = bse_launch_fwd_stick(pl, h->Z, cnt, h->uG + v0 * pl.npw_h, pl.inv2n, h->stream))) return rc; }
+    }
+    return bse_launch_weight_pw(h->uG, h->uGw, pl.npw_h, h->Nv, h->Omega, h->stream);
+}
+
+// real-space staging of one group of trial blocks: a_r, acc_r = [Bg][Nv][N]; Bg from the memory that is free now
+int ensure_vec_stage(bse_handle *h, int B) {
+    const size_t per_block = (size_t)h->Nv * h->N * 8 * 2;
+    if (h->Bg >= 1 && (h->Bg >= B || h->Bg_final)) return BSE_OK;
+    cudaFree(h->a_r); cudaFree(h->acc_r);
+    h->a_r = h->acc_r = nullptr; h->Bg = 0;
+    size_t free_b = 0, total_b = 0;
+    cudaMemGetInfo(&free_b, &total_b);
+    const size_t reserve = (size_t)512 << 20;
+    long long bg = free_b > reserve ? (long long)((free_b - reserve) / per_block) : 0;
+    if (bg < 1) {
+        char msg[200];
+        snprintf(msg, sizeof msg, "PW layout needs %.2f GB of real-space staging per trial block, %.2f GB free",
+                 per_block / 1e9, free_b / 1e9);
+        bse_set_error(msg);
+        return BSE_ENOMEM;
+    }
+    h->Bg_final = bg < B;
+    if (bg > B) bg = B;
+    BSE_CUDA(cudaMalloc(&h->a_r, (size_t)bg * h->Nv * h->N * 8));
+    BSE_CUDA(cudaMalloc(&h->acc_r, (size_t)bg * h->Nv * h->N * 8));
+    h->Bg = (int)bg;
+    return BSE_OK;
+}
+
+// acc (real space, [nb][Nv][N]) for the listed pairs: tau from the store or rebuilt per batch   (a9, a10)
+int accumulate_all(bse_handle *h, const double *a, double *acc, int nb) {
+    const unsigned mode = h->flags & BSE_TAU_MASK;
+    int rc;
+    if (mode == BSE_TAU_REAL) {
+        StageTimer t(h, BSE_ST_ACCUM);
+        return bse_launch_accumulate(h, h->tau_r, 0, h->P, a, acc, nb, true);
+    }
+    if ((rc = ensure_tau_batch(h))) return rc;
+    for (long long p0 = 0; p0 < h->P; p0 += h->Pb) {
+        const int cnt = (int)std::min<long long>(h->Pb, h->P - p0);
+        if (mode == BSE_TAU_PW) {
+            { StageTimer t(h, BSE_ST_INV_STICK);
+              if ((rc = bse_launch_inv_stick(h->fft, h->tau_g + p0 * h->fft.npw_h, cnt, h->Z, h->stream))) return rc; }
+            { StageTimer t(h, BSE_ST_INV_PLANE);
+              if ((rc = bse_launch_inv_plane(h->fft, h->Z, cnt, h->N, h->tau_batch, h->stream))) return rc; }
+        } else {
+            if ((rc = run_pair_batch(h, p0, cnt, h->T, h->tau_batch))) return rc;
+        }
+        StageTimer t(h, BSE_ST_ACCUM);
+        if ((rc = bse_launch_accumulate(h, h->tau_batch, p0, cnt, a, acc, nb, p0 == 0))) return rc;
+    }
+    return BSE_OK;
+}
+
+// PW layout (a12): a, out = [B][Nv][npw_h] complex on H
+int apply_pw(bse_handle *h, const double2 *a, double2 *out, int B) {
+    const FftPlan &pl = h->fft;
+    int rc;
+    if ((rc = ensure_u_pw(h))) return rc;
+    if ((rc = ensure_vec_stage(h, B))) return rc;
+    const long long Nv = h->Nv, npw_h = pl.npw_h;
+    for (int b0 = 0; b0 < B; b0 += h->Bg) {
+        const int nb = std::min(h->Bg, B - b0);
+        const long long fields = (long long)nb * Nv;
+        const double2 *ag = a + (long long)b0 * Nv * npw_h;
+        double2 *og = out + (long long)b0 * Nv * npw_h;
+        for (long long f0 = 0; f0 < fields; f0 += h->Pb) {           // a(G) -> a(r)
+            const int cnt = (int)std::min<long long>(h->Pb, fields - f0);
+            { StageTimer t(h, BSE_ST_INV_STICK);
+              if ((rc = bse_launch_inv_stick(pl, ag + f0 * npw_h, cnt, h->Z, h->stream))) return rc; }
+            { StageTimer t(h, BSE_ST_INV_PLANE);
+              if ((rc = bse_launch_inv_plane(pl, h->Z, cnt, h->N, h->a_r + f0 * h->N, h->stream))) return rc; }
+        }
+        if ((rc = accumulate_all(h, h->a_r, h->acc_r, nb))) return rc;
+        for (long long f0 = 0; f0 < fields; f0 += h->Pb) {           // acc(r) -> acc(G), truncated to S (S15)
+            const int cnt = (int)std::min<long long>(h->Pb, fields - f0);
+            { StageTimer t(h, BSE_ST_FWD_PLANE);
+              if ((rc = bse_launch_fwd_plane(pl, h->acc_r, nullptr, f0, cnt, h->N, h->Z, h->stream))) return rc; }
+            { StageTimer t(h, BSE_ST_FWD_STICK);
+              if ((rc = bse_launch_fwd_stick(pl, h->Z, cnt, og + f0 * npw_h, pl.inv2n, h->stream))) return rc; }
+        }
+    }
+    // P_c in PW: S = <u_w|acc> (real dot GEMM against the weighted copy), out -= S u(G)
+    const long long rows = (long long)B * Nv, K2 = 2 * npw_h, lds = ldS(h);
+    if ((rc = ensure_sov(h, rows))) return rc;
+    long long mc = rows;
+    const long long per_row = Nv * 8 * 2;
+    if (rows * per_row > (long long)h->part_bytes) mc = std::max<long long>(64, (long long)(h->part_bytes / per_row) / 64 * 64);
+    double *o = (double *)out;
+    for (long long r0 = 0; r0 < rows; r0 += mc) {
+        const int m = (int)std::min(mc, rows - r0);
+        { StageTimer t(h, BSE_ST_PC_OVERLAP);
+          if ((rc = bse_gemm_dot(o + r0 * K2, K2, (const double *)h->uGw, K2, m, h->Nv, K2, false, false, h->part,
+                                 h->part_bytes, h->Sov + r0 * lds, lds, 1.0, nullptr, h->stream))) return rc; }
+        { StageTimer t(h, BSE_ST_PC_UPDATE);
+          if ((rc = bse_gemm_nn(h->Sov + r0 * lds, lds, (const double *)h->uG, K2, m, K2, h->Nv, EPI_SUB, nullptr, nullptr,
+                                o + r0 * K2, K2, h->stream))) return rc; }
+    }
+    return BSE_OK;
+}
 }  // namespace
 
 extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cell[9], double ecut, int Nv,
@@ -224,7 +349,6 @@ extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cel
     for (int a = 0; a < Npdep; ++a)
         if (!(lambda[a] < 1.0)) { bse_set_error("lambda >= 1"); return BSE_EINVAL; }
     if ((flags & BSE_TAU_MASK) == 3u) { bse_set_error("bad tau storage flag"); return BSE_EINVAL; }
-    if (flags & BSE_VEC_PW) { bse_set_error("BSE_VEC_PW is not implemented in this version"); return BSE_EUNSUPPORTED; }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         bse_set_error("no CUDA device: this library has no CPU fallback");
@@ -303,6 +427,7 @@ extern "C" int bse_destroy(bse_handle *h) {
     cudaFree(h->rowptr); cudaFree(h->pid); cudaFree(h->pairs); cudaFree(h->adj_ptr); cudaFree(h->adj);
     cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);
     cudaFree(h->part); cudaFree(h->Sov); cudaFree(h->tau_batch); cudaFree(h->a_dev); cudaFree(h->out_dev);
+    cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->a_r); cudaFree(h->acc_r);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
     delete h;
@@ -354,33 +479,15 @@ extern "C" int bse_apply_k1x(bse_handle *h, const double *a, double *out, int B)
     if (!h || !a || !out || B <= 0) { bse_set_error("null pointer or B <= 0"); return BSE_EINVAL; }
     if (!h->built) { bse_set_error("bse_apply_k1x before bse_build_tau"); return BSE_ESTATE; }
     if (a == out) { bse_set_error("out must not alias a"); return BSE_EINVAL; }
-    const unsigned mode = h->flags & BSE_TAU_MASK;
     int rc;
-    if (mode == BSE_TAU_REAL) {
-        StageTimer t(h, BSE_ST_ACCUM);
-        if ((rc = bse_launch_accumulate(h, h->tau_r, 0, h->P, a, out, B, true))) return rc;
-    } else {
-        if ((rc = ensure_tau_batch(h))) return rc;
-        for (long long p0 = 0; p0 < h->P; p0 += h->Pb) {
-            const int cnt = (int)std::min<long long>(h->Pb, h->P - p0);
-            if (mode == BSE_TAU_PW) {
-                { StageTimer t(h, BSE_ST_INV_STICK);
-                  if ((rc = bse_launch_inv_stick(h->fft, h->tau_g + p0 * h->fft.npw_h, cnt, h->Z, h->stream))) return rc; }
-                { StageTimer t(h, BSE_ST_INV_PLANE);
-                  if ((rc = bse_launch_inv_plane(h->fft, h->Z, cnt, h->N, h->tau_batch, h->stream))) return rc; }
-            } else {
-                if ((rc = run_pair_batch(h, p0, cnt, h->T, h->tau_batch))) return rc;
-            }
-            StageTimer t(h, BSE_ST_ACCUM);
-            if ((rc = bse_launch_accumulate(h, h->tau_batch, p0, cnt, a, out, B, p0 == 0))) return rc;
-        }
-    }
+    if (h->flags & BSE_VEC_PW) return apply_pw(h, (const double2 *)a, (double2 *)out, B);
+    if ((rc = accumulate_all(h, a, out, B))) return rc;
     return p_c_project(h, out, B);
 }
 
 extern "C" int bse_apply_k1x_host(bse_handle *h, const double *a_host, double *out_host, int B) {
     if (!h || !a_host || !out_host || B <= 0) { bse_set_error("null pointer or B <= 0"); return BSE_EINVAL; }
-    const size_t bytes = (size_t)B * h->Nv * h->N * 8;
+    const size_t bytes = (h->flags & BSE_VEC_PW) ? (size_t)B * h->Nv * h->fft.npw_h * 16 : (size_t)B * h->Nv * h->N * 8;
     if (h->a_dev_bytes < bytes) {
         cudaFree(h->a_dev); cudaFree(h->out_dev);
         h->a_dev = h->out_dev = nullptr; h->a_dev_bytes = 0;

@@ -68,6 +68,11 @@ struct bse_handle {
     double *Sov = nullptr;           // [B*Nv][Nv] P_c overlaps
     size_t Sov_elems = 0;
     double *tau_batch = nullptr;     // [Pb][N] scratch for PW / STREAM modes
+    // PW layout (a12): u on H, its weighted copy for <u_w|.>, real-space staging of one group of Bg trial blocks
+    double2 *uG = nullptr, *uGw = nullptr;         // [Nv][npw_h]
+    double *a_r = nullptr, *acc_r = nullptr;       // [Bg][Nv][N]
+    int Bg = 0;
+    bool Bg_final = false;                         // Bg is already the most that fits
     double *a_dev = nullptr, *out_dev = nullptr;   // staging for the host-pointer entry point
     size_t a_dev_bytes = 0;
     // profiling
@@ -109,5 +114,8 @@ int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, 
 
 // k1x_kernels.cu
 int bse_launch_pairlist(bse_handle *h);                 // M -> rowcnt,rowptr,pid,pairs (count only if pairs==nullptr)
+// dst[w][k] = Omega * wt * src[w][k], wt = 2 for G != 0 and (1, 0) on (re, im) of G = 0 (entry 0 of H)
+int bse_launch_weight_pw(const double2 *src, double2 *dst, long long npw_h, long long rows, double Omega,
+                         cudaStream_t s);
 int bse_launch_accumulate(bse_handle *h, const double *tau, long long p_first, long long p_count,
                           const double *a, double *acc, int B, bool zero_init);

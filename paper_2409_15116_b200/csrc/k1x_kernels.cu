@@ -122,7 +122,23 @@ accumulate_kernel(const double *__restrict__ tau, long long p_first, long long p
     }
 }
 
+__global__ void weight_pw_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst, long long npw_h,
+                                 long long total, double Omega) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= total) return;
+    const double2 c = src[i];
+    dst[i] = (i % npw_h == 0) ? make_double2(Omega * c.x, 0.0) : make_double2(2.0 * Omega * c.x, 2.0 * Omega * c.y);
+}
+
 }  // namespace
+
+int bse_launch_weight_pw(const double2 *src, double2 *dst, long long npw_h, long long rows, double Omega,
+                         cudaStream_t s) {
+    const long long total = npw_h * rows;
+    weight_pw_kernel<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(src, dst, npw_h, total, Omega);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
 
 int bse_launch_pairlist(bse_handle *h) {
     const int Nv = h->Nv;

@@ -95,6 +95,46 @@ def _check_full(w, flags=0, check_g=True):
         g.close()
 
 
+def _check_pw(w, flags=0):
+    """PW layout (a12): a, out on the half sphere H; reference = oracle apply_k1x_pw (O8 'K1x PW')."""
+    bse = _bse()
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    pairs_ref, _ = orc.screen_pairs(w.u, w.eta)
+    g = Gpu(w, flags | bse.BSE_VEC_PW)
+    try:
+        pairs = g.build()
+        assert np.array_equal(pairs, pairs_ref)
+        tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs_ref, want="r")
+        ref = orc.apply_k1x_pw(tab, w.u, pairs_ref, tau_ref, w.a_pw)
+        a_d = torch.from_numpy(np.ascontiguousarray(w.a_pw).view(np.float64)).to("cuda:0")
+        out = torch.empty_like(a_d)
+        bse.bse_apply_k1x(g.h, a_d, out, w.a_pw.shape[0])
+        torch.cuda.synchronize()
+        got = out.cpu().numpy().view(np.complex128).reshape(ref.shape)
+        wt = np.full(tab.npw_h, 2.0)
+        wt[0] = 1.0                                   # S18: PW norm with weight 2 on G != 0
+        err = np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum())
+        assert err <= TOL, err
+        # second call reuses the staging buffers and gives the same bits
+        out2 = torch.empty_like(a_d)
+        bse.bse_apply_k1x(g.h, a_d, out2, w.a_pw.shape[0])
+        torch.cuda.synchronize()
+        assert torch.equal(out, out2)
+        return got
+    finally:
+        g.close()
+
+
+def test_pw_layout_all_tau_modes():
+    bse = _bse()
+    w = wl.make(1)
+    o = [_check_pw(w, f) for f in (bse.BSE_TAU_REAL, bse.BSE_TAU_PW, bse.BSE_TAU_STREAM)]
+    assert rel(o[1], o[0]) < 1e-12 and rel(o[2], o[0]) < 1e-12
+    cfg = wl.Config("edge", 9.0, 12, 5, 7, 3.0, 1.3, 0.8, 3.0, 0.05, 3, "random", seed=112)
+    _check_pw(wl.make(cfg=cfg))
+    _check_pw(wl.make(2, Nv=12, Npdep=40, B=2), bse.BSE_TAU_PW)
+
+
 def test_cfg1_full_all_modes():
     w = wl.make(1)
     bse = _bse()
@@ -187,7 +227,7 @@ def test_error_paths():
         (dict(ecut=40.0), bse.BSE_EINVAL),                 # sphere does not fit
         (dict(eta=-1.0), bse.BSE_EINVAL),
         (dict(grid=[12, 12, 10]), bse.BSE_EUNSUPPORTED),
-        (dict(flags=bse.BSE_VEC_PW), bse.BSE_EUNSUPPORTED),
+        (dict(flags=3), bse.BSE_EINVAL),                   # bad tau storage flag
     ]:
         args = dict(grid=[w.n] * 3, ecut=w.ecut, lam=w.lam, eta=0.0, flags=0)
         args.update(kwargs)
