@@ -140,6 +140,23 @@ def overlap_matrix(u: np.ndarray) -> np.ndarray:
     return (M / (d[:, None] * d[None, :]))
 
 
+def overlap_rows(get_u, Nv: int, rows):
+    """Rows of O (eq. 16) without holding all of u in extended precision: O[v, :] for v in `rows`.
+    get_u(w) returns orbital w as a float64 [N] array (so the caller may stream it from anywhere).
+    Same sums as overlap_matrix, one (v, w) pair at a time.  Used for the sampled screen check at the full size of
+    configs 4-5, where the N_v x N_v x N long-double SYRK of overlap_matrix would take hours."""
+    qrows = {v: (get_u(v) ** 2).astype(np.longdouble) for v in rows}
+    M = np.empty((len(rows), Nv), dtype=np.longdouble)
+    d = np.empty(Nv, dtype=np.longdouble)
+    for w in range(Nv):
+        qw = (get_u(w) ** 2).astype(np.longdouble)
+        d[w] = (qw * qw).sum()
+        for i, v in enumerate(rows):
+            M[i, w] = (qrows[v] * qw).sum()
+    dd = np.sqrt(d)
+    return np.asarray(M / (dd[list(rows)][:, None] * dd[None, :]), dtype=np.float64)
+
+
 def screen_pairs(u: np.ndarray, eta: float):
     """Surviving unordered pairs v <= w with O_vw >= eta, lexicographic (tau := 0 if O is
     *smaller than* the threshold; diagonal always kept).  Returns (pairs [P][2] int32, O float64)."""
@@ -236,7 +253,12 @@ def apply_k1x_pw(tab: Tables, u, pairs, tau, a_pw) -> np.ndarray:
     out = np.empty((B, Nv, tab.npw_h), dtype=np.complex128)
     for b in range(B):
         for v in range(Nv):
-            accS = tab.to_G(acc[b, v])
-            ov = tab.Omega * (np.conj(uS) @ accS)                # <u_w|acc>, real up to rounding
-            out[b, v] = S_to_H(tab, accS - ov.real @ uS)
+            out[b, v] = S_to_H(tab, p_c_pw(tab, uS, tab.to_G(acc[b, v])))
     return out
+
+
+def p_c_pw(tab: Tables, uS: np.ndarray, accS: np.ndarray) -> np.ndarray:
+    """P_c in PW on the full sphere: x - sum_w u_w <u_w|x>, <f|g> = Omega sum_{G in S} conj f(G) g(G).
+    uS: [Nv][Npw] orbital coefficients on S; accS: [Npw]."""
+    ov = tab.Omega * (np.conj(uS) @ accS)                        # <u_w|acc>, real up to rounding
+    return accS - ov.real @ uS

@@ -291,3 +291,143 @@ def make(cfg_id=None, *, cfg: Config | None = None, Nv=None, Npdep=None, B=None,
 
     return Workload(cfg=c, n=n, L=L, ecut=c.ecut, eta=c.eta, mill=mill, u=u, u_pw=u_pw,
                     phi=phi, lam=lam, a_pw=a_pw, sites=sites)
+
+
+# =============================================================================================================
+# Device generator for the large configurations (cfg 3-5): the same recipe executed with torch on a given device
+# (the GPU when there is one), because at 144^3 / 160^3 with 1024 orbitals the arrays are tens of GB and the numpy
+# path above takes tens of minutes.  Still inputs only: torch.fft / torch.linalg are used to band-limit,
+# orthonormalise and transform the INPUT functions; none of the method's steps (screen, pair integral, K1x, P_c of
+# the accumulated result) is evaluated here.  Differences from `make`: non-polynomial raw orbitals are the periodised
+# Gaussians given analytically in reciprocal space, g_v(G) ~ exp(-|G|^2 sigma^2 / 2) exp(-i G.R_v) (identical to the
+# minimum-image Gaussian up to exp(-(L/2)^2 / 2 sigma^2) < 1e-30 at cfg 4-5); phi and a are drawn from a seeded
+# torch.Generator on the device (so the draws differ from `make`, and depend on the device type, not on the run).
+@dataclasses.dataclass
+class DeviceWorkload:
+    cfg: Config
+    n: int
+    L: float
+    ecut: float
+    eta: float
+    mill: np.ndarray        # host [Npw_h][3] int32
+    u: "object"             # torch [Nv][N] float64 on the device
+    u_pw: "object"          # torch [Nv][Npw_h] complex128
+    phi: "object"           # torch [Npdep][Npw_h] complex128
+    lam: np.ndarray         # host [Npdep]
+    a_pw: "object"          # torch [B][Nv][Npw_h] complex128
+    sites: np.ndarray
+
+    @property
+    def N(self):
+        return self.n ** 3
+
+    @property
+    def Nv(self):
+        return self.u.shape[0]
+
+    @property
+    def cell(self):
+        return np.diag([self.L] * 3).astype(np.float64)
+
+
+def make_device(cfg_id=None, device="cuda:0", *, cfg: Config | None = None, Nv=None, Npdep=None, B=None,
+                seed=None) -> DeviceWorkload:
+    import torch
+    c = dataclasses.replace(CONFIGS[cfg_id] if cfg is None else cfg)
+    if Nv is not None:
+        c.Nv = Nv
+    if Npdep is not None:
+        c.Npdep = Npdep
+    if B is not None:
+        c.B = B
+    if seed is not None:
+        c.seed = seed
+    dev = torch.device(device)
+    rng = np.random.default_rng(c.seed)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(c.seed)
+    n, L = c.n, c.L
+    N = n ** 3
+    Omega = L ** 3
+    mill = half_sphere(n, L, c.ecut)
+    npw_h = mill.shape[0]
+    assert tuple(mill[0]) == (0, 0, 0)
+    if c.sites == "random":
+        sites = _sites_random(rng, c.Nv, L, c.sigma)
+    elif c.sites == "bcc":
+        sites = _sites_bcc(rng, c.Nv, L)
+    else:
+        sites = _sites_diamond_line(rng, c.Nv, L, c.sigma)
+    coefs = rng.normal(0.0, 0.35, size=(c.Nv, len(_POLY))) if c.poly else None
+
+    m_t = torch.from_numpy(mill.astype(np.int64)).to(dev)
+    i1, i2, i3 = m_t[:, 0] % n, m_t[:, 1] % n, m_t[:, 2]
+    z0 = m_t[:, 2] == 0
+    j1, j2 = (-m_t[z0, 0]) % n, (-m_t[z0, 1]) % n
+
+    def to_real(cH):                       # [k][Npw_h] complex -> [k][N] real (input prep, as pw_to_real)
+        k = cH.shape[0]
+        F = torch.zeros((k, n, n, n // 2 + 1), dtype=torch.complex128, device=dev)
+        F[:, i1, i2, i3] = cH
+        F[:, j1, j2, 0] = torch.conj(cH[:, z0])
+        F[:, 0, 0, 0] = cH[:, 0].real.to(torch.complex128)
+        return (torch.fft.irfftn(F, s=(n, n, n), dim=(1, 2, 3)) * float(N)).reshape(k, N)
+
+    def hdot(a, b):                        # full-sphere sum of conj(a) b for Hermitian sets stored on H
+        return 2.0 * (torch.conj(a) @ b.T).real - (torch.conj(a[:, :1]) @ b[:, :1].T).real
+
+    # raw orbitals -> coefficients on H
+    if coefs is None:
+        G = (2.0 * math.pi / L) * m_t.to(torch.float64)                    # [Npw_h][3]
+        R_t = torch.from_numpy(sites).to(dev)
+        ph = G @ R_t.T                                                     # [Npw_h][Nv]
+        env = torch.exp(-0.5 * c.sigma ** 2 * (G * G).sum(1))
+        g_pw = (env[:, None] * torch.polar(torch.ones_like(ph), -ph)).T.contiguous()
+        del ph
+    else:
+        g_pw = torch.empty((c.Nv, npw_h), dtype=torch.complex128, device=dev)
+        for v in range(c.Nv):
+            g = torch.from_numpy(_raw_orbital(n, L, c.sigma, sites[v], coefs[v])).to(dev)
+            g_pw[v] = torch.fft.rfftn(g, dim=(0, 1, 2))[i1, i2, i3] / float(N)
+    # Loewdin in PW
+    S = Omega * hdot(g_pw, g_pw)
+    w, V = torch.linalg.eigh(0.5 * (S + S.T))
+    assert float(w.min()) > 1e-10 * float(w.max()), "raw orbitals are linearly dependent"
+    Sm12 = ((V / torch.sqrt(w)) @ V.T).to(torch.complex128)
+    u_pw = Sm12 @ g_pw
+    del g_pw
+    u_pw[:, 0] = u_pw[:, 0].real.to(torch.complex128)
+    u = torch.empty((c.Nv, N), dtype=torch.float64, device=dev)
+    step = max(1, min(16, (1 << 28) // N))
+    for v0 in range(0, c.Nv, step):
+        u[v0:v0 + step] = to_real(u_pw[v0:v0 + step])
+
+    # PDEP basis
+    npd = c.Npdep
+    assert npd <= 2 * (npw_h - 1)
+    A = torch.randn((2 * (npw_h - 1), npd), dtype=torch.float64, device=dev, generator=gen)
+    Q, _ = torch.linalg.qr(A, mode="reduced")
+    del A
+    Q = Q / math.sqrt(2.0)
+    phi = torch.zeros((npd, npw_h), dtype=torch.complex128, device=dev)
+    phi[:, 1:] = torch.complex(Q[0::2, :], Q[1::2, :]).T
+    del Q
+    lam = -c.lam_c * np.exp(-c.lam_k * np.arange(npd) / npd)
+
+    # trial blocks
+    a_pw = torch.empty((c.B, c.Nv, npw_h), dtype=torch.complex128, device=dev)
+    for b in range(c.B):
+        ab = torch.complex(torch.randn((c.Nv, npw_h), dtype=torch.float64, device=dev, generator=gen),
+                           torch.randn((c.Nv, npw_h), dtype=torch.float64, device=dev, generator=gen))
+        ab[:, 0] = ab[:, 0].real.to(torch.complex128)
+        ov = Omega * hdot(u_pw, ab)                                        # [w][v] = <u_w|a_v>
+        ab = ab - ov.T.to(torch.complex128) @ u_pw
+        ab[:, 0] = ab[:, 0].real.to(torch.complex128)
+        nrm = Omega * float(torch.trace(hdot(ab, ab)))
+        a_pw[b] = ab / math.sqrt(nrm)
+        del ab
+    if dev.type == "cuda":
+        torch.cuda.synchronize(dev)
+        torch.cuda.empty_cache()           # the library allocates with cudaMalloc: give the cached blocks back
+    return DeviceWorkload(cfg=c, n=n, L=L, ecut=c.ecut, eta=c.eta, mill=mill, u=u, u_pw=u_pw, phi=phi, lam=lam,
+                          a_pw=a_pw, sites=sites)

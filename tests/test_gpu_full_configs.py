@@ -1,0 +1,171 @@
+"""GPU parity at the FULL size of BASELINE.json configs 3, 4 and 5, on sampled outputs the oracle can compute one by one.
+
+The oracle cannot run these configurations in full (its long-double screen alone is N_v^2 N = 4e12 operations at cfg 4-5, one
+pair integral takes ~10 s), so each test checks, against oracle values computed one at a time on the same inputs:
+  * the surviving-pair list restricted to sampled rows v (every w, both orders) - bit-exact, with the S10 guard band asserted
+    on those rows - and the GPU's O rows to 1e-12;
+  * tau_vw(r) for every pair of one complete row v* (the row with the fewest neighbours, >= 3) - 1e-10 relative L2 each;
+  * the K1x output row out[b, v*] for sampled blocks b in the layout the config uses (PW on H for cfg 4-5) - 1e-10.
+Inputs come from workloads.make_device (seeded, built on the GPU with torch: input preparation only).
+Launch configuration = the one bench.py uses for that config (tau storage / vector layout per SURVEY.md 8(d) item 7).
+"""
+import time
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle import bse_oracle as orc                      # noqa: E402
+from paper_2409_15116_b200 import workloads as wl         # noqa: E402
+
+TOL = 1e-10
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(np.asarray(b)))
+
+
+def _need_memory(gb):
+    free, _ = torch.cuda.mem_get_info()
+    if free < gb * 1e9:
+        pytest.skip(f"needs {gb} GB of free device memory, {free / 1e9:.0f} GB available")
+
+
+def _sampled_full_check(cfg_id, tau_flag, vec_pw, screen_rows, blocks, need_gb):
+    from paper_2409_15116_b200 import bse
+    _need_memory(need_gb)
+    t0 = time.time()
+    w = wl.make_device(cfg_id, "cuda:0")
+    u_pw_host = w.u_pw.cpu().numpy()
+    w.u_pw = None                                           # not an input of the library: free its device copy
+    Nv, N, B = w.Nv, w.N, w.a_pw.shape[0]
+    npw_h = w.mill.shape[0]
+    phi_d = torch.view_as_real(w.phi).contiguous()
+    flags = tau_flag | (bse.BSE_VEC_PW if vec_pw else bse.BSE_VEC_REAL)
+    h = bse.bse_create([w.n] * 3, w.cell, w.ecut, Nv, w.u, w.phi.shape[0], phi_d, w.lam, w.eta, flags)
+    try:
+        assert np.array_equal(bse.bse_gvectors(h), w.mill)
+        bse.bse_build_tau(h)
+        pairs = bse.bse_get_pairs(h)
+        P = len(pairs)
+        index = {(int(v), int(x)): p for p, (v, x) in enumerate(pairs)}
+        assert all(pairs[p][0] <= pairs[p][1] for p in range(P))
+        assert np.array_equal(pairs, np.array(sorted(index), dtype=np.int32))            # lexicographic, unique
+        nbr = [[] for _ in range(Nv)]
+        for (v, x) in index:
+            nbr[v].append(x)
+            if x != v:
+                nbr[x].append(v)
+        print(f"\ncfg{cfg_id}: generated in {time.time() - t0:.0f} s, P = {P} of {Nv * (Nv + 1) // 2} "
+              f"({100.0 * (P - Nv) / (Nv * (Nv - 1) // 2):.2f} % of off-diagonal pairs kept)")
+
+        # ---- a1: screen on sampled rows, oracle rows computed one (v, w) at a time in long double
+        def get_u(v):
+            return w.u[v].cpu().numpy()
+        Or = orc.overlap_rows(get_u, Nv, screen_rows)
+        O_gpu = bse.bse_get_overlap(h, Nv)
+        for i, v in enumerate(screen_rows):
+            off = np.arange(Nv) != v
+            assert np.min(np.abs(Or[i][off] - w.eta)) / w.eta > 1e-9, "guard band S10 violated on a sampled row"
+            ref = sorted(x for x in range(Nv) if x == v or Or[i, x] >= w.eta)
+            assert sorted(nbr[v]) == ref, f"pair list differs from the oracle on row {v}"
+            assert np.abs(O_gpu[v] - Or[i]).max() < 1e-12
+
+        # ---- apply on the GPU
+        if vec_pw:
+            a_d = torch.view_as_real(w.a_pw).contiguous()
+        else:
+            a_d = torch.empty((B, Nv, N), dtype=torch.float64, device="cuda:0")
+            tabs = _scatter_tables(w)
+            for b in range(B):
+                for v0 in range(0, Nv, 16):
+                    a_d[b, v0:v0 + 16] = _to_real(w, w.a_pw[b, v0:v0 + 16], tabs)
+        out = torch.empty_like(a_d)
+        torch.cuda.empty_cache()
+        try:
+            bse.bse_apply_k1x(h, a_d, out, B)
+        except bse.BseError as e:
+            if e.code == bse.BSE_ENOMEM:
+                pytest.skip(f"device memory: {e}")
+            raise
+        torch.cuda.synchronize()
+
+        # ---- one complete row v*: tau of each of its pairs, then the K1x output row for sampled blocks
+        cand = [v for v in range(Nv) if len(nbr[v]) >= 3]
+        vs = min(cand, key=lambda v: (len(nbr[v]), v))
+        tab = orc.Tables(w.n, w.L, w.ecut)
+        phiS = tab.expand_H_to_S(w.phi.cpu().numpy())
+        u_vs = get_u(vs)
+        acc = {b: np.zeros(N) for b in blocks}
+        dst = torch.empty((1, N), dtype=torch.float64, device="cuda:0")
+        worst = 0.0
+        for x in sorted(nbr[vs]):
+            t_ref = orc.tau_r(tab, u_vs, get_u(x), phiS, w.lam)
+            bse.bse_get_tau(h, index[(min(vs, x), max(vs, x))], 1, dst, bse.BSE_TAU_REAL)
+            torch.cuda.synchronize()
+            e = rel(dst[0].cpu().numpy(), t_ref)
+            worst = max(worst, e)
+            assert e <= TOL, (vs, x, e)
+            for b in blocks:
+                acc[b] += t_ref * tab.to_r(tab.expand_H_to_S(w.a_pw[b, x].cpu().numpy()))
+        uS = tab.expand_H_to_S(u_pw_host)      # the generator's coefficients of the same orbitals ...
+        assert rel(uS[vs], tab.to_G(u_vs)) < 1e-12          # ... which are what the oracle's own transform gives
+        errs = []
+        for b in blocks:
+            if vec_pw:
+                ref = orc.S_to_H(tab, orc.p_c_pw(tab, uS, tab.to_G(acc[b])))
+                got = torch.view_as_complex(out[b, vs]).cpu().numpy()
+                wt = np.full(npw_h, 2.0)
+                wt[0] = 1.0
+                e = float(np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum()))
+            else:
+                ref = orc.p_c_real(tab, w.u.cpu().numpy(), acc[b])
+                e = rel(out[b, vs].cpu().numpy(), ref)
+            errs.append(e)
+            assert e <= TOL, (b, e)
+        print(f"cfg{cfg_id}: row v* = {vs} with {len(nbr[vs])} neighbours; worst tau error {worst:.2e}; "
+              f"K1x row errors {['%.2e' % e for e in errs]}; total {time.time() - t0:.0f} s")
+    finally:
+        bse.bse_destroy(h)
+        del w
+        torch.cuda.empty_cache()
+
+
+def _scatter_tables(w):
+    n = w.n
+    m = torch.from_numpy(w.mill.astype(np.int64)).to("cuda:0")
+    z0 = m[:, 2] == 0
+    return (m[:, 0] % n, m[:, 1] % n, m[:, 2], z0, (-m[z0, 0]) % n, (-m[z0, 1]) % n)
+
+
+def _to_real(w, cH, tabs):
+    """Input preparation for the REAL layout: f(r) = sum_{G in S} c(G) e^{iG.r} of the trial-block coefficients."""
+    n = w.n
+    i1, i2, i3, z0, j1, j2 = tabs
+    F = torch.zeros((cH.shape[0], n, n, n // 2 + 1), dtype=torch.complex128, device="cuda:0")
+    F[:, i1, i2, i3] = cH
+    F[:, j1, j2, 0] = torch.conj(cH[:, z0])
+    F[:, 0, 0, 0] = cH[:, 0].real.to(torch.complex128)
+    return (torch.fft.irfftn(F, s=(n, n, n), dim=(1, 2, 3)) * float(n) ** 3).reshape(cH.shape[0], -1)
+
+
+def test_cfg3_full_size_real_layout():
+    from paper_2409_15116_b200 import bse
+    _sampled_full_check(3, bse.BSE_TAU_PW, False, screen_rows=[3, 101, 255], blocks=[0, 7], need_gb=60)
+
+
+def test_cfg3_full_size_pw_layout():
+    from paper_2409_15116_b200 import bse
+    _sampled_full_check(3, bse.BSE_TAU_PW, True, screen_rows=[17], blocks=[5], need_gb=40)
+
+
+def test_cfg4_full_size():
+    from paper_2409_15116_b200 import bse
+    _sampled_full_check(4, bse.BSE_TAU_PW, True, screen_rows=[777], blocks=[7], need_gb=120)
+
+
+def test_cfg5_full_size_streamed():
+    from paper_2409_15116_b200 import bse
+    _sampled_full_check(5, bse.BSE_TAU_STREAM, True, screen_rows=[1010], blocks=[15], need_gb=178)

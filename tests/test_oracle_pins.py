@@ -267,3 +267,12 @@ def test_workload_cfg1_inputs():
     assert np.all(w.lam < 0) and abs(w.lam[0] + 0.8) < 1e-15
     pairs, O = orc.screen_pairs(w.u, w.eta)
     assert len(pairs) == 36                                       # config 1: "all 36 pairs"
+
+
+def test_P11b_overlap_rows_equals_overlap_matrix_rows():
+    """overlap_rows (streamed form used for the sampled screen check at cfg 4-5) gives the rows of overlap_matrix."""
+    w = wl.make(1)
+    O = np.asarray(orc.overlap_matrix(w.u), dtype=np.float64)
+    rows = [0, 5, 7]
+    Or = orc.overlap_rows(lambda v: w.u[v], w.Nv, rows)
+    assert np.abs(Or - O[rows]).max() < 1e-15
