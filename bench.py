@@ -76,26 +76,9 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
-def stage_model(w, P, B, npw_h, NS):
-    """Algorithmic flops and compulsory HBM bytes per stage for one step."""
-    n, N, Nv, Npd = w.n, w.N, w.Nv, w.phi.shape[0]
-    z = 16 * n * NS
-    g = 16 * npw_h
-    fft_plane = 2.5 * n * n * np.log2(n) * n + 5 * n * np.log2(n) * (w_cols(w)) * n     # rows (real) + kept columns
-    fft_stick = 5 * n * np.log2(n) * NS
-    return {
-        "screen_syrk": dict(flops=Nv * (Nv + 1) * N, bytes=8 * Nv * N, bound="tensor"),
-        "pair_list": dict(flops=0, bytes=8 * Nv * Nv, bound="hbm"),
-        "fwd_plane": dict(flops=P * fft_plane, bytes=P * (8 * N + z), bound="hbm"),
-        "fwd_stick": dict(flops=P * fft_stick, bytes=P * (z + g), bound="hbm"),
-        "pdep_project": dict(flops=2 * P * Npd * 2 * npw_h, bytes=P * g + Npd * g, bound="tensor"),
-        "pdep_backproject": dict(flops=2 * P * Npd * 2 * npw_h, bytes=2 * P * g + Npd * g, bound="tensor"),
-        "inv_stick": dict(flops=P * fft_stick, bytes=P * (g + z), bound="hbm"),
-        "inv_plane": dict(flops=P * fft_plane, bytes=P * (z + 8 * N), bound="hbm"),
-        "k1x_accumulate": dict(flops=2 * B * N * (2 * P - Nv), bytes=8 * N * (P + 2 * B * Nv), bound="hbm"),
-        "pc_overlap": dict(flops=2 * B * Nv * Nv * N, bytes=8 * N * (B * Nv + Nv), bound="tensor"),
-        "pc_update": dict(flops=2 * B * Nv * Nv * N, bytes=8 * N * (2 * B * Nv + Nv), bound="tensor"),
-    }
+BOUND = {"screen_syrk": "tensor", "pair_list": "hbm", "fwd_plane": "hbm", "fwd_stick": "hbm", "pdep_project": "tensor",
+         "pdep_backproject": "tensor", "inv_stick": "hbm", "inv_plane": "hbm", "k1x_accumulate": "hbm",
+         "pc_overlap": "tensor", "pc_update": "tensor"}
 
 
 def w_cols(w):
@@ -174,7 +157,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-based); 2 = configs[1]")
-    ap.add_argument("--tau", default="real", choices=["real", "pw", "stream"])
+    ap.add_argument("--tau", default=None, choices=["real", "pw", "stream"],
+                    help="tau storage; default per config: 1-2 real, 3-4 pw, 5 stream (SURVEY.md 8(d) item 7)")
+    ap.add_argument("--vec", default=None, choices=["real", "pw"], help="layout of a/out; default: 1-3 real, 4-5 pw")
+    ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -184,6 +170,14 @@ def main():
         run_reference(args, rank)
         return
     args.warmup = max(args.warmup, 3)
+    if args.tau is None:
+        args.tau = {1: "real", 2: "real", 3: "pw", 4: "pw", 5: "stream"}[args.config]
+    if args.vec is None:
+        args.vec = "pw" if args.config >= 4 else "real"
+    large = args.config >= 3
+    if large:
+        args.no_e2e = True                # host copies of u / a are tens of GB: e2e is quoted on the default config
+        args.no_cpu_baseline = True       # the oracle's full long-double screen does not finish in bounded time
 
     import torch
     import torch.distributed as dist
@@ -195,17 +189,34 @@ def main():
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
         dist.init_process_group("nccl", device_id=dev)
 
-    w = wl.make(args.config)
-    B = w.a_pw.shape[0]
-    a_host = torch.from_numpy(np.ascontiguousarray(w.a_real())).pin_memory()
-    u_host = torch.from_numpy(w.u).pin_memory()
-    phi_host = torch.from_numpy(np.ascontiguousarray(w.phi).view(np.float64)).pin_memory()
-    out_host = torch.empty_like(a_host).pin_memory()
-    u_d, phi_d, a_d = u_host.to(dev), phi_host.to(dev), a_host.to(dev)
+    if large:
+        w = wl.make_device(args.config, dev)
+        B = w.a_pw.shape[0]
+        u_d = w.u
+        phi_d = torch.view_as_real(w.phi).contiguous()
+        if args.vec == "pw":
+            a_d = torch.view_as_real(w.a_pw).contiguous()
+        else:
+            a_d = wl.device_a_real(w)
+            w.a_pw = None
+        w.u_pw = None
+        torch.cuda.empty_cache()
+        n_pdep = w.phi.shape[0]
+    else:
+        w = wl.make(args.config)
+        B = w.a_pw.shape[0]
+        a_np = w.a_real() if args.vec == "real" else np.ascontiguousarray(w.a_pw).view(np.float64)
+        a_host = torch.from_numpy(np.ascontiguousarray(a_np)).pin_memory()
+        u_host = torch.from_numpy(w.u).pin_memory()
+        phi_host = torch.from_numpy(np.ascontiguousarray(w.phi).view(np.float64)).pin_memory()
+        out_host = torch.empty_like(a_host).pin_memory()
+        u_d, phi_d, a_d = u_host.to(dev), phi_host.to(dev), a_host.to(dev)
+        n_pdep = w.phi.shape[0]
     out_d = torch.empty_like(a_d)
     flags = {"real": bse.BSE_TAU_REAL, "pw": bse.BSE_TAU_PW, "stream": bse.BSE_TAU_STREAM}[args.tau]
+    flags |= bse.BSE_VEC_PW if args.vec == "pw" else bse.BSE_VEC_REAL
     stream = torch.cuda.current_stream().cuda_stream
-    h = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u_d, w.phi.shape[0], phi_d, w.lam, w.eta, flags, stream)
+    h = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u_d, n_pdep, phi_d, w.lam, w.eta, flags, stream)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
     def step(timed):
@@ -253,20 +264,15 @@ def main():
     # ---- per-stage device times (CUDA events on the library's stream, one extra profiled pass per step) ----
     bse.bse_profile_enable(h, True)
     bse.bse_profile_reset(h)
-    nprof = max(3, min(args.steps, 5))
+    nprof = 1 if large else max(3, min(args.steps, 5))
     for _ in range(nprof):
         step(False)
     torch.cuda.synchronize()
     prof = bse.bse_profile_get(h)
+    work = bse.bse_profile_model(h)      # algorithmic flops / compulsory bytes of those launches
     bse.bse_profile_enable(h, False)
     npw_h = bse.bse_npw_half(h)
-    NS = None
-    # NS (number of half sticks) recomputed here from the sphere definition for the byte model
-    R = w_cols(w) - 1
-    mx = wl.msq_max(w.L, w.ecut)
-    NS = sum(1 for m2 in range(-R, R + 1) for m3 in range(0, R + 1)
-             if m2 * m2 + m3 * m3 <= mx and not (m3 == 0 and m2 < 0))
-    model = stage_model(w, P, B, npw_h, NS)
+    model = {s_: dict(flops=work[s_][0] / nprof, bytes=work[s_][1] / nprof, bound=BOUND[s_]) for s_ in bse.STAGES}
     hbm_gbs, peak_src = load_peaks()
     dmma_tf, dfma_tf = bse.bse_probe_fp64_peak(stream)
     stages = {}
@@ -304,28 +310,35 @@ def main():
                 "mbytes": round(tot_b / 1e6, 1), "fp64_dmma_tflops": round(dmma_tf, 2), "fp64_dfma_tflops": round(dfma_tf, 2)}
 
     # ---- end to end through the C ABI with host (pinned) buffers ----
-    e2e_build, e2e_apply = [], []
-    for i in range(2 + 3):
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        hh = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u_host, w.phi.shape[0], phi_host, w.lam, w.eta,
-                            flags | bse.BSE_PTR_HOST, stream)
-        bse.bse_build_tau(hh)
-        torch.cuda.synchronize()
-        t1 = time.perf_counter()
-        bse.bse_apply_k1x_host(hh, a_host, out_host, B)
-        t2 = time.perf_counter()
-        bse.bse_destroy(hh)
-        if i >= 2:
-            e2e_build.append(t1 - t0)
-            e2e_apply.append(t2 - t1)
-    e2e_b, e2e_a = float(np.mean(e2e_build)), float(np.mean(e2e_apply))
-    if world > 1:
-        t = torch.tensor([e2e_b, e2e_a], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_b, e2e_a = t.tolist()
-    h2d = u_host.numel() * 8 + phi_host.numel() * 8 + a_host.numel() * 8
-    d2h = out_host.numel() * 8 + 8
+    e2e = None
+    if not args.no_e2e:
+        e2e_build, e2e_apply = [], []
+        for i in range(2 + 3):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            hh = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u_host, w.phi.shape[0], phi_host, w.lam, w.eta,
+                                flags | bse.BSE_PTR_HOST, stream)
+            bse.bse_build_tau(hh)
+            torch.cuda.synchronize()
+            t1 = time.perf_counter()
+            bse.bse_apply_k1x_host(hh, a_host, out_host, B)
+            t2 = time.perf_counter()
+            bse.bse_destroy(hh)
+            if i >= 2:
+                e2e_build.append(t1 - t0)
+                e2e_apply.append(t2 - t1)
+        e2e_b, e2e_a = float(np.mean(e2e_build)), float(np.mean(e2e_apply))
+        if world > 1:
+            t = torch.tensor([e2e_b, e2e_a], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_b, e2e_a = t.tolist()
+        h2d = u_host.numel() * 8 + phi_host.numel() * 8 + a_host.numel() * 8
+        d2h = out_host.numel() * 8 + 8
+        e2e = {"value": world * P / e2e_b, "unit": "pairs/s", "k1x_applies_per_s": world * B / e2e_a,
+               "build_ms": 1e3 * e2e_b, "apply_ms": 1e3 * e2e_a, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h),
+               "what": "bse_create(BSE_PTR_HOST: H2D of u, phi) + bse_build_tau, then bse_apply_k1x_host (H2D a, D2H out); "
+                       "pinned host buffers"}
 
     bse.bse_destroy(h)
     if rank != 0:
@@ -346,16 +359,13 @@ def main():
         "warmup": args.warmup, "ms_per_step": tb_ms + ta_ms, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{args.config - 1}] (cfg{args.config}): grid {w.n}^3, Nv={w.Nv}, "
-                               f"Npdep={w.phi.shape[0]}, Npw_h={npw_h}, eta={w.eta}, P={P} surviving pairs, B={B}",
-                   "tau_storage": args.tau, "vec_layout": "real", "parallelism": "replicas" if world > 1 else "1gpu",
+                               f"Npdep={n_pdep}, Npw_h={npw_h}, eta={w.eta}, P={P} surviving pairs, B={B}",
+                   "tau_storage": args.tau, "vec_layout": args.vec, "parallelism": "replicas" if world > 1 else "1gpu",
                    "l2": "512 MB buffer written between timed steps (L2 flush); inputs also exceed L2"},
         "k1x_applies_per_s": world * B / (ta_ms * 1e-3), "build_ms": tb_ms, "apply_ms": ta_ms, "pairs": P,
         "gpu_launches": int(launches), "wall_s_timed_region": wall,
         "clocks": clocks,
-        "e2e": {"value": world * P / e2e_b, "unit": "pairs/s", "k1x_applies_per_s": world * B / e2e_a,
-                "build_ms": 1e3 * e2e_b, "apply_ms": 1e3 * e2e_a, "h2d_bytes_per_step": int(h2d),
-                "d2h_bytes_per_step": int(d2h),
-                "what": "bse_create(BSE_PTR_HOST: H2D of u, phi) + bse_build_tau, then bse_apply_k1x_host (H2D a, D2H out); pinned host buffers"},
+        "e2e": e2e,
         "roofline": roof, "pipeline_roofline": pipeline, "stages": stages, "cpu_baseline": cpu,
     }
     print(json.dumps(line))

@@ -96,6 +96,9 @@ enum { BSE_ST_SCREEN = 0, BSE_ST_PAIRLIST, BSE_ST_FWD_PLANE, BSE_ST_FWD_STICK, B
 int bse_profile_enable(bse_handle *h, int enable);
 int bse_profile_reset(bse_handle *h);
 int bse_profile_get(const bse_handle *h, double *ms /* [BSE_ST_COUNT] */, long long *launches /* [BSE_ST_COUNT] */);
+/* Algorithmic work of the launches since the last reset (always counted): flops and compulsory HBM bytes per stage,
+ * by the per-unit figures of DESIGN.md section 6 times the units each launch processed. */
+int bse_profile_model(const bse_handle *h, double *flops /* [BSE_ST_COUNT] */, double *bytes /* [BSE_ST_COUNT] */);
 const char *bse_stage_name(int stage);
 
 /* FP64 peak probe: runs a dependent-free DMMA (mma.sync m8n8k4 f64) chain and a DFMA chain on every SM and

@@ -23,8 +23,8 @@ BSE_TAU_REAL, BSE_TAU_PW, BSE_TAU_STREAM = 0x0, 0x1, 0x2
 BSE_VEC_REAL, BSE_VEC_PW, BSE_PTR_HOST = 0x0, 0x4, 0x8
 STAGES = ["screen_syrk", "pair_list", "fwd_plane", "fwd_stick", "pdep_project", "pdep_backproject",
           "inv_stick", "inv_plane", "k1x_accumulate", "pc_overlap", "pc_update"]
-# kernels launched per stage invocation (bse_api.cu): split-K GEMMs launch GEMM + reduce, pair list 6 kernels
-KERNELS_PER_STAGE = [2, 6, 1, 1, 2, 1, 1, 1, 1, 2, 1]
+# kernels launched per stage invocation (bse_api.cu): split-K GEMMs launch GEMM + reduce, pair list 1 kernel
+KERNELS_PER_STAGE = [2, 1, 1, 1, 2, 1, 1, 1, 1, 2, 1]
 
 _vp, _i, _d, _u, _ll = C.c_void_p, C.c_int, C.c_double, C.c_uint, C.c_longlong
 _sig = {
@@ -42,6 +42,7 @@ _sig = {
     "bse_profile_enable": [_vp, _i],
     "bse_profile_reset": [_vp],
     "bse_profile_get": [_vp, C.POINTER(_d), C.POINTER(_ll)],
+    "bse_profile_model": [_vp, C.POINTER(_d), C.POINTER(_d)],
     "bse_probe_fp64_peak": [C.POINTER(_d), C.POINTER(_d), _vp],
 }
 for _name, _args in _sig.items():
@@ -149,6 +150,13 @@ def bse_profile_get(h):
     ln = (_ll * len(STAGES))()
     _check(lib.bse_profile_get(h, ms, ln), "bse_profile_get")
     return {s: (ms[i], ln[i]) for i, s in enumerate(STAGES)}
+
+
+def bse_profile_model(h):
+    fl = (_d * len(STAGES))()
+    by = (_d * len(STAGES))()
+    _check(lib.bse_profile_model(h, fl, by), "bse_profile_model")
+    return {s: (fl[i], by[i]) for i, s in enumerate(STAGES)}
 
 
 def bse_probe_fp64_peak(stream=None):

@@ -35,7 +35,9 @@ int upload(T *&dst, const std::vector<T> &src) {
 
 struct StageTimer {
     bse_handle *h; int st;
-    StageTimer(bse_handle *h_, int st_) : h(h_), st(st_) {
+    StageTimer(bse_handle *h_, int st_, double flops, double bytes) : h(h_), st(st_) {
+        h->st_flops[st] += flops;
+        h->st_bytes[st] += bytes;
         if (h->prof) cudaEventRecord(h->ev0, h->stream);
     }
     ~StageTimer() {
@@ -142,32 +144,83 @@ void free_plan(FftPlan &pl) {
 inline long long ldD(const bse_handle *h) { return (h->Npdep + 1) & ~1; }
 inline long long ldS(const bse_handle *h) { return (h->Nv + 1) & ~1; }
 
+// ---------------------------------------------------------------------------------------------------------
+// Stage wrappers: one kernel sequence + its event timer + its ALGORITHMIC flops and compulsory HBM bytes (the roofline
+// model of DESIGN.md section 6; bse_profile_model returns the sums).  lg = log2(n); z = bytes of one field's stick
+// planes Z; g = bytes of one field on H.
+struct Model {
+    double lg, N8, z, g, plane_flops, stick_flops;
+    explicit Model(const bse_handle *h) {
+        const double n = h->n;
+        lg = std::log2(n);
+        N8 = 8.0 * (double)h->N;
+        z = 16.0 * n * h->fft.NS;
+        g = 16.0 * (double)h->fft.npw_h;
+        plane_flops = 2.5 * n * n * n * lg + 5.0 * n * n * h->fft.W * lg;     // n^2 real rows + n W kept columns
+        stick_flops = 5.0 * n * lg * h->fft.NS;
+    }
+};
+
+int st_fwd_plane(bse_handle *h, const double *fields, const int2 *pairs, long long p0, int cnt) {
+    const Model m(h);
+    StageTimer t(h, BSE_ST_FWD_PLANE, cnt * m.plane_flops, cnt * (m.N8 + m.z));
+    return bse_launch_fwd_plane(h->fft, fields, pairs, p0, cnt, h->N, h->Z, h->stream);
+}
+int st_fwd_stick(bse_handle *h, int cnt, double2 *X, const double *scale) {
+    const Model m(h);
+    StageTimer t(h, BSE_ST_FWD_STICK, cnt * m.stick_flops, cnt * (m.z + m.g));
+    return bse_launch_fwd_stick(h->fft, h->Z, cnt, X, scale, h->stream);
+}
+int st_inv_stick(bse_handle *h, const double2 *T, int cnt) {
+    const Model m(h);
+    StageTimer t(h, BSE_ST_INV_STICK, cnt * m.stick_flops, cnt * (m.z + m.g));
+    return bse_launch_inv_stick(h->fft, T, cnt, h->Z, h->stream);
+}
+int st_inv_plane(bse_handle *h, int cnt, double *out) {
+    const Model m(h);
+    StageTimer t(h, BSE_ST_INV_PLANE, cnt * m.plane_flops, cnt * (m.N8 + m.z));
+    return bse_launch_inv_plane(h->fft, h->Z, cnt, h->N, out, h->stream);
+}
+// C[M][Nn] = alpha colscale[n] sum_k A[m][k] B[n][k]   (split-K DMMA)
+int st_gemm_dot(bse_handle *h, int stage, const double *A, long long lda, const double *B, long long ldb, int M, int Nn,
+                long long K, bool sq, double *C, long long ldc, double alpha, const double *colscale) {
+    const double flops = sq ? (double)M * (Nn + 1) * (double)K : 2.0 * M * Nn * (double)K;
+    const double bytes = sq ? 8.0 * M * (double)K : 8.0 * ((double)M * K + (double)Nn * K);
+    StageTimer t(h, stage, flops, bytes);
+    return bse_gemm_dot(A, lda, B, ldb, M, Nn, K, sq, sq, h->part, h->part_bytes, C, ldc, alpha, colscale, h->stream);
+}
+// NN form with the EPI_TAU / EPI_SUB epilogue: reads A [M][K], B [K][Nn], one [M][Nn] operand, writes [M][Nn]
+int st_gemm_nn(bse_handle *h, int stage, const double *A, long long lda, const double *B, long long ldb, int M,
+               long long Nn, int K, int epi, const double *Xin, const double *cs2, double *C, long long ldc) {
+    StageTimer t(h, stage, 2.0 * M * (double)Nn * K, 8.0 * (2.0 * M * (double)Nn + (double)K * Nn));
+    return bse_gemm_nn(A, lda, B, ldb, M, Nn, K, epi, Xin, cs2, C, ldc, h->stream);
+}
+// a10 for the pairs [p0, p0+cnt): compulsory traffic = tau of the batch; a and acc once per call (charged to the
+// first batch); flops 2 nb N per directed pair
+int st_accumulate(bse_handle *h, const double *tau, long long p0, long long cnt, const double *a, double *acc, int nb,
+                  bool first) {
+    const Model m(h);
+    const double directed = (double)h->nadj * (double)cnt / (double)std::max<long long>(h->P, 1);
+    StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)h->N * directed,
+                 m.N8 * ((double)cnt + (first ? 2.0 * nb * h->Nv : 0.0)));
+    return bse_launch_accumulate(h, tau, p0, cnt, a, acc, nb, first);
+}
+
 // tau for pairs [p0, p0+cnt): a2..a8 into dstG ([cnt][npw_h] complex), then a9 into dstR ([cnt][N]) if given
 int run_pair_batch(bse_handle *h, long long p0, int cnt, double2 *dstG, double *dstR) {
     const FftPlan &pl = h->fft;
-    int rc;
-    { StageTimer t(h, BSE_ST_FWD_PLANE);
-      if ((rc = bse_launch_fwd_plane(pl, h->u, h->pairs, p0, cnt, h->N, h->Z, h->stream))) return rc; }
-    { StageTimer t(h, BSE_ST_FWD_STICK);
-      if ((rc = bse_launch_fwd_stick(pl, h->Z, cnt, h->X, pl.vc12n, h->stream))) return rc; }
     const long long K2 = 2 * pl.npw_h;
-    { StageTimer t(h, BSE_ST_PROJECT);
-      if ((rc = bse_gemm_dot((const double *)h->X, K2, h->phi, K2, cnt, h->Npdep, K2, false, false, h->part,
-                             h->part_bytes, h->Dm, ldD(h), 1.0, h->f2, h->stream))) return rc; }
-    { StageTimer t(h, BSE_ST_BACKPROJECT);
-      if ((rc = bse_gemm_nn(h->Dm, ldD(h), h->phi, K2, cnt, K2, h->Npdep, EPI_TAU, (const double *)h->X, pl.vc12,
-                            (double *)dstG, K2, h->stream))) return rc; }
+    int rc;
+    if ((rc = st_fwd_plane(h, h->u, h->pairs, p0, cnt))) return rc;
+    if ((rc = st_fwd_stick(h, cnt, h->X, pl.vc12n))) return rc;
+    if ((rc = st_gemm_dot(h, BSE_ST_PROJECT, (const double *)h->X, K2, h->phi, K2, cnt, h->Npdep, K2, false, h->Dm,
+                          ldD(h), 1.0, h->f2))) return rc;
+    if ((rc = st_gemm_nn(h, BSE_ST_BACKPROJECT, h->Dm, ldD(h), h->phi, K2, cnt, K2, h->Npdep, EPI_TAU,
+                         (const double *)h->X, pl.vc12, (double *)dstG, K2))) return rc;
     if (dstR) {
-        { StageTimer t(h, BSE_ST_INV_STICK);
-          if ((rc = bse_launch_inv_stick(pl, dstG, cnt, h->Z, h->stream))) return rc; }
-        { StageTimer t(h, BSE_ST_INV_PLANE);
-          if ((rc = bse_launch_inv_plane(pl, h->Z, cnt, h->N, dstR, h->stream))) return rc; }
+        if ((rc = st_inv_stick(h, dstG, cnt))) return rc;
+        if ((rc = st_inv_plane(h, cnt, dstR))) return rc;
     }
-    return BSE_OK;
-}
-
-int ensure_tau_batch(bse_handle *h) {
-    if (!h->tau_batch) BSE_CUDA(cudaMalloc(&h->tau_batch, (size_t)h->Pb * h->N * 8));
     return BSE_OK;
 }
 
@@ -183,28 +236,24 @@ int ensure_sov(bse_handle *h, long long rows) {
     return BSE_OK;
 }
 
-int p_c_project(bse_handle *h, double *out, int B) {
-    // out currently holds acc.  S = dV acc u^T (split-K dot GEMM), out -= S u (NN GEMM)
-    const long long rows = (long long)B * h->Nv;
+// P_c on `rows` vectors of length K held in x: S = x ub^T (split-K dot GEMM; ub carries the inner
+// product's weights), x -= S uk (NN GEMM).  REAL: ub = uk = u, alpha = dV.  PW: ub = uGw, uk = uG, alpha = 1.
+int p_c_rows(bse_handle *h, double *x, long long rows, long long K, const double *ub, const double *uk, double alpha) {
     const long long lds = ldS(h);
-    int rc0;
-    if ((rc0 = ensure_sov(h, rows))) return rc0;
+    int rc;
+    if ((rc = ensure_sov(h, rows))) return rc;
     long long mc = rows;
     const long long per_row = (long long)h->Nv * 8 * 2;
     if (rows * per_row > (long long)h->part_bytes) mc = std::max<long long>(64, (long long)(h->part_bytes / per_row) / 64 * 64);
-    int rc;
     for (long long r0 = 0; r0 < rows; r0 += mc) {
         const int m = (int)std::min(mc, rows - r0);
-        { StageTimer t(h, BSE_ST_PC_OVERLAP);
-          if ((rc = bse_gemm_dot(out + r0 * h->N, h->N, h->u, h->N, m, h->Nv, h->N, false, false, h->part,
-                                 h->part_bytes, h->Sov + r0 * lds, lds, h->dV, nullptr, h->stream))) return rc; }
-        { StageTimer t(h, BSE_ST_PC_UPDATE);
-          if ((rc = bse_gemm_nn(h->Sov + r0 * lds, lds, h->u, h->N, m, h->N, h->Nv, EPI_SUB, nullptr, nullptr,
-                                out + r0 * h->N, h->N, h->stream))) return rc; }
+        if ((rc = st_gemm_dot(h, BSE_ST_PC_OVERLAP, x + r0 * K, K, ub, K, m, h->Nv, K, false, h->Sov + r0 * lds, lds,
+                              alpha, nullptr))) return rc;
+        if ((rc = st_gemm_nn(h, BSE_ST_PC_UPDATE, h->Sov + r0 * lds, lds, uk, K, m, K, h->Nv, EPI_SUB, nullptr, nullptr,
+                             x + r0 * K, K))) return rc;
     }
     return BSE_OK;
 }
-
 
 // u_w(G) on H for the PW layout (a12): forward transform of every orbital, no pair product, scale 1/(2N) -> uG;
 // uGw = Omega * wt(G) * uG with wt = 2 (G != 0), (1, 0) on (re, im) of G = 0, so that the half-sphere real dot product
@@ -218,60 +267,175 @@ int ensure_u_pw(bse_handle *h) {
     int rc;
     for (long long v0 = 0; v0 < h->Nv; v0 += h->Pb) {
         const int cnt = (int)std::min<long long>(h->Pb, h->Nv - v0);
-        { StageTimer t(h, BSE_ST_FWD_PLANE);
-          if ((rc = bse_launch_fwd_plane(pl, h->u, nullptr, v0, cnt, h->N, h->Z, h->stream))) return rc; }
-        { StageTimer t(h, BSE_ST_FWD_STICK);
-          if ((rc = bse_launch_fwd_stick(pl, h->Z, cnt, h->uG + v0 * pl.npw_h, pl.inv2n, h->stream))) return rc; }
+        if ((rc = st_fwd_plane(h, h->u, nullptr, v0, cnt))) return rc;
+        if ((rc = st_fwd_stick(h, cnt, h->uG + v0 * pl.npw_h, pl.inv2n))) return rc;
     }
     return bse_launch_weight_pw(h->uG, h->uGw, pl.npw_h, h->Nv, h->Omega, h->stream);
 }
 
-// real-space staging of one group of trial blocks: a_r, acc_r = [Bg][Nv][N]; Bg from the memory that is free now
-int ensure_vec_stage(bse_handle *h, int B) {
-    const size_t per_block = (size_t)h->Nv * h->N * 8 * 2;
-    if (h->Bg >= 1 && (h->Bg >= B || h->Bg_final)) return BSE_OK;
-    cudaFree(h->a_r); cudaFree(h->acc_r);
-    h->a_r = h->acc_r = nullptr; h->Bg = 0;
-    size_t free_b = 0, total_b = 0;
-    cudaMemGetInfo(&free_b, &total_b);
-    const size_t reserve = (size_t)512 << 20;
-    long long bg = free_b > reserve ? (long long)((free_b - reserve) / per_block) : 0;
-    if (bg < 1) {
-        char msg[200];
-        snprintf(msg, sizeof msg, "PW layout needs %.2f GB of real-space staging per trial block, %.2f GB free",
-                 per_block / 1e9, free_b / 1e9);
-        bse_set_error(msg);
+// pair-batch workspaces Z, X, T, Dm for `pb` fields (tau_batch follows lazily); called at create and again after the
+// pair list is known if one row of the adjacency has more entries than the batch holds
+int alloc_batch_ws(bse_handle *h, long long pb) {
+    cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm); cudaFree(h->tau_batch);
+    h->Z = h->X = h->T = nullptr; h->Dm = nullptr; h->tau_batch = nullptr;
+    h->Pb = 0;
+    if (cudaMalloc(&h->Z, (size_t)pb * h->n * h->fft.NS * 16) || cudaMalloc(&h->X, (size_t)pb * h->fft.npw_h * 16) ||
+        cudaMalloc(&h->T, (size_t)pb * h->fft.npw_h * 16) || cudaMalloc(&h->Dm, (size_t)pb * ldD(h) * 8)) {
+        (void)cudaGetLastError();
+        bse_set_error("out of device memory (pair-batch workspaces)");
         return BSE_ENOMEM;
     }
-    h->Bg_final = bg < B;
-    if (bg > B) bg = B;
-    BSE_CUDA(cudaMalloc(&h->a_r, (size_t)bg * h->Nv * h->N * 8));
-    BSE_CUDA(cudaMalloc(&h->acc_r, (size_t)bg * h->Nv * h->N * 8));
-    h->Bg = (int)bg;
+    h->Pb = pb;
     return BSE_OK;
 }
 
-// acc (real space, [nb][Nv][N]) for the listed pairs: tau from the store or rebuilt per batch   (a9, a10)
-int accumulate_all(bse_handle *h, const double *a, double *acc, int nb) {
+// tau store of the REAL / PW modes (grow-only); BSE_TAU_STREAM uses the PW store as a transient that is refilled inside
+// every apply call (tau(G) is 16 N / N_pw_h ~ 16x smaller than tau(r), which stays streamed in batches)
+int ensure_tau_store(bse_handle *h, bool real) {
+    const size_t need = real ? (size_t)h->P * h->N * 8 : (size_t)h->P * h->fft.npw_h * 16;
+    if (need <= h->tau_bytes && (real ? h->tau_r != nullptr : h->tau_g != nullptr)) return BSE_OK;
+    cudaFree(h->tau_r); h->tau_r = nullptr;
+    cudaFree(h->tau_g); h->tau_g = nullptr;
+    h->tau_bytes = 0;
+    size_t free_b = 0, total_b = 0;
+    cudaMemGetInfo(&free_b, &total_b);
+    if (need + ((size_t)256 << 20) > free_b) {
+        char msg[160];
+        snprintf(msg, sizeof msg, "tau store needs %.2f GB, %.2f GB free%s", need / 1e9, free_b / 1e9,
+                 real ? ": use BSE_TAU_PW or BSE_TAU_STREAM" : "");
+        bse_set_error(msg);
+        return BSE_ENOMEM;
+    }
+    if (real) BSE_CUDA(cudaMalloc(&h->tau_r, need));
+    else BSE_CUDA(cudaMalloc(&h->tau_g, need));
+    h->tau_bytes = need;
+    return BSE_OK;
+}
+
+int fill_tau_store(bse_handle *h, bool real) {
+    int rc;
+    for (long long p0 = 0; p0 < h->P; p0 += h->Pb) {
+        const int cnt = (int)std::min<long long>(h->Pb, h->P - p0);
+        if (real) rc = run_pair_batch(h, p0, cnt, h->T, h->tau_r + p0 * h->N);
+        else rc = run_pair_batch(h, p0, cnt, h->tau_g + p0 * h->fft.npw_h, nullptr);
+        if (rc) return rc;
+    }
+    return BSE_OK;
+}
+
+// Memory plan of the apply, made from what is free at the first call (and again if B grows or the list changes):
+//   tau_batch [Pacc][N]   tau(r) of the directed entries of one row batch (batched tau modes)
+//   a_r  [Bg][Nv][N]      PW layout: real-space trial blocks of one group (every neighbour of a row may be needed)
+//   acc_r[Bg][rows_cap][N] PW layout: accumulated rows of the current row batch (all Nv rows with BSE_TAU_REAL)
+// A larger row batch re-reads a fewer times and lets rows that share neighbours hit L2, a larger group inverts tau fewer
+// times: 60 % of the free memory goes to the group, the rest to the batch.
+int plan_apply_memory(bse_handle *h, int B) {
+    const bool pw = (h->flags & BSE_VEC_PW) != 0;
+    const bool batched = (h->flags & BSE_TAU_MASK) != BSE_TAU_REAL;
+    if (h->plan_ok && h->plan_nadj == h->nadj && (!pw || h->Bg >= B || h->Bg_final)) return BSE_OK;
+    cudaFree(h->tau_batch); cudaFree(h->a_r); cudaFree(h->acc_r);
+    h->tau_batch = h->a_r = h->acc_r = nullptr;
+    h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
+    size_t free_b = 0, total_b = 0;
+    cudaMemGetInfo(&free_b, &total_b);
+    const double N8 = 8.0 * (double)h->N;
+    const double avail = 0.92 * (double)free_b - 512.0 * 1048576.0;   // leave the caller some room
+    const double avgdeg = std::max(1.0, (double)h->nadj / h->Nv);
+    int maxdeg = 1;
+    for (int v = 0; v < h->Nv; ++v) maxdeg = std::max(maxdeg, h->adj_ptr_h[v + 1] - h->adj_ptr_h[v]);
+    auto nomem = [&](const char *what, double need) {
+        char msg[200];
+        snprintf(msg, sizeof msg, "%s needs %.2f GB, %.2f GB free", what, need / 1e9, free_b / 1e9);
+        bse_set_error(msg);
+        return BSE_ENOMEM;
+    };
+    long long bg = 0, pacc = 0, rows_cap = 0;
+    if (!pw) {
+        if (batched) {
+            pacc = (long long)std::min<double>((double)h->nadj, 0.9 * avail / N8);
+            if (pacc < maxdeg) return nomem("tau(r) of one row of pairs", maxdeg * N8);
+        }
+    } else if (!batched) {
+        bg = (long long)std::min<double>(B, avail / (2.0 * h->Nv * N8));
+        if (bg < 1) return nomem("real-space staging of one trial block (PW layout)", 2.0 * h->Nv * N8);
+        rows_cap = h->Nv;
+    } else {
+        // tau(r) of every directed entry is re-made once per group, so take the fewest groups whose row batch still
+        // holds max(longest row, min(nadj, 256)) entries; then the smallest group size with that many groups
+        const long long want = std::max<long long>(maxdeg, std::min<long long>(h->nadj, 256));
+        auto pacc_of = [&](long long g) {
+            const double rest = avail - (double)g * h->Nv * N8;
+            return rest <= 0 ? 0LL : (long long)std::min<double>((double)h->nadj, rest / (N8 * (1.0 + 2.0 * g / avgdeg)));
+        };
+        bg = B;
+        while (bg >= 1 && pacc_of(bg) < want) --bg;
+        if (bg < 1) return nomem("real-space staging of one trial block plus one row batch (PW layout)",
+                                 (h->Nv + 2.0 * want) * N8);
+        const long long groups = (B + bg - 1) / bg;
+        while (bg > 1 && (B + bg - 2) / (bg - 1) == groups) --bg;
+        pacc = pacc_of(bg);
+        rows_cap = std::min<long long>(h->Nv, std::max<long long>(1, (long long)(2.0 * pacc / avgdeg)));
+    }
+    if (pacc) BSE_CUDA(cudaMalloc(&h->tau_batch, (size_t)pacc * h->N * 8));
+    if (bg) {
+        BSE_CUDA(cudaMalloc(&h->a_r, (size_t)bg * h->Nv * h->N * 8));
+        BSE_CUDA(cudaMalloc(&h->acc_r, (size_t)bg * rows_cap * h->N * 8));
+    }
+    h->Bg = (int)bg; h->Bg_final = bg < B; h->Pacc = pacc; h->rows_cap = (int)rows_cap;
+    h->plan_ok = true;
+    h->plan_nadj = h->nadj;
+    return BSE_OK;
+}
+
+// forward transform of `rows` accumulated fields of each of nb blocks into the PW output (a12): acc(G) on H
+int rows_to_pw(bse_handle *h, const double *acc, long long acc_ld, int rows, int nb, double2 *out_pw, int v0) {
+    const long long npw_h = h->fft.npw_h;
+    int rc;
+    for (int b = 0; b < nb; ++b)
+        for (int r0 = 0; r0 < rows; r0 += (int)h->Pb) {
+            const int cnt = (int)std::min<long long>(h->Pb, rows - r0);
+            if ((rc = st_fwd_plane(h, acc + (long long)b * acc_ld * h->N, nullptr, r0, cnt))) return rc;
+            if ((rc = st_fwd_stick(h, cnt, out_pw + ((long long)b * h->Nv + v0 + r0) * npw_h, h->fft.inv2n))) return rc;
+        }
+    return BSE_OK;
+}
+
+// a9 + a10 for nb trial blocks a = [nb][Nv][N] (real space).
+//   REAL vec layout: acc_real = out ([nb][Nv][N]), out_pw = nullptr.
+//   PW vec layout:   acc_real = nullptr, rows are accumulated in h->acc_r and transformed to out_pw ([nb][Nv][npw_h]).
+// BSE_TAU_REAL: one launch over the symmetric pair list.  BSE_TAU_PW / STREAM: row batches; the batch holds tau(r) of every
+// directed entry of its rows (inverse FFT gathered from the tau(G) store), so each output row is written once.
+int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, double2 *out_pw) {
     const unsigned mode = h->flags & BSE_TAU_MASK;
     int rc;
     if (mode == BSE_TAU_REAL) {
-        StageTimer t(h, BSE_ST_ACCUM);
-        return bse_launch_accumulate(h, h->tau_r, 0, h->P, a, acc, nb, true);
+        double *acc = acc_real ? acc_real : h->acc_r;
+        if ((rc = st_accumulate(h, h->tau_r, 0, h->P, a, acc, nb, true))) return rc;
+        return out_pw ? rows_to_pw(h, acc, h->Nv, h->Nv, nb, out_pw, 0) : BSE_OK;
     }
-    if ((rc = ensure_tau_batch(h))) return rc;
-    for (long long p0 = 0; p0 < h->P; p0 += h->Pb) {
-        const int cnt = (int)std::min<long long>(h->Pb, h->P - p0);
-        if (mode == BSE_TAU_PW) {
-            { StageTimer t(h, BSE_ST_INV_STICK);
-              if ((rc = bse_launch_inv_stick(h->fft, h->tau_g + p0 * h->fft.npw_h, cnt, h->Z, h->stream))) return rc; }
-            { StageTimer t(h, BSE_ST_INV_PLANE);
-              if ((rc = bse_launch_inv_plane(h->fft, h->Z, cnt, h->N, h->tau_batch, h->stream))) return rc; }
-        } else {
-            if ((rc = run_pair_batch(h, p0, cnt, h->T, h->tau_batch))) return rc;
+    const Model m(h);
+    const std::vector<int> &ap = h->adj_ptr_h;
+    const double uniq = (double)h->P / (double)std::max<long long>(h->nadj, 1);   // share of the directed entries that is
+                                                                                   // algorithmic work (tau_vw = tau_wv)
+    const int rows_cap = acc_real ? h->Nv : h->rows_cap;
+    for (int v0 = 0; v0 < h->Nv;) {
+        int v1 = v0 + 1;
+        while (v1 < h->Nv && ap[v1 + 1] - ap[v0] <= h->Pacc && v1 - v0 < rows_cap) ++v1;
+        const int e0 = ap[v0], cnt = ap[v1] - e0, rows = v1 - v0;
+        for (int c0 = 0; c0 < cnt; c0 += (int)h->Pb) {                // tau(G) -> tau(r) of the batch's entries
+            const int c = (int)std::min<long long>(h->Pb, cnt - c0);
+            { StageTimer t(h, BSE_ST_INV_STICK, uniq * c * m.stick_flops, uniq * c * (m.z + m.g));
+              if ((rc = bse_launch_inv_stick(h->fft, h->tau_g, c, h->Z, h->stream, h->adj, e0 + c0))) return rc; }
+            { StageTimer t(h, BSE_ST_INV_PLANE, uniq * c * m.plane_flops, uniq * c * (m.N8 + m.z));
+              if ((rc = bse_launch_inv_plane(h->fft, h->Z, c, h->N, h->tau_batch + (long long)c0 * h->N, h->stream))) return rc; }
         }
-        StageTimer t(h, BSE_ST_ACCUM);
-        if ((rc = bse_launch_accumulate(h, h->tau_batch, p0, cnt, a, acc, nb, p0 == 0))) return rc;
+        { StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)h->N * cnt,
+                       m.N8 * (uniq * cnt + nb * rows + (v0 == 0 ? (double)nb * h->Nv : 0.0)));
+          if (acc_real) rc = bse_launch_accumulate_rows(h, h->tau_batch, e0, v0, rows, a, acc_real, h->Nv, 0, nb);
+          else rc = bse_launch_accumulate_rows(h, h->tau_batch, e0, v0, rows, a, h->acc_r, h->rows_cap, v0, nb);
+          if (rc) return rc; }
+        if (out_pw && (rc = rows_to_pw(h, h->acc_r, h->rows_cap, rows, nb, out_pw, v0))) return rc;
+        v0 = v1;
     }
     return BSE_OK;
 }
@@ -281,47 +445,22 @@ int apply_pw(bse_handle *h, const double2 *a, double2 *out, int B) {
     const FftPlan &pl = h->fft;
     int rc;
     if ((rc = ensure_u_pw(h))) return rc;
-    if ((rc = ensure_vec_stage(h, B))) return rc;
     const long long Nv = h->Nv, npw_h = pl.npw_h;
     for (int b0 = 0; b0 < B; b0 += h->Bg) {
         const int nb = std::min(h->Bg, B - b0);
         const long long fields = (long long)nb * Nv;
         const double2 *ag = a + (long long)b0 * Nv * npw_h;
-        double2 *og = out + (long long)b0 * Nv * npw_h;
         for (long long f0 = 0; f0 < fields; f0 += h->Pb) {           // a(G) -> a(r)
             const int cnt = (int)std::min<long long>(h->Pb, fields - f0);
-            { StageTimer t(h, BSE_ST_INV_STICK);
-              if ((rc = bse_launch_inv_stick(pl, ag + f0 * npw_h, cnt, h->Z, h->stream))) return rc; }
-            { StageTimer t(h, BSE_ST_INV_PLANE);
-              if ((rc = bse_launch_inv_plane(pl, h->Z, cnt, h->N, h->a_r + f0 * h->N, h->stream))) return rc; }
+            if ((rc = st_inv_stick(h, ag + f0 * npw_h, cnt))) return rc;
+            if ((rc = st_inv_plane(h, cnt, h->a_r + f0 * h->N))) return rc;
         }
-        if ((rc = accumulate_all(h, h->a_r, h->acc_r, nb))) return rc;
-        for (long long f0 = 0; f0 < fields; f0 += h->Pb) {           // acc(r) -> acc(G), truncated to S (S15)
-            const int cnt = (int)std::min<long long>(h->Pb, fields - f0);
-            { StageTimer t(h, BSE_ST_FWD_PLANE);
-              if ((rc = bse_launch_fwd_plane(pl, h->acc_r, nullptr, f0, cnt, h->N, h->Z, h->stream))) return rc; }
-            { StageTimer t(h, BSE_ST_FWD_STICK);
-              if ((rc = bse_launch_fwd_stick(pl, h->Z, cnt, og + f0 * npw_h, pl.inv2n, h->stream))) return rc; }
-        }
+        if ((rc = accumulate_all(h, h->a_r, nb, nullptr, out + (long long)b0 * Nv * npw_h))) return rc;
     }
     // P_c in PW: S = <u_w|acc> (real dot GEMM against the weighted copy), out -= S u(G)
-    const long long rows = (long long)B * Nv, K2 = 2 * npw_h, lds = ldS(h);
-    if ((rc = ensure_sov(h, rows))) return rc;
-    long long mc = rows;
-    const long long per_row = Nv * 8 * 2;
-    if (rows * per_row > (long long)h->part_bytes) mc = std::max<long long>(64, (long long)(h->part_bytes / per_row) / 64 * 64);
-    double *o = (double *)out;
-    for (long long r0 = 0; r0 < rows; r0 += mc) {
-        const int m = (int)std::min(mc, rows - r0);
-        { StageTimer t(h, BSE_ST_PC_OVERLAP);
-          if ((rc = bse_gemm_dot(o + r0 * K2, K2, (const double *)h->uGw, K2, m, h->Nv, K2, false, false, h->part,
-                                 h->part_bytes, h->Sov + r0 * lds, lds, 1.0, nullptr, h->stream))) return rc; }
-        { StageTimer t(h, BSE_ST_PC_UPDATE);
-          if ((rc = bse_gemm_nn(h->Sov + r0 * lds, lds, (const double *)h->uG, K2, m, K2, h->Nv, EPI_SUB, nullptr, nullptr,
-                                o + r0 * K2, K2, h->stream))) return rc; }
-    }
-    return BSE_OK;
+    return p_c_rows(h, (double *)out, (long long)B * Nv, 2 * npw_h, (const double *)h->uGw, (const double *)h->uG, 1.0);
 }
+
 }  // namespace
 
 extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cell[9], double ecut, int Nv,
@@ -401,14 +540,12 @@ extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cel
     cudaMemGetInfo(&free_b, &total_b);
     const size_t per_pair = (size_t)h->n * h->fft.NS * 16 + 2 * (size_t)h->fft.npw_h * 16 + (size_t)ldD(h) * 8;
     const size_t per_pair_r = (size_t)h->N * 8;   // tau_batch, allocated lazily (PW / STREAM / get_tau)
-    size_t budget = std::min<size_t>((size_t)6 << 30, free_b / 4);
+    size_t budget = std::min<size_t>((size_t)12 << 30, free_b / 4);
     long long Pb = (long long)(budget / (per_pair + per_pair_r));
-    Pb = std::max<long long>(1, std::min<long long>(Pb, 256));
-    h->Pb = Pb;
+    Pb = std::max<long long>(1, std::min<long long>(Pb, 512));
     h->part_bytes = std::max<size_t>((size_t)64 << 20, nv2 * 8 * 2);
-    if (cudaMalloc(&h->Z, (size_t)Pb * h->n * h->fft.NS * 16) || cudaMalloc(&h->X, (size_t)Pb * h->fft.npw_h * 16) ||
-        cudaMalloc(&h->T, (size_t)Pb * h->fft.npw_h * 16) || cudaMalloc(&h->Dm, (size_t)Pb * ldD(h) * 8) ||
-        cudaMalloc(&h->part, h->part_bytes)) {
+    if ((rc = alloc_batch_ws(h, Pb))) return fail(rc);
+    if (cudaMalloc(&h->part, h->part_bytes)) {
         bse_set_error("out of device memory (workspaces)");
         return fail(BSE_ENOMEM);
     }
@@ -439,37 +576,14 @@ extern "C" int bse_build_tau(bse_handle *h) {
     int rc;
     h->built = false;
     // a1: M = (u^2)(u^2)^T, then the threshold decision and the list, all on the device
-    { StageTimer t(h, BSE_ST_SCREEN);
-      if ((rc = bse_gemm_dot(h->u, h->N, h->u, h->N, h->Nv, h->Nv, h->N, true, true, h->part, h->part_bytes, h->Mmat,
-                             h->Nv, 1.0, nullptr, h->stream))) return rc; }
-    { StageTimer t(h, BSE_ST_PAIRLIST);
+    if ((rc = st_gemm_dot(h, BSE_ST_SCREEN, h->u, h->N, h->u, h->N, h->Nv, h->Nv, h->N, true, h->Mmat, h->Nv, 1.0,
+                          nullptr))) return rc;
+    { StageTimer t(h, BSE_ST_PAIRLIST, 0.0, 8.0 * h->Nv * (double)h->Nv);
       if ((rc = bse_launch_pairlist(h))) return rc; }
     const unsigned mode = h->flags & BSE_TAU_MASK;
     if (mode != BSE_TAU_STREAM) {
-        const size_t need = (mode == BSE_TAU_REAL) ? (size_t)h->P * h->N * 8 : (size_t)h->P * h->fft.npw_h * 16;
-        if (need > h->tau_bytes) {            // grow-only store: a rebuild with the same list allocates nothing
-            cudaFree(h->tau_r); h->tau_r = nullptr;
-            cudaFree(h->tau_g); h->tau_g = nullptr;
-            h->tau_bytes = 0;
-            size_t free_b = 0, total_b = 0;
-            cudaMemGetInfo(&free_b, &total_b);
-            if (need + ((size_t)256 << 20) > free_b) {
-                char msg[160];
-                snprintf(msg, sizeof msg, "tau store needs %.2f GB, %.2f GB free: use BSE_TAU_PW or BSE_TAU_STREAM",
-                         need / 1e9, free_b / 1e9);
-                bse_set_error(msg);
-                return BSE_ENOMEM;
-            }
-            if (mode == BSE_TAU_REAL) BSE_CUDA(cudaMalloc(&h->tau_r, need));
-            else BSE_CUDA(cudaMalloc(&h->tau_g, need));
-            h->tau_bytes = need;
-        }
-        for (long long p0 = 0; p0 < h->P; p0 += h->Pb) {
-            const int cnt = (int)std::min<long long>(h->Pb, h->P - p0);
-            if (mode == BSE_TAU_REAL) rc = run_pair_batch(h, p0, cnt, h->T, h->tau_r + p0 * h->N);
-            else rc = run_pair_batch(h, p0, cnt, h->tau_g + p0 * h->fft.npw_h, nullptr);
-            if (rc) return rc;
-        }
+        if ((rc = ensure_tau_store(h, mode == BSE_TAU_REAL))) return rc;
+        if ((rc = fill_tau_store(h, mode == BSE_TAU_REAL))) return rc;
     }
     h->built = true;
     return BSE_OK;
@@ -480,9 +594,14 @@ extern "C" int bse_apply_k1x(bse_handle *h, const double *a, double *out, int B)
     if (!h->built) { bse_set_error("bse_apply_k1x before bse_build_tau"); return BSE_ESTATE; }
     if (a == out) { bse_set_error("out must not alias a"); return BSE_EINVAL; }
     int rc;
+    if ((h->flags & BSE_TAU_MASK) == BSE_TAU_STREAM) {       // tau rebuilt inside every apply: tau(G) transient, tau(r) streamed
+        if ((rc = ensure_tau_store(h, false))) return rc;
+        if ((rc = fill_tau_store(h, false))) return rc;
+    }
+    if ((rc = plan_apply_memory(h, B))) return rc;
     if (h->flags & BSE_VEC_PW) return apply_pw(h, (const double2 *)a, (double2 *)out, B);
-    if ((rc = accumulate_all(h, a, out, B))) return rc;
-    return p_c_project(h, out, B);
+    if ((rc = accumulate_all(h, a, B, out, nullptr))) return rc;
+    return p_c_rows(h, out, (long long)B * h->Nv, h->N, h->u, h->u, h->dV);
 }
 
 extern "C" int bse_apply_k1x_host(bse_handle *h, const double *a_host, double *out_host, int B) {
@@ -534,9 +653,10 @@ extern "C" int bse_get_overlap(const bse_handle *h, double *O) {
     std::vector<double> M((size_t)Nv * Nv);
     BSE_CUDA(cudaMemcpyAsync(M.data(), h->Mmat, M.size() * 8, cudaMemcpyDeviceToHost, h->stream));
     BSE_CUDA(cudaStreamSynchronize(h->stream));
-    for (int v = 0; v < Nv; ++v)
-        for (int w = 0; w < Nv; ++w)
-            O[(size_t)v * Nv + w] = M[(size_t)v * Nv + w] / std::sqrt(M[(size_t)v * Nv + v] * M[(size_t)w * Nv + w]);
+    for (int v = 0; v < Nv; ++v)             // the device holds the upper triangle (v <= w) only
+        for (int w = v; w < Nv; ++w)
+            O[(size_t)v * Nv + w] = O[(size_t)w * Nv + v] =
+                M[(size_t)v * Nv + w] / std::sqrt(M[(size_t)v * Nv + v] * M[(size_t)w * Nv + w]);
     return BSE_OK;
 }
 extern "C" int bse_get_tau(bse_handle *h, long long first, long long count, double *dst, unsigned layout) {
@@ -572,7 +692,7 @@ extern "C" int bse_profile_enable(bse_handle *h, int enable) {
 }
 extern "C" int bse_profile_reset(bse_handle *h) {
     if (!h) return BSE_EINVAL;
-    for (int i = 0; i < BSE_ST_COUNT; ++i) { h->st_ms[i] = 0; h->st_launch[i] = 0; }
+    for (int i = 0; i < BSE_ST_COUNT; ++i) { h->st_ms[i] = 0; h->st_launch[i] = 0; h->st_flops[i] = 0; h->st_bytes[i] = 0; }
     return BSE_OK;
 }
 extern "C" int bse_profile_get(const bse_handle *h, double *ms, long long *launches) {
@@ -580,6 +700,14 @@ extern "C" int bse_profile_get(const bse_handle *h, double *ms, long long *launc
     for (int i = 0; i < BSE_ST_COUNT; ++i) {
         if (ms) ms[i] = h->st_ms[i];
         if (launches) launches[i] = h->st_launch[i];
+    }
+    return BSE_OK;
+}
+extern "C" int bse_profile_model(const bse_handle *h, double *flops, double *bytes) {
+    if (!h) return BSE_EINVAL;
+    for (int i = 0; i < BSE_ST_COUNT; ++i) {
+        if (flops) flops[i] = h->st_flops[i];
+        if (bytes) bytes[i] = h->st_bytes[i];
     }
     return BSE_OK;
 }

@@ -52,6 +52,7 @@ struct bse_handle {
     int *adj_ptr = nullptr;          // device [Nv+1] directed adjacency (both directions)
     int2 *adj = nullptr;             // device [nadj] (w, pair index), sorted by w within a row
     long long P = -1, nadj = 0;
+    std::vector<int> adj_ptr_h;      // host copy of adj_ptr (row batches of the batched tau modes)
     bool built = false;
     // tau store
     double *tau_r = nullptr;         // [P][N]
@@ -67,18 +68,21 @@ struct bse_handle {
     size_t part_bytes = 0;
     double *Sov = nullptr;           // [B*Nv][Nv] P_c overlaps
     size_t Sov_elems = 0;
-    double *tau_batch = nullptr;     // [Pb][N] scratch for PW / STREAM modes
+    double *tau_batch = nullptr;     // [Pacc][N] tau(r) of one row batch (PW / STREAM modes)
     // PW layout (a12): u on H, its weighted copy for <u_w|.>, real-space staging of one group of Bg trial blocks
     double2 *uG = nullptr, *uGw = nullptr;         // [Nv][npw_h]
     double *a_r = nullptr, *acc_r = nullptr;       // [Bg][Nv][N]
-    int Bg = 0;
-    bool Bg_final = false;                         // Bg is already the most that fits
+    int Bg = 0, rows_cap = 0;                      // acc_r holds rows_cap rows per block (row batches)
+    bool Bg_final = false, plan_ok = false;
+    long long plan_nadj = -1;
+    long long Pacc = 0;                            // capacity of tau_batch in directed entries                         // Bg is already the most that fits
     double *a_dev = nullptr, *out_dev = nullptr;   // staging for the host-pointer entry point
     size_t a_dev_bytes = 0;
     // profiling
     bool prof = false;
     double st_ms[BSE_ST_COUNT] = {0};
     long long st_launch[BSE_ST_COUNT] = {0};
+    double st_flops[BSE_ST_COUNT] = {0}, st_bytes[BSE_ST_COUNT] = {0};   // algorithmic work of the launches so far
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
 };
 
@@ -99,7 +103,9 @@ int bse_launch_fwd_plane(const FftPlan &pl, const double *fields, const int2 *pa
                          long long N, double2 *Z, cudaStream_t s);
 int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2 *X, const double *scale,
                          cudaStream_t s);
-int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2 *Z, cudaStream_t s);
+// gather != nullptr: field p is read from T + gather[g0 + p].y * npw_h (directed adjacency entries -> pair index)
+int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2 *Z, cudaStream_t s,
+                         const int2 *gather = nullptr, int g0 = 0);
 int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long long N, double *out, cudaStream_t s);
 
 // gemm_dmma.cu
@@ -114,6 +120,9 @@ int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, 
 
 // k1x_kernels.cu
 int bse_launch_pairlist(bse_handle *h);                 // M -> rowcnt,rowptr,pid,pairs (count only if pairs==nullptr)
+// row-complete accumulation of rows [v0, v0+nrows): tau_dir[e - e0] for every directed entry e of those rows
+int bse_launch_accumulate_rows(bse_handle *h, const double *tau_dir, int e0, int v0, int nrows, const double *a,
+                               double *acc, long long acc_ld, int v_base, int B);
 // dst[w][k] = Omega * wt * src[w][k], wt = 2 for G != 0 and (1, 0) on (re, im) of G = 0 (entry 0 of H)
 int bse_launch_weight_pw(const double2 *src, double2 *dst, long long npw_h, long long rows, double Omega,
                          cudaStream_t s);

@@ -79,16 +79,32 @@ dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restri
     const long long kbeg = (long long)blockIdx.z * kchunk;
     const long long kend = (kbeg + kchunk < K) ? kbeg + kchunk : K;
     const int nk = (int)((kend - kbeg + BK - 1) / BK);
+    if (SQA && SQB && n0 + BN <= m0) return;      // screen SYRK: M is symmetric, only tiles touching v <= w are formed
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wm = (warp >> 1) * 32, wn = (warp & 1) * 32;
     const int lr = lane >> 2, lc = lane & 3;
 
+    // EPI_TAU / EPI_SUB: the accumulators start from the epilogue operand (Xin, resp. C), whose global loads then overlap
+    // the cp.async prologue instead of sitting exposed after the k loop; EPI_SUB multiplies with -A (C - A B).
     double acc[4][4][2];
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+        for (int j = 0; j < 4; ++j) {
+            acc[i][j][0] = acc[i][j][1] = 0.0;
+            if (EPI == EPI_TAU || EPI == EPI_SUB) {
+                const int m = m0 + wm + i * 8 + lr;
+                const long long nn = n0 + wn + j * 8 + 2 * lc;
+                if (m < M && nn + 1 < Ntot) {
+                    const double *src = (EPI == EPI_TAU ? Xin : C) + (long long)m * ldc + nn;
+                    const double2 x = __ldcs(reinterpret_cast<const double2 *>(src));
+                    acc[i][j][0] = x.x; acc[i][j][1] = x.y;
+                } else if (m < M && nn < Ntot) {
+                    acc[i][j][0] = ((EPI == EPI_TAU ? Xin : C) + (long long)m * ldc + nn)[0];
+                }
+            }
+        }
 
     auto issue = [&](int kt) {
         if (kt < nk) {
@@ -115,6 +131,7 @@ dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restri
             for (int i = 0; i < 4; ++i) {
                 af[i] = as[(wm + i * 8 + lr) * LDK + kk + lc];
                 if (SQA) af[i] *= af[i];
+                if (EPI == EPI_SUB) af[i] = -af[i];
             }
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -143,14 +160,9 @@ dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restri
             double v0 = acc[i][j][0], v1 = acc[i][j][1];
             double *dst = Cout + (long long)m * ldc + nn;
             if (EPI == EPI_TAU) {
-                const double2 x = *reinterpret_cast<const double2 *>(Xin + (long long)m * ldc + nn);
                 const double sc = cs2[nn >> 1];
-                v0 = sc * (x.x + v0);
-                v1 = sc * (x.y + v1);
-            } else if (EPI == EPI_SUB) {
-                const double2 x = *reinterpret_cast<const double2 *>(dst);
-                v0 = x.x - v0;
-                v1 = x.y - v1;
+                v0 *= sc;
+                v1 *= sc;
             }
             if (EPI == EPI_PARTIAL) {          // ldc may be odd here: scalar stores
                 dst[0] = v0;
@@ -202,7 +214,8 @@ int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb,
     if (M <= 0 || N <= 0) return BSE_OK;
     const int tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
     const long long ksteps = (K + BK - 1) / BK;
-    long long splits = (2LL * 148 + (long long)tm * tn - 1) / ((long long)tm * tn);
+    const long long tiles = (squareA && squareB) ? (long long)tm * (tm + 1) / 2 : (long long)tm * tn;   // SYRK: v <= w tiles
+    long long splits = (2LL * 148 + tiles - 1) / tiles;
     if (splits > ksteps / 8) splits = ksteps / 8;
     if (splits < 1) splits = 1;
     const long long cap = (long long)(part_bytes / ((size_t)M * N * 8));

@@ -11,71 +11,98 @@ __device__ __forceinline__ bool keep_pair(const double *M, int Nv, int v, int w,
     return o >= eta;
 }
 
-__global__ void row_count_kernel(const double *__restrict__ M, int Nv, double eta, int *__restrict__ cnt) {
-    const int v = blockIdx.x * blockDim.x + threadIdx.x;
-    if (v >= Nv) return;
-    int c = 0;
-    for (int w = v; w < Nv; ++w) c += keep_pair(M, Nv, v, w, eta) ? 1 : 0;
-    cnt[v] = c;
-}
-
-// exclusive scan of cnt[0..n) into ptr[0..n]; one CTA, staged through shared memory in chunks
-__global__ void scan_kernel(const int *__restrict__ cnt, int n, int *__restrict__ ptr) {
-    __shared__ int buf[1024];
-    __shared__ int carry;
-    if (threadIdx.x == 0) carry = 0;
-    __syncthreads();
+// exclusive scan of vals[0..n) in place (global memory), total returned to every thread; one CTA of 1024 threads
+__device__ int block_exclusive_scan(int *vals, int n, int *smem_warp /*[33]*/) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int carry = 0;
     for (int base = 0; base < n; base += 1024) {
         const int i = base + threadIdx.x;
-        buf[threadIdx.x] = (i < n) ? cnt[i] : 0;
+        const int x = (i < n) ? vals[i] : 0;
+        int incl = x;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += y;
+        }
+        if (lane == 31) smem_warp[warp] = incl;
         __syncthreads();
-        if (threadIdx.x == 0) {
-            int run = carry;
-            for (int k = 0; k < 1024; ++k) { const int c = buf[k]; buf[k] = run; run += c; }
-            carry = run;
+        if (warp == 0) {
+            int w = smem_warp[lane];
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, w, d);
+                if (lane >= d) w += y;
+            }
+            smem_warp[lane] = w;                      // inclusive warp totals
         }
         __syncthreads();
-        if (i < n) ptr[i] = buf[threadIdx.x];
+        const int before = (warp ? smem_warp[warp - 1] : 0) + carry;
+        if (i < n) vals[i] = before + incl - x;
+        carry += smem_warp[31];
         __syncthreads();
     }
-    if (threadIdx.x == 0) ptr[n] = carry;
+    return carry;
 }
 
-__global__ void fill_pairs_kernel(const double *__restrict__ M, int Nv, double eta, const int *__restrict__ rowptr,
-                                  int2 *__restrict__ pairs, int *__restrict__ pid) {
-    const int v = blockIdx.x * blockDim.x + threadIdx.x;
-    if (v >= Nv) return;
-    int idx = rowptr[v];
-    for (int w = 0; w < v; ++w) pid[(long long)v * Nv + w] = -1;
-    for (int w = v; w < Nv; ++w) {
-        if (keep_pair(M, Nv, v, w, eta)) {
-            pairs[idx] = make_int2(v, w);
-            pid[(long long)v * Nv + w] = idx++;
-        } else {
-            pid[(long long)v * Nv + w] = -1;
+// a1 decision + pair list + directed adjacency in ONE launch (one CTA, warp per row, lanes over w: coalesced rows of M,
+// ballot prefix keeps the lexicographic order).  pid is written symmetrically (pid[v][w] = pid[w][v] = pair index or -1).
+__global__ void __launch_bounds__(1024)
+pairlist_kernel(const double *__restrict__ M, int Nv, double eta, int *__restrict__ rowptr, int2 *__restrict__ pairs,
+                int *__restrict__ pid, int *__restrict__ adj_ptr, int2 *__restrict__ adj) {
+    __shared__ int sw[33];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    for (int v = warp; v < Nv; v += nwarp) {                                  // kept pairs per row (w >= v)
+        int c = 0;
+        for (int w0 = v & ~31; w0 < Nv; w0 += 32) {
+            const int w = w0 + lane;
+            const bool k = (w >= v && w < Nv) ? keep_pair(M, Nv, v, w, eta) : false;
+            c += __popc(__ballot_sync(0xffffffffu, k));
+        }
+        if (lane == 0) rowptr[v] = c;
+    }
+    __syncthreads();
+    const int P = block_exclusive_scan(rowptr, Nv, sw);
+    if (threadIdx.x == 0) rowptr[Nv] = P;
+    __syncthreads();
+    for (int v = warp; v < Nv; v += nwarp) {                                  // fill pairs and the symmetric pid
+        int base = rowptr[v];
+        for (int w0 = v & ~31; w0 < Nv; w0 += 32) {
+            const int w = w0 + lane;
+            const bool in = (w >= v && w < Nv);
+            const bool k = in ? keep_pair(M, Nv, v, w, eta) : false;
+            const unsigned bal = __ballot_sync(0xffffffffu, k);
+            const int idx = base + __popc(bal & ((1u << lane) - 1u));
+            if (in) {
+                const int val = k ? idx : -1;
+                if (k) pairs[idx] = make_int2(v, w);
+                pid[(long long)v * Nv + w] = val;
+                pid[(long long)w * Nv + v] = val;
+            }
+            base += __popc(bal);
         }
     }
-}
-
-__global__ void adj_count_kernel(const int *__restrict__ pid, int Nv, int *__restrict__ cnt) {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= Nv) return;
-    int c = 0;
-    for (int x = 0; x < Nv; ++x) {
-        const int p = (x < t) ? pid[(long long)x * Nv + t] : pid[(long long)t * Nv + x];
-        c += (p >= 0) ? 1 : 0;
+    __syncthreads();
+    for (int t = warp; t < Nv; t += nwarp) {                                  // directed entries per row
+        int c = 0;
+        for (int x0 = 0; x0 < Nv; x0 += 32) {
+            const int x = x0 + lane;
+            c += __popc(__ballot_sync(0xffffffffu, x < Nv && pid[(long long)t * Nv + x] >= 0));
+        }
+        if (lane == 0) adj_ptr[t] = c;
     }
-    cnt[t] = c;
-}
-
-__global__ void adj_fill_kernel(const int *__restrict__ pid, int Nv, const int *__restrict__ ptr,
-                                int2 *__restrict__ adj) {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= Nv) return;
-    int idx = ptr[t];
-    for (int x = 0; x < Nv; ++x) {
-        const int p = (x < t) ? pid[(long long)x * Nv + t] : pid[(long long)t * Nv + x];
-        if (p >= 0) adj[idx++] = make_int2(x, p);
+    __syncthreads();
+    const int nadj = block_exclusive_scan(adj_ptr, Nv, sw);
+    if (threadIdx.x == 0) adj_ptr[Nv] = nadj;
+    __syncthreads();
+    for (int t = warp; t < Nv; t += nwarp) {
+        int base = adj_ptr[t];
+        for (int x0 = 0; x0 < Nv; x0 += 32) {
+            const int x = x0 + lane;
+            const int p = (x < Nv) ? pid[(long long)t * Nv + x] : -1;
+            const unsigned bal = __ballot_sync(0xffffffffu, p >= 0);
+            if (p >= 0) adj[base + __popc(bal & ((1u << lane) - 1u))] = make_int2(x, p);
+            base += __popc(bal);
+        }
     }
 }
 
@@ -122,6 +149,37 @@ accumulate_kernel(const double *__restrict__ tau, long long p_first, long long p
     }
 }
 
+// Row-complete form used with the batched tau modes: the batch holds tau of EVERY directed entry e of rows
+// [v0, v0 + gridDim.x) (tau_dir[e - e0] = tau of pair adj[e].y), so each output row is written once, never re-read:
+//   acc[(b * acc_ld + v - v_base)][r] = sum_{e in row v} tau_dir[e - e0][r] * a[b][adj[e].x][r]
+// grid = (rows, ceil(N / (2*blockDim))); rows vary fastest across resident CTAs, so they share the r-tile of a in L2.
+template <int BB>
+__global__ void __launch_bounds__(256)
+accumulate_rows_kernel(const double *__restrict__ tau_dir, int e0, int v0, const int *__restrict__ adj_ptr,
+                       const int2 *__restrict__ adj, const double *__restrict__ a, double *__restrict__ acc, int Nv,
+                       long long N, int b0, long long acc_ld, int v_base) {
+    const int v = v0 + blockIdx.x;
+    const long long r = 2 * ((long long)blockIdx.y * blockDim.x + threadIdx.x);
+    if (r >= N) return;
+    const int ea = adj_ptr[v], eb = adj_ptr[v + 1];
+    double2 s[BB];
+#pragma unroll
+    for (int b = 0; b < BB; ++b) s[b] = make_double2(0.0, 0.0);
+    for (int e = ea; e < eb; ++e) {
+        const int w = adj[e].x;
+        const double2 t = *reinterpret_cast<const double2 *>(tau_dir + (long long)(e - e0) * N + r);
+#pragma unroll
+        for (int b = 0; b < BB; ++b) {
+            const double2 x = *reinterpret_cast<const double2 *>(a + ((long long)(b0 + b) * Nv + w) * N + r);
+            s[b].x = fma(t.x, x.x, s[b].x);
+            s[b].y = fma(t.y, x.y, s[b].y);
+        }
+    }
+#pragma unroll
+    for (int b = 0; b < BB; ++b)
+        *reinterpret_cast<double2 *>(acc + ((long long)(b0 + b) * acc_ld + (v - v_base)) * N + r) = s[b];
+}
+
 __global__ void weight_pw_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst, long long npw_h,
                                  long long total, double Omega) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -142,20 +200,15 @@ int bse_launch_weight_pw(const double2 *src, double2 *dst, long long npw_h, long
 
 int bse_launch_pairlist(bse_handle *h) {
     const int Nv = h->Nv;
-    const int nb = (Nv + 127) / 128;
-    row_count_kernel<<<nb, 128, 0, h->stream>>>(h->Mmat, Nv, h->eta, h->rowcnt);
-    scan_kernel<<<1, 1024, 0, h->stream>>>(h->rowcnt, Nv, h->rowptr);
-    fill_pairs_kernel<<<nb, 128, 0, h->stream>>>(h->Mmat, Nv, h->eta, h->rowptr, h->pairs, h->pid);
-    adj_count_kernel<<<nb, 128, 0, h->stream>>>(h->pid, Nv, h->rowcnt);
-    scan_kernel<<<1, 1024, 0, h->stream>>>(h->rowcnt, Nv, h->adj_ptr);
-    adj_fill_kernel<<<nb, 128, 0, h->stream>>>(h->pid, Nv, h->adj_ptr, h->adj);
+    pairlist_kernel<<<1, 1024, 0, h->stream>>>(h->Mmat, Nv, h->eta, h->rowptr, h->pairs, h->pid, h->adj_ptr, h->adj);
     BSE_CUDA(cudaGetLastError());
     int P = 0, nadj = 0;
     BSE_CUDA(cudaMemcpyAsync(&P, h->rowptr + Nv, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
-    BSE_CUDA(cudaMemcpyAsync(&nadj, h->adj_ptr + Nv, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    h->adj_ptr_h.resize(Nv + 1);
+    BSE_CUDA(cudaMemcpyAsync(h->adj_ptr_h.data(), h->adj_ptr, (size_t)(Nv + 1) * 4, cudaMemcpyDeviceToHost, h->stream));
     BSE_CUDA(cudaStreamSynchronize(h->stream));
     h->P = P;
-    h->nadj = nadj;
+    h->nadj = nadj = h->adj_ptr_h[Nv];
     return BSE_OK;
 }
 
@@ -185,6 +238,27 @@ int bse_launch_accumulate(bse_handle *h, const double *tau, long long p_first, l
             b0 += 1;
         }
     }
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+int bse_launch_accumulate_rows(bse_handle *h, const double *tau_dir, int e0, int v0, int nrows, const double *a,
+                               double *acc, long long acc_ld, int v_base, int B) {
+    const int threads = 256;
+    const long long tiles = (h->N / 2 + threads - 1) / threads;
+    dim3 grid(nrows, (unsigned)tiles);
+    int b0 = 0;
+#define BSE_ROWS(BB)                                                                                              \
+    accumulate_rows_kernel<BB><<<grid, threads, 0, h->stream>>>(tau_dir, e0, v0, h->adj_ptr, h->adj, a, acc, h->Nv, \
+                                                                h->N, b0, acc_ld, v_base)
+    while (b0 < B) {
+        const int left = B - b0;
+        if (left >= 8) { BSE_ROWS(8); b0 += 8; }
+        else if (left >= 4) { BSE_ROWS(4); b0 += 4; }
+        else if (left >= 2) { BSE_ROWS(2); b0 += 2; }
+        else { BSE_ROWS(1); b0 += 1; }
+    }
+#undef BSE_ROWS
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }

@@ -431,3 +431,25 @@ def make_device(cfg_id=None, device="cuda:0", *, cfg: Config | None = None, Nv=N
         torch.cuda.empty_cache()           # the library allocates with cudaMalloc: give the cached blocks back
     return DeviceWorkload(cfg=c, n=n, L=L, ecut=c.ecut, eta=c.eta, mill=mill, u=u, u_pw=u_pw, phi=phi, lam=lam,
                           a_pw=a_pw, sites=sites)
+
+
+def device_a_real(w: DeviceWorkload):
+    """[B][Nv][N] real-space trial blocks of a DeviceWorkload (inverse transform of a_pw; input preparation)."""
+    import torch
+    n, dev = w.n, w.a_pw.device
+    m = torch.from_numpy(w.mill.astype(np.int64)).to(dev)
+    i1, i2, i3 = m[:, 0] % n, m[:, 1] % n, m[:, 2]
+    z0 = m[:, 2] == 0
+    j1, j2 = (-m[z0, 0]) % n, (-m[z0, 1]) % n
+    B, Nv, _ = w.a_pw.shape
+    out = torch.empty((B, Nv, n ** 3), dtype=torch.float64, device=dev)
+    step = max(1, min(16, (1 << 28) // n ** 3))
+    for b in range(B):
+        for v0 in range(0, Nv, step):
+            cH = w.a_pw[b, v0:v0 + step]
+            F = torch.zeros((cH.shape[0], n, n, n // 2 + 1), dtype=torch.complex128, device=dev)
+            F[:, i1, i2, i3] = cH
+            F[:, j1, j2, 0] = torch.conj(cH[:, z0])
+            F[:, 0, 0, 0] = cH[:, 0].real.to(torch.complex128)
+            out[b, v0:v0 + step] = (torch.fft.irfftn(F, s=(n, n, n), dim=(1, 2, 3)) * float(n) ** 3).reshape(cH.shape[0], -1)
+    return out
