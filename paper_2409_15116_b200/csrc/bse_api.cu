@@ -323,6 +323,45 @@ int fill_tau_store(bse_handle *h, bool real) {
     return BSE_OK;
 }
 
+// Row batches of the batched tau modes: consecutive rows are added while the pairs they touch (each counted once: a pair
+// with both ends in the batch serves both rows) fit the tau(r) batch buffer and the rows fit acc_r.
+int plan_row_batches(bse_handle *h, int rows_cap) {
+    const std::vector<int> &ap = h->adj_ptr_h;
+    const int Nv = h->Nv;
+    h->batches.clear();
+    std::vector<int> pairs_all, eslot((size_t)h->nadj), mark((size_t)std::max<long long>(h->P, 1), -1);
+    std::vector<int> cur;
+    for (int v0 = 0; v0 < Nv;) {
+        cur.clear();
+        int v1 = v0;
+        while (v1 < Nv && v1 - v0 < rows_cap) {
+            int fresh = 0;
+            for (int e = ap[v1]; e < ap[v1 + 1]; ++e) fresh += mark[h->adj_h[2 * e + 1]] != v0 ? 1 : 0;
+            if (v1 > v0 && (long long)cur.size() + fresh > h->Pacc) break;
+            for (int e = ap[v1]; e < ap[v1 + 1]; ++e) {
+                const int pidx = h->adj_h[2 * e + 1];
+                if (mark[pidx] != v0) { mark[pidx] = v0; cur.push_back(pidx); }
+            }
+            ++v1;
+        }
+        std::sort(cur.begin(), cur.end());                     // ascending pair index: sequential reads of the tau(G) store
+        for (int e = ap[v0]; e < ap[v1]; ++e)
+            eslot[e] = (int)(std::lower_bound(cur.begin(), cur.end(), h->adj_h[2 * e + 1]) - cur.begin());
+        h->batches.push_back({v0, v1, (int)pairs_all.size(), (int)cur.size()});
+        pairs_all.insert(pairs_all.end(), cur.begin(), cur.end());
+        v0 = v1;
+    }
+    h->uniq_share = (double)h->P / (double)std::max<size_t>(pairs_all.size(), 1);
+    cudaFree(h->batch_pairs); cudaFree(h->eslot);
+    h->batch_pairs = h->eslot = nullptr;
+    BSE_CUDA(cudaMalloc(&h->batch_pairs, std::max<size_t>(pairs_all.size(), 1) * 4));
+    BSE_CUDA(cudaMalloc(&h->eslot, std::max<size_t>(eslot.size(), 1) * 4));
+    BSE_CUDA(cudaMemcpyAsync(h->batch_pairs, pairs_all.data(), pairs_all.size() * 4, cudaMemcpyHostToDevice, h->stream));
+    BSE_CUDA(cudaMemcpyAsync(h->eslot, eslot.data(), eslot.size() * 4, cudaMemcpyHostToDevice, h->stream));
+    BSE_CUDA(cudaStreamSynchronize(h->stream));                // the host vectors go out of scope
+    return BSE_OK;
+}
+
 // Memory plan of the apply, made from what is free at the first call (and again if B grows or the list changes):
 //   tau_batch [Pacc][N]   tau(r) of the directed entries of one row batch (batched tau modes)
 //   a_r  [Bg][Nv][N]      PW layout: real-space trial blocks of one group (every neighbour of a row may be needed)
@@ -382,6 +421,10 @@ int plan_apply_memory(bse_handle *h, int B) {
         BSE_CUDA(cudaMalloc(&h->acc_r, (size_t)bg * rows_cap * h->N * 8));
     }
     h->Bg = (int)bg; h->Bg_final = bg < B; h->Pacc = pacc; h->rows_cap = (int)rows_cap;
+    if (batched) {
+        int rc = plan_row_batches(h, pw ? (int)rows_cap : h->Nv);
+        if (rc) return rc;
+    }
     h->plan_ok = true;
     h->plan_nadj = h->nadj;
     return BSE_OK;
@@ -415,27 +458,22 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
     }
     const Model m(h);
     const std::vector<int> &ap = h->adj_ptr_h;
-    const double uniq = (double)h->P / (double)std::max<long long>(h->nadj, 1);   // share of the directed entries that is
-                                                                                   // algorithmic work (tau_vw = tau_wv)
-    const int rows_cap = acc_real ? h->Nv : h->rows_cap;
-    for (int v0 = 0; v0 < h->Nv;) {
-        int v1 = v0 + 1;
-        while (v1 < h->Nv && ap[v1 + 1] - ap[v0] <= h->Pacc && v1 - v0 < rows_cap) ++v1;
-        const int e0 = ap[v0], cnt = ap[v1] - e0, rows = v1 - v0;
-        for (int c0 = 0; c0 < cnt; c0 += (int)h->Pb) {                // tau(G) -> tau(r) of the batch's entries
-            const int c = (int)std::min<long long>(h->Pb, cnt - c0);
+    const double uniq = h->uniq_share;        // share of the inverted fields that is algorithmic work (each pair once)
+    for (const bse_handle::RowBatch &bt : h->batches) {
+        const int v0 = bt.v0, rows = bt.v1 - bt.v0, cnt = ap[bt.v1] - ap[bt.v0];
+        for (int c0 = 0; c0 < bt.nu; c0 += (int)h->Pb) {              // tau(G) -> tau(r) of the batch's pairs
+            const int c = (int)std::min<long long>(h->Pb, bt.nu - c0);
             { StageTimer t(h, BSE_ST_INV_STICK, uniq * c * m.stick_flops, uniq * c * (m.z + m.g));
-              if ((rc = bse_launch_inv_stick(h->fft, h->tau_g, c, h->Z, h->stream, h->adj, e0 + c0))) return rc; }
+              if ((rc = bse_launch_inv_stick(h->fft, h->tau_g, c, h->Z, h->stream, h->batch_pairs, bt.u0 + c0))) return rc; }
             { StageTimer t(h, BSE_ST_INV_PLANE, uniq * c * m.plane_flops, uniq * c * (m.N8 + m.z));
               if ((rc = bse_launch_inv_plane(h->fft, h->Z, c, h->N, h->tau_batch + (long long)c0 * h->N, h->stream))) return rc; }
         }
         { StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)h->N * cnt,
-                       m.N8 * (uniq * cnt + nb * rows + (v0 == 0 ? (double)nb * h->Nv : 0.0)));
-          if (acc_real) rc = bse_launch_accumulate_rows(h, h->tau_batch, e0, v0, rows, a, acc_real, h->Nv, 0, nb);
-          else rc = bse_launch_accumulate_rows(h, h->tau_batch, e0, v0, rows, a, h->acc_r, h->rows_cap, v0, nb);
+                       m.N8 * (uniq * bt.nu + nb * rows + (v0 == 0 ? (double)nb * h->Nv : 0.0)));
+          if (acc_real) rc = bse_launch_accumulate_rows(h, h->tau_batch, h->eslot, v0, rows, a, acc_real, h->Nv, 0, nb);
+          else rc = bse_launch_accumulate_rows(h, h->tau_batch, h->eslot, v0, rows, a, h->acc_r, h->rows_cap, v0, nb);
           if (rc) return rc; }
         if (out_pw && (rc = rows_to_pw(h, h->acc_r, h->rows_cap, rows, nb, out_pw, v0))) return rc;
-        v0 = v1;
     }
     return BSE_OK;
 }
@@ -565,6 +603,7 @@ extern "C" int bse_destroy(bse_handle *h) {
     cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);
     cudaFree(h->part); cudaFree(h->Sov); cudaFree(h->tau_batch); cudaFree(h->a_dev); cudaFree(h->out_dev);
     cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->a_r); cudaFree(h->acc_r);
+    cudaFree(h->batch_pairs); cudaFree(h->eslot);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
     delete h;

@@ -54,7 +54,7 @@ int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2
     return ((const FftOps *)pl.ops)->fwd_stick(to_dev(pl), Z, count, X, pl.npw_h, scale, s);
 }
 int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2 *Z, cudaStream_t s,
-                         const int2 *gather, int g0) {
+                         const int *gather, int g0) {
     if (count <= 0) return BSE_OK;
     return ((const FftOps *)pl.ops)->inv_stick(to_dev(pl), T, count, pl.npw_h, Z, s, gather, g0);
 }

@@ -317,7 +317,7 @@ fwd_stick_kernel(PlanDev P, const double2 *__restrict__ Z, double2 *__restrict__
 template <int R1, int R2>
 __global__ void __launch_bounds__(256)
 inv_stick_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, double2 *__restrict__ Z,
-                 const int2 *__restrict__ gather, int g0) {
+                 const int *__restrict__ gather, int g0) {
     using G = Geo<R1, R2>;
     constexpr int n = G::n, LDS = G::LDS, R2p = G::R2p, TS = G::TS;
     extern __shared__ __align__(16) unsigned char smem[];
@@ -327,7 +327,7 @@ inv_stick_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, doub
     const int NS = P.NS;
     const int s0 = blockIdx.x * TS;
     const long long p = blockIdx.y;
-    const double2 *tg = T + (gather ? (long long)gather[g0 + p].y : p) * npw_h;
+    const double2 *tg = T + (gather ? (long long)gather[g0 + p] : p) * npw_h;
     __syncthreads();
     for (int task = threadIdx.x; task < TS * R2; task += blockDim.x) {
         const int j = task / TS, sl = task - j * TS;
@@ -369,7 +369,7 @@ struct FftOps {
     int (*fwd_plane)(const PlanDev &, const double *, const int2 *, long long, int, long long, double2 *, cudaStream_t);
     int (*inv_plane)(const PlanDev &, const double2 *, int, long long, double *, cudaStream_t);
     int (*fwd_stick)(const PlanDev &, const double2 *, int, double2 *, long long, const double *, cudaStream_t);
-    int (*inv_stick)(const PlanDev &, const double2 *, int, long long, double2 *, cudaStream_t, const int2 *, int);
+    int (*inv_stick)(const PlanDev &, const double2 *, int, long long, double2 *, cudaStream_t, const int *, int);
 };
 
 inline int plane_threads(int tasks) {
@@ -423,7 +423,7 @@ struct Launch {
         return BSE_OK;
     }
     static int inv_stick(const PlanDev &P, const double2 *T, int count, long long npw_h, double2 *Z, cudaStream_t s,
-                         const int2 *gather, int g0) {
+                         const int *gather, int g0) {
         int rc = set_smem((const void *)inv_stick_kernel<R1, R2>, G::stick_smem);
         if (rc) return rc;
         for (int c0 = 0; c0 < count; c0 += 65535) {

@@ -149,13 +149,15 @@ accumulate_kernel(const double *__restrict__ tau, long long p_first, long long p
     }
 }
 
-// Row-complete form used with the batched tau modes: the batch holds tau of EVERY directed entry e of rows
-// [v0, v0 + gridDim.x) (tau_dir[e - e0] = tau of pair adj[e].y), so each output row is written once, never re-read:
-//   acc[(b * acc_ld + v - v_base)][r] = sum_{e in row v} tau_dir[e - e0][r] * a[b][adj[e].x][r]
+// Row-complete form used with the batched tau modes: the batch holds tau(r) of every pair that rows
+// [v0, v0 + gridDim.x) touch, once (a pair with both ends in the batch serves both rows); eslot[e] is the slot of
+// directed entry e in the batch.  Each output row is written once, never re-read:
+//   acc[(b * acc_ld + v - v_base)][r] = sum_{e in row v} tau_b[eslot[e]][r] * a[b][adj[e].x][r]
 // grid = (rows, ceil(N / (2*blockDim))); rows vary fastest across resident CTAs, so they share the r-tile of a in L2.
 template <int BB>
 __global__ void __launch_bounds__(256)
-accumulate_rows_kernel(const double *__restrict__ tau_dir, int e0, int v0, const int *__restrict__ adj_ptr,
+accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict__ eslot, int v0,
+                       const int *__restrict__ adj_ptr,
                        const int2 *__restrict__ adj, const double *__restrict__ a, double *__restrict__ acc, int Nv,
                        long long N, int b0, long long acc_ld, int v_base) {
     const int v = v0 + blockIdx.x;
@@ -167,7 +169,7 @@ accumulate_rows_kernel(const double *__restrict__ tau_dir, int e0, int v0, const
     for (int b = 0; b < BB; ++b) s[b] = make_double2(0.0, 0.0);
     for (int e = ea; e < eb; ++e) {
         const int w = adj[e].x;
-        const double2 t = *reinterpret_cast<const double2 *>(tau_dir + (long long)(e - e0) * N + r);
+        const double2 t = *reinterpret_cast<const double2 *>(tau_dir + (long long)eslot[e] * N + r);
 #pragma unroll
         for (int b = 0; b < BB; ++b) {
             const double2 x = *reinterpret_cast<const double2 *>(a + ((long long)(b0 + b) * Nv + w) * N + r);
@@ -209,6 +211,9 @@ int bse_launch_pairlist(bse_handle *h) {
     BSE_CUDA(cudaStreamSynchronize(h->stream));
     h->P = P;
     h->nadj = nadj = h->adj_ptr_h[Nv];
+    h->adj_h.resize((size_t)nadj * 2);         // (w, pair) of every directed entry: row batches are planned on the host
+    BSE_CUDA(cudaMemcpyAsync(h->adj_h.data(), h->adj, (size_t)nadj * 8, cudaMemcpyDeviceToHost, h->stream));
+    BSE_CUDA(cudaStreamSynchronize(h->stream));
     return BSE_OK;
 }
 
@@ -242,14 +247,14 @@ int bse_launch_accumulate(bse_handle *h, const double *tau, long long p_first, l
     return BSE_OK;
 }
 
-int bse_launch_accumulate_rows(bse_handle *h, const double *tau_dir, int e0, int v0, int nrows, const double *a,
+int bse_launch_accumulate_rows(bse_handle *h, const double *tau_dir, const int *eslot, int v0, int nrows, const double *a,
                                double *acc, long long acc_ld, int v_base, int B) {
     const int threads = 256;
     const long long tiles = (h->N / 2 + threads - 1) / threads;
     dim3 grid(nrows, (unsigned)tiles);
     int b0 = 0;
 #define BSE_ROWS(BB)                                                                                              \
-    accumulate_rows_kernel<BB><<<grid, threads, 0, h->stream>>>(tau_dir, e0, v0, h->adj_ptr, h->adj, a, acc, h->Nv, \
+    accumulate_rows_kernel<BB><<<grid, threads, 0, h->stream>>>(tau_dir, eslot, v0, h->adj_ptr, h->adj, a, acc, h->Nv, \
                                                                 h->N, b0, acc_ld, v_base)
     while (b0 < B) {
         const int left = B - b0;
