@@ -52,10 +52,12 @@ struct StageTimer {
     }
 };
 
-int build_fft_plan(bse_handle *h) {
-    FftPlan &pl = h->fft;
-    const int n = h->n;
+// Tables of one FFT grid of edge n (the problem's grid, or the coarser apply grid of the PW layout).  The order of H is
+// the normative one of the PROBLEM grid h->n whatever n is, so PW arrays mean the same thing on both grids.
+int build_fft_plan(bse_handle *h, FftPlan &pl, int n) {
     pl.n = n;
+    pl.N = (long long)n * n * n;
+    const int nkey = h->n;
     int rc;
     if ((rc = bse_fft_select(pl))) return rc;
     const int msq = h->msq_max;
@@ -71,7 +73,7 @@ int build_fft_plan(bse_handle *h) {
                 if (m1 * m1 + m2 * m2 + m3 * m3 > msq) continue;
                 const bool half = (m3 > 0) || (m3 == 0 && m2 > 0) || (m3 == 0 && m2 == 0 && m1 >= 0);
                 if (!half) continue;
-                const long long key = ((long long)((m1 + n) % n) * n + (m2 + n) % n) * n + (m3 + n) % n;
+                const long long key = ((long long)((m1 + nkey) % nkey) * nkey + (m2 + nkey) % nkey) * nkey + (m3 + nkey) % nkey;
                 H.push_back({m1, m2, m3, key});
             }
     std::sort(H.begin(), H.end(), [](const M3 &a, const M3 &b) { return a.key < b.key; });
@@ -87,8 +89,8 @@ int build_fft_plan(bse_handle *h) {
         h->mill[3 * i] = H[i].m1; h->mill[3 * i + 1] = H[i].m2; h->mill[3 * i + 2] = H[i].m3;
         const int q = H[i].m1 * H[i].m1 + H[i].m2 * H[i].m2 + H[i].m3 * H[i].m3;
         vc12[i] = q == 0 ? 0.0 : std::sqrt(4.0 * M_PI) / (twopi_L * std::sqrt((double)q));
-        vc12n[i] = vc12[i] / (2.0 * (double)h->N);
-        inv2n[i] = 1.0 / (2.0 * (double)h->N);
+        vc12n[i] = vc12[i] / (2.0 * (double)pl.N);
+        inv2n[i] = 1.0 / (2.0 * (double)pl.N);
     }
     // half sticks ordered by (t2 = m2 mod n, m3): stick index = soff[t2] + m3 for wmin[t2] <= m3 <= wmax[t2]
     std::vector<int> soff(n, 0), wmax(n, -1), wmin(n, 0);
@@ -150,36 +152,36 @@ inline long long ldS(const bse_handle *h) { return (h->Nv + 1) & ~1; }
 // planes Z; g = bytes of one field on H.
 struct Model {
     double lg, N8, z, g, plane_flops, stick_flops;
-    explicit Model(const bse_handle *h) {
-        const double n = h->n;
+    explicit Model(const FftPlan &pl) {
+        const double n = pl.n;
         lg = std::log2(n);
-        N8 = 8.0 * (double)h->N;
-        z = 16.0 * n * h->fft.NS;
-        g = 16.0 * (double)h->fft.npw_h;
-        plane_flops = 2.5 * n * n * n * lg + 5.0 * n * n * h->fft.W * lg;     // n^2 real rows + n W kept columns
-        stick_flops = 5.0 * n * lg * h->fft.NS;
+        N8 = 8.0 * (double)pl.N;
+        z = 16.0 * n * pl.NS;
+        g = 16.0 * (double)pl.npw_h;
+        plane_flops = 2.5 * n * n * n * lg + 5.0 * n * n * pl.W * lg;         // n^2 real rows + n W kept columns
+        stick_flops = 5.0 * n * lg * pl.NS;
     }
 };
 
-int st_fwd_plane(bse_handle *h, const double *fields, const int2 *pairs, long long p0, int cnt) {
-    const Model m(h);
+int st_fwd_plane(bse_handle *h, const FftPlan &pl, const double *fields, const int2 *pairs, long long p0, int cnt) {
+    const Model m(pl);
     StageTimer t(h, BSE_ST_FWD_PLANE, cnt * m.plane_flops, cnt * (m.N8 + m.z));
-    return bse_launch_fwd_plane(h->fft, fields, pairs, p0, cnt, h->N, h->Z, h->stream);
+    return bse_launch_fwd_plane(pl, fields, pairs, p0, cnt, pl.N, h->Z, h->stream);
 }
-int st_fwd_stick(bse_handle *h, int cnt, double2 *X, const double *scale) {
-    const Model m(h);
+int st_fwd_stick(bse_handle *h, const FftPlan &pl, int cnt, double2 *X, const double *scale) {
+    const Model m(pl);
     StageTimer t(h, BSE_ST_FWD_STICK, cnt * m.stick_flops, cnt * (m.z + m.g));
-    return bse_launch_fwd_stick(h->fft, h->Z, cnt, X, scale, h->stream);
+    return bse_launch_fwd_stick(pl, h->Z, cnt, X, scale, h->stream);
 }
-int st_inv_stick(bse_handle *h, const double2 *T, int cnt) {
-    const Model m(h);
+int st_inv_stick(bse_handle *h, const FftPlan &pl, const double2 *T, int cnt) {
+    const Model m(pl);
     StageTimer t(h, BSE_ST_INV_STICK, cnt * m.stick_flops, cnt * (m.z + m.g));
-    return bse_launch_inv_stick(h->fft, T, cnt, h->Z, h->stream);
+    return bse_launch_inv_stick(pl, T, cnt, h->Z, h->stream);
 }
-int st_inv_plane(bse_handle *h, int cnt, double *out) {
-    const Model m(h);
+int st_inv_plane(bse_handle *h, const FftPlan &pl, int cnt, double *out) {
+    const Model m(pl);
     StageTimer t(h, BSE_ST_INV_PLANE, cnt * m.plane_flops, cnt * (m.N8 + m.z));
-    return bse_launch_inv_plane(h->fft, h->Z, cnt, h->N, out, h->stream);
+    return bse_launch_inv_plane(pl, h->Z, cnt, pl.N, out, h->stream);
 }
 // C[M][Nn] = alpha colscale[n] sum_k A[m][k] B[n][k]   (split-K DMMA)
 int st_gemm_dot(bse_handle *h, int stage, const double *A, long long lda, const double *B, long long ldb, int M, int Nn,
@@ -199,7 +201,7 @@ int st_gemm_nn(bse_handle *h, int stage, const double *A, long long lda, const d
 // first batch); flops 2 nb N per directed pair
 int st_accumulate(bse_handle *h, const double *tau, long long p0, long long cnt, const double *a, double *acc, int nb,
                   bool first) {
-    const Model m(h);
+    const Model m(h->fft);
     const double directed = (double)h->nadj * (double)cnt / (double)std::max<long long>(h->P, 1);
     StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)h->N * directed,
                  m.N8 * ((double)cnt + (first ? 2.0 * nb * h->Nv : 0.0)));
@@ -211,15 +213,15 @@ int run_pair_batch(bse_handle *h, long long p0, int cnt, double2 *dstG, double *
     const FftPlan &pl = h->fft;
     const long long K2 = 2 * pl.npw_h;
     int rc;
-    if ((rc = st_fwd_plane(h, h->u, h->pairs, p0, cnt))) return rc;
-    if ((rc = st_fwd_stick(h, cnt, h->X, pl.vc12n))) return rc;
+    if ((rc = st_fwd_plane(h, pl, h->u, h->pairs, p0, cnt))) return rc;
+    if ((rc = st_fwd_stick(h, pl, cnt, h->X, pl.vc12n))) return rc;
     if ((rc = st_gemm_dot(h, BSE_ST_PROJECT, (const double *)h->X, K2, h->phi, K2, cnt, h->Npdep, K2, false, h->Dm,
                           ldD(h), 1.0, h->f2))) return rc;
     if ((rc = st_gemm_nn(h, BSE_ST_BACKPROJECT, h->Dm, ldD(h), h->phi, K2, cnt, K2, h->Npdep, EPI_TAU,
                          (const double *)h->X, pl.vc12, (double *)dstG, K2))) return rc;
     if (dstR) {
-        if ((rc = st_inv_stick(h, dstG, cnt))) return rc;
-        if ((rc = st_inv_plane(h, cnt, dstR))) return rc;
+        if ((rc = st_inv_stick(h, pl, dstG, cnt))) return rc;
+        if ((rc = st_inv_plane(h, pl, cnt, dstR))) return rc;
     }
     return BSE_OK;
 }
@@ -267,8 +269,8 @@ int ensure_u_pw(bse_handle *h) {
     int rc;
     for (long long v0 = 0; v0 < h->Nv; v0 += h->Pb) {
         const int cnt = (int)std::min<long long>(h->Pb, h->Nv - v0);
-        if ((rc = st_fwd_plane(h, h->u, nullptr, v0, cnt))) return rc;
-        if ((rc = st_fwd_stick(h, cnt, h->uG + v0 * pl.npw_h, pl.inv2n))) return rc;
+        if ((rc = st_fwd_plane(h, pl, h->u, nullptr, v0, cnt))) return rc;
+        if ((rc = st_fwd_stick(h, pl, cnt, h->uG + v0 * pl.npw_h, pl.inv2n))) return rc;
     }
     return bse_launch_weight_pw(h->uG, h->uGw, pl.npw_h, h->Nv, h->Omega, h->stream);
 }
@@ -377,7 +379,7 @@ int plan_apply_memory(bse_handle *h, int B) {
     h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
     size_t free_b = 0, total_b = 0;
     cudaMemGetInfo(&free_b, &total_b);
-    const double N8 = 8.0 * (double)h->N;
+    const double N8 = 8.0 * (double)h->ap->N;      // staging lives on the apply grid
     const double avail = 0.92 * (double)free_b - 512.0 * 1048576.0;   // leave the caller some room
     const double avgdeg = std::max(1.0, (double)h->nadj / h->Nv);
     int maxdeg = 1;
@@ -415,10 +417,10 @@ int plan_apply_memory(bse_handle *h, int B) {
         pacc = pacc_of(bg);
         rows_cap = std::min<long long>(h->Nv, std::max<long long>(1, (long long)(2.0 * pacc / avgdeg)));
     }
-    if (pacc) BSE_CUDA(cudaMalloc(&h->tau_batch, (size_t)pacc * h->N * 8));
+    if (pacc) BSE_CUDA(cudaMalloc(&h->tau_batch, (size_t)pacc * h->ap->N * 8));
     if (bg) {
-        BSE_CUDA(cudaMalloc(&h->a_r, (size_t)bg * h->Nv * h->N * 8));
-        BSE_CUDA(cudaMalloc(&h->acc_r, (size_t)bg * rows_cap * h->N * 8));
+        BSE_CUDA(cudaMalloc(&h->a_r, (size_t)bg * h->Nv * h->ap->N * 8));
+        BSE_CUDA(cudaMalloc(&h->acc_r, (size_t)bg * rows_cap * h->ap->N * 8));
     }
     h->Bg = (int)bg; h->Bg_final = bg < B; h->Pacc = pacc; h->rows_cap = (int)rows_cap;
     if (batched) {
@@ -432,13 +434,14 @@ int plan_apply_memory(bse_handle *h, int B) {
 
 // forward transform of `rows` accumulated fields of each of nb blocks into the PW output (a12): acc(G) on H
 int rows_to_pw(bse_handle *h, const double *acc, long long acc_ld, int rows, int nb, double2 *out_pw, int v0) {
-    const long long npw_h = h->fft.npw_h;
+    const FftPlan &pl = *h->ap;
+    const long long npw_h = pl.npw_h;
     int rc;
     for (int b = 0; b < nb; ++b)
         for (int r0 = 0; r0 < rows; r0 += (int)h->Pb) {
             const int cnt = (int)std::min<long long>(h->Pb, rows - r0);
-            if ((rc = st_fwd_plane(h, acc + (long long)b * acc_ld * h->N, nullptr, r0, cnt))) return rc;
-            if ((rc = st_fwd_stick(h, cnt, out_pw + ((long long)b * h->Nv + v0 + r0) * npw_h, h->fft.inv2n))) return rc;
+            if ((rc = st_fwd_plane(h, pl, acc + (long long)b * acc_ld * pl.N, nullptr, r0, cnt))) return rc;
+            if ((rc = st_fwd_stick(h, pl, cnt, out_pw + ((long long)b * h->Nv + v0 + r0) * npw_h, pl.inv2n))) return rc;
         }
     return BSE_OK;
 }
@@ -456,7 +459,8 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
         if ((rc = st_accumulate(h, h->tau_r, 0, h->P, a, acc, nb, true))) return rc;
         return out_pw ? rows_to_pw(h, acc, h->Nv, h->Nv, nb, out_pw, 0) : BSE_OK;
     }
-    const Model m(h);
+    const FftPlan &pl = *h->ap;
+    const Model m(pl);
     const std::vector<int> &ap = h->adj_ptr_h;
     const double uniq = h->uniq_share;        // share of the inverted fields that is algorithmic work (each pair once)
     for (const bse_handle::RowBatch &bt : h->batches) {
@@ -464,14 +468,14 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
         for (int c0 = 0; c0 < bt.nu; c0 += (int)h->Pb) {              // tau(G) -> tau(r) of the batch's pairs
             const int c = (int)std::min<long long>(h->Pb, bt.nu - c0);
             { StageTimer t(h, BSE_ST_INV_STICK, uniq * c * m.stick_flops, uniq * c * (m.z + m.g));
-              if ((rc = bse_launch_inv_stick(h->fft, h->tau_g, c, h->Z, h->stream, h->batch_pairs, bt.u0 + c0))) return rc; }
+              if ((rc = bse_launch_inv_stick(pl, h->tau_g, c, h->Z, h->stream, h->batch_pairs, bt.u0 + c0))) return rc; }
             { StageTimer t(h, BSE_ST_INV_PLANE, uniq * c * m.plane_flops, uniq * c * (m.N8 + m.z));
-              if ((rc = bse_launch_inv_plane(h->fft, h->Z, c, h->N, h->tau_batch + (long long)c0 * h->N, h->stream))) return rc; }
+              if ((rc = bse_launch_inv_plane(pl, h->Z, c, pl.N, h->tau_batch + (long long)c0 * pl.N, h->stream))) return rc; }
         }
-        { StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)h->N * cnt,
+        { StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)pl.N * cnt,
                        m.N8 * (uniq * bt.nu + nb * rows + (v0 == 0 ? (double)nb * h->Nv : 0.0)));
-          if (acc_real) rc = bse_launch_accumulate_rows(h, h->tau_batch, h->eslot, v0, rows, a, acc_real, h->Nv, 0, nb);
-          else rc = bse_launch_accumulate_rows(h, h->tau_batch, h->eslot, v0, rows, a, h->acc_r, h->rows_cap, v0, nb);
+          if (acc_real) rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, v0, rows, a, acc_real, h->Nv, 0, nb);
+          else rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, v0, rows, a, h->acc_r, h->rows_cap, v0, nb);
           if (rc) return rc; }
         if (out_pw && (rc = rows_to_pw(h, h->acc_r, h->rows_cap, rows, nb, out_pw, v0))) return rc;
     }
@@ -480,7 +484,7 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
 
 // PW layout (a12): a, out = [B][Nv][npw_h] complex on H
 int apply_pw(bse_handle *h, const double2 *a, double2 *out, int B) {
-    const FftPlan &pl = h->fft;
+    const FftPlan &pl = *h->ap;
     int rc;
     if ((rc = ensure_u_pw(h))) return rc;
     const long long Nv = h->Nv, npw_h = pl.npw_h;
@@ -490,8 +494,8 @@ int apply_pw(bse_handle *h, const double2 *a, double2 *out, int B) {
         const double2 *ag = a + (long long)b0 * Nv * npw_h;
         for (long long f0 = 0; f0 < fields; f0 += h->Pb) {           // a(G) -> a(r)
             const int cnt = (int)std::min<long long>(h->Pb, fields - f0);
-            if ((rc = st_inv_stick(h, ag + f0 * npw_h, cnt))) return rc;
-            if ((rc = st_inv_plane(h, cnt, h->a_r + f0 * h->N))) return rc;
+            if ((rc = st_inv_stick(h, pl, ag + f0 * npw_h, cnt))) return rc;
+            if ((rc = st_inv_plane(h, pl, cnt, h->a_r + f0 * pl.N))) return rc;
         }
         if ((rc = accumulate_all(h, h->a_r, nb, nullptr, out + (long long)b0 * Nv * npw_h))) return rc;
     }
@@ -543,7 +547,20 @@ extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cel
     int rc = BSE_OK;
     auto fail = [&](int code) { bse_destroy(h); return code; };
     if (2 * R >= h->n) { bse_set_error("sphere does not fit the grid (R >= n/2)"); return fail(BSE_EINVAL); }
-    if ((rc = build_fft_plan(h))) return fail(rc);
+    if ((rc = build_fft_plan(h, h->fft, h->n))) return fail(rc);
+    // Apply grid of the PW layout: tau(r) a(r) is a product of two functions band-limited to |m| <= R per axis, so its
+    // components inside S are alias-free on any grid with n_a >= 3R + 1; the apply then moves (n_a / n)^3 of the bytes.
+    // (The REAL layout is defined on the problem grid, and a BSE_TAU_REAL store holds tau on it, so both keep n.)
+    h->ap = &h->fft;
+    if ((flags & BSE_VEC_PW) && (flags & BSE_TAU_MASK) != BSE_TAU_REAL) {
+        static const int sizes[] = {12, 16, 20, 24, 30, 32, 36, 40, 48, 60, 64, 72, 80, 96, 100, 108, 120, 128, 144, 160};
+        for (int na : sizes)
+            if (na >= 3 * R + 1 && na < h->n) {
+                if ((rc = build_fft_plan(h, h->ffta, na))) return fail(rc);
+                h->ap = &h->ffta;
+                break;
+            }
+    }
     if ((long long)Npdep > 2 * (h->fft.npw_h - 1)) { bse_set_error("Npdep > 2 (Npw_h - 1)"); return fail(BSE_EINVAL); }
     const long long K2 = 2 * h->fft.npw_h;
     if (flags & BSE_PTR_HOST) {
@@ -598,6 +615,7 @@ extern "C" int bse_destroy(bse_handle *h) {
     if (!h) return BSE_OK;
     cudaStreamSynchronize(h->stream);
     free_plan(h->fft);
+    free_plan(h->ffta);
     cudaFree(h->u_owned); cudaFree(h->phi_owned); cudaFree(h->f2); cudaFree(h->Mmat); cudaFree(h->rowcnt);
     cudaFree(h->rowptr); cudaFree(h->pid); cudaFree(h->pairs); cudaFree(h->adj_ptr); cudaFree(h->adj);
     cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);

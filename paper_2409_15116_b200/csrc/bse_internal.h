@@ -13,6 +13,7 @@
 // by (m2 mod n, m3).
 struct FftPlan {
     int n = 0, R1 = 0, R2 = 0;
+    long long N = 0;     // n^3
     int R = 0;           // floor(sqrt(msq_max))
     int W = 0;           // kept m3 columns in the plane pass: m3 = 0..R  -> W = R + 1
     int NS = 0;          // number of half sticks
@@ -42,7 +43,9 @@ struct bse_handle {
     const double *phi = nullptr;     // device [Npdep][2 Npw_h]
     double *u_owned = nullptr, *phi_owned = nullptr;
     std::vector<int> mill;           // host [npw_h][3]
-    FftPlan fft;
+    FftPlan fft;                     // the problem grid n
+    FftPlan ffta;                    // coarser apply grid of the PW layout (n_a >= 3R+1), if one exists
+    const FftPlan *ap = nullptr;     // grid the apply runs on: &ffta or &fft
     double *f2 = nullptr;            // device [Npdep]  2 lambda/(1-lambda)
     // screen / pair list
     double *Mmat = nullptr;          // device [Nv][Nv]  sum_r u_v^2 u_w^2
@@ -127,7 +130,7 @@ int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, 
 // k1x_kernels.cu
 int bse_launch_pairlist(bse_handle *h);                 // M -> rowcnt,rowptr,pid,pairs (count only if pairs==nullptr)
 // row-complete accumulation of rows [v0, v0+nrows): tau_b[eslot[e]] for every directed entry e of those rows
-int bse_launch_accumulate_rows(bse_handle *h, const double *tau_b, const int *eslot, int v0, int nrows, const double *a,
+int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_b, const int *eslot, int v0, int nrows, const double *a,
                                double *acc, long long acc_ld, int v_base, int B);
 // dst[w][k] = Omega * wt * src[w][k], wt = 2 for G != 0 and (1, 0) on (re, im) of G = 0 (entry 0 of H)
 int bse_launch_weight_pw(const double2 *src, double2 *dst, long long npw_h, long long rows, double Omega,

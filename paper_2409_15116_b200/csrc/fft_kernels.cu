@@ -5,7 +5,7 @@
 namespace bsefft {
 FftOps ops_12(); FftOps ops_16(); FftOps ops_20(); FftOps ops_24(); FftOps ops_30(); FftOps ops_32(); FftOps ops_36();
 FftOps ops_40(); FftOps ops_48(); FftOps ops_60(); FftOps ops_64(); FftOps ops_72(); FftOps ops_80(); FftOps ops_96();
-FftOps ops_100(); FftOps ops_120(); FftOps ops_128(); FftOps ops_144(); FftOps ops_160();
+FftOps ops_100(); FftOps ops_108(); FftOps ops_120(); FftOps ops_128(); FftOps ops_144(); FftOps ops_160();
 }  // namespace bsefft
 
 using bsefft::FftOps;
@@ -15,7 +15,7 @@ static const FftOps *find_ops(int n) {
     static const FftOps table[] = {
         bsefft::ops_12(), bsefft::ops_16(), bsefft::ops_20(), bsefft::ops_24(), bsefft::ops_30(), bsefft::ops_32(),
         bsefft::ops_36(), bsefft::ops_40(), bsefft::ops_48(), bsefft::ops_60(), bsefft::ops_64(), bsefft::ops_72(),
-        bsefft::ops_80(), bsefft::ops_96(), bsefft::ops_100(), bsefft::ops_120(), bsefft::ops_128(), bsefft::ops_144(),
+        bsefft::ops_80(), bsefft::ops_96(), bsefft::ops_100(), bsefft::ops_108(), bsefft::ops_120(), bsefft::ops_128(), bsefft::ops_144(),
         bsefft::ops_160()};
     for (const FftOps &o : table)
         if (o.n == n) return &o;
@@ -25,7 +25,7 @@ static const FftOps *find_ops(int n) {
 int bse_fft_select(FftPlan &pl) {
     const FftOps *o = find_ops(pl.n);
     if (!o) {
-        bse_set_error("no FFT kernel for this grid edge (supported n: 12 16 20 24 30 32 36 40 48 60 64 72 80 96 100 120 128 144 160)");
+        bse_set_error("no FFT kernel for this grid edge (supported n: 12 16 20 24 30 32 36 40 48 60 64 72 80 96 100 108 120 128 144 160)");
         return BSE_EUNSUPPORTED;
     }
     pl.R1 = o->R1; pl.R2 = o->R2; pl.ops = o;

@@ -46,6 +46,14 @@ struct Geo {
     static __host__ __device__ constexpr int natslot(int e) { return (e / R2) * R2p + e % R2; }
     static __host__ __device__ constexpr int fwdslot(int k) { return (k % R1) * R2p + k / R1; }
     static constexpr int plane_smem = (n / 2) * LD * 16 + n * 16 + 3 * n * 4;
+    // plane kernels: threads per CTA (one sweep of the rows pass per <= 512 threads) and the CTAs per SM to compile for
+    static constexpr int plane_tasks = (n / 2) * R2;
+    static constexpr int plane_iters = (plane_tasks + 511) / 512;
+    static constexpr int plane_thr = (((plane_tasks + plane_iters - 1) / plane_iters + 31) / 32 * 32) < 64
+                                         ? 64 : ((plane_tasks + plane_iters - 1) / plane_iters + 31) / 32 * 32;
+    static constexpr int smem_ctas = 232448 / (plane_smem + 1024);
+    static constexpr int reg_ctas = 65536 / (plane_thr * 100);          // keep >= 100 registers per thread
+    static constexpr int plane_minb = smem_ctas < reg_ctas ? (smem_ctas < 1 ? 1 : smem_ctas) : (reg_ctas < 1 ? 1 : reg_ctas);
     static constexpr int stick_smem = TS * LDS * 16 + n * 16;
 };
 
@@ -70,7 +78,7 @@ __device__ __forceinline__ void plane_tables(unsigned char *smem, const PlanDev 
 // the single field p0+p (no product: forward wrapper of the PW layout, step a12).
 // Output carries a factor 2 (the 1/2 of the two-row untangling is folded into the stick pass's scale).
 template <int R1, int R2>
-__global__ void __launch_bounds__(512)
+__global__ void __launch_bounds__(Geo<R1, R2>::plane_thr, Geo<R1, R2>::plane_minb)
 fwd_plane_kernel(PlanDev P, const double *__restrict__ fields, const int2 *__restrict__ pairs, long long p0,
                  long long N, double2 *__restrict__ Z) {
     using G = Geo<R1, R2>;
@@ -173,7 +181,7 @@ fwd_plane_kernel(PlanDev P, const double *__restrict__ fields, const int2 *__res
 // ---------------------------------------------------------------------------------------------------------
 // inverse plane pass.  grid = (n planes, count).  Z[p][i1][NS] -> out[p][N] real.
 template <int R1, int R2>
-__global__ void __launch_bounds__(512)
+__global__ void __launch_bounds__(Geo<R1, R2>::plane_thr, Geo<R1, R2>::plane_minb)
 inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out) {
     using G = Geo<R1, R2>;
     constexpr int n = G::n, LD = G::LD, R2p = G::R2p;
@@ -381,15 +389,17 @@ inline int plane_threads(int tasks) {
 template <int R1, int R2>
 struct Launch {
     using G = Geo<R1, R2>;
-    static int set_smem(const void *fn, int bytes) {
+    static int set_smem(const void *fn, int bytes, bool plane = false) {
         if (bytes > 48 * 1024) BSE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+        if (plane)      // the plane passes live in shared memory: take the whole carve-out so that smem_ctas CTAs fit
+            BSE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         return BSE_OK;
     }
     static int fwd_plane(const PlanDev &P, const double *fields, const int2 *pairs, long long p0, int count, long long N,
                          double2 *Z, cudaStream_t s) {
-        int rc = set_smem((const void *)fwd_plane_kernel<R1, R2>, G::plane_smem);
+        int rc = set_smem((const void *)fwd_plane_kernel<R1, R2>, G::plane_smem, true);
         if (rc) return rc;
-        const int threads = plane_threads((G::n / 2) * R2);
+        const int threads = G::plane_thr;
         for (int c0 = 0; c0 < count; c0 += 65535) {
             const int c = count - c0 < 65535 ? count - c0 : 65535;
             fwd_plane_kernel<R1, R2><<<dim3(G::n, c), threads, G::plane_smem, s>>>(
@@ -399,9 +409,9 @@ struct Launch {
         return BSE_OK;
     }
     static int inv_plane(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s) {
-        int rc = set_smem((const void *)inv_plane_kernel<R1, R2>, G::plane_smem);
+        int rc = set_smem((const void *)inv_plane_kernel<R1, R2>, G::plane_smem, true);
         if (rc) return rc;
-        const int threads = plane_threads((G::n / 2) * R2);
+        const int threads = G::plane_thr;
         for (int c0 = 0; c0 < count; c0 += 65535) {
             const int c = count - c0 < 65535 ? count - c0 : 65535;
             inv_plane_kernel<R1, R2><<<dim3(G::n, c), threads, G::plane_smem, s>>>(

@@ -247,15 +247,15 @@ int bse_launch_accumulate(bse_handle *h, const double *tau, long long p_first, l
     return BSE_OK;
 }
 
-int bse_launch_accumulate_rows(bse_handle *h, const double *tau_dir, const int *eslot, int v0, int nrows, const double *a,
+int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_dir, const int *eslot, int v0, int nrows, const double *a,
                                double *acc, long long acc_ld, int v_base, int B) {
     const int threads = 256;
-    const long long tiles = (h->N / 2 + threads - 1) / threads;
+    const long long tiles = (N / 2 + threads - 1) / threads;
     dim3 grid(nrows, (unsigned)tiles);
     int b0 = 0;
 #define BSE_ROWS(BB)                                                                                              \
     accumulate_rows_kernel<BB><<<grid, threads, 0, h->stream>>>(tau_dir, eslot, v0, h->adj_ptr, h->adj, a, acc, h->Nv, \
-                                                                h->N, b0, acc_ld, v_base)
+                                                                N, b0, acc_ld, v_base)
     while (b0 < B) {
         const int left = B - b0;
         if (left >= 8) { BSE_ROWS(8); b0 += 8; }

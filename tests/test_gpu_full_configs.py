@@ -168,4 +168,4 @@ def test_cfg4_full_size():
 
 def test_cfg5_full_size_streamed():
     from paper_2409_15116_b200 import bse
-    _sampled_full_check(5, bse.BSE_TAU_STREAM, True, screen_rows=[1010], blocks=[15], need_gb=178)
+    _sampled_full_check(5, bse.BSE_TAU_STREAM, True, screen_rows=[1010], blocks=[15], need_gb=150)
