@@ -391,7 +391,7 @@ struct Launch {
     using G = Geo<R1, R2>;
     static int set_smem(const void *fn, int bytes, bool plane = false) {
         if (bytes > 48 * 1024) BSE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-        if (plane)      // the plane passes live in shared memory: take the whole carve-out so that smem_ctas CTAs fit
+        if (plane && bytes >= 64 * 1024)   // large planes: take the whole carve-out so that smem_ctas CTAs fit
             BSE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         return BSE_OK;
     }

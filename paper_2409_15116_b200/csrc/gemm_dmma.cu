@@ -74,8 +74,11 @@ dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restri
     double *Bs = sm + STAGES * A_TILE;
     constexpr int B_TILE = BN_MAJOR ? B_TILE_N : B_TILE_K;
 
-    const int m0 = blockIdx.y * BM;
-    const long long n0 = (long long)blockIdx.x * BN;
+    // NN form: 1-D grid with the m tile fastest, so the CTAs that share one [K][64] panel of B (the big operand: u or Phi)
+    // run back to back and the panel is read from HBM once.  Dot form: (n tile, m tile, k split).
+    const int tm_ = (M + BM - 1) / BM;
+    const int m0 = (BN_MAJOR ? (int)(blockIdx.x % tm_) : (int)blockIdx.y) * BM;
+    const long long n0 = (long long)(BN_MAJOR ? blockIdx.x / tm_ : blockIdx.x) * BN;
     const long long kbeg = (long long)blockIdx.z * kchunk;
     const long long kend = (kbeg + kchunk < K) ? kbeg + kchunk : K;
     const int nk = (int)((kend - kbeg + BK - 1) / BK);
@@ -246,7 +249,8 @@ int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, 
     if (M <= 0 || N <= 0) return BSE_OK;
     const int tm = (M + BM - 1) / BM;
     const long long tn = (N + BN - 1) / BN;
-    dim3 grid((unsigned)tn, tm, 1);
+    if (tn * tm > 2147483647LL) { bse_set_error("bse_gemm_nn: too many tiles"); return BSE_EUNSUPPORTED; }
+    dim3 grid((unsigned)(tn * tm), 1, 1);
     int rc;
     if (epi == EPI_TAU) {
         auto k = dgemm_kernel<true, EPI_TAU, false, false>;
