@@ -32,6 +32,24 @@ sys.path.insert(0, ROOT)
 METRIC = "screened pair integrals/s (tau build incl. screen; K1x applies/s beside it), fp64, B200"
 
 
+def max_over_ranks(values, dist=None, device=None):
+    """Element-wise MAX over the ranks of the default process group (every rank gets the result).
+    Multi-GPU = independent replicas: the step time of the job is the slowest replica's."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return [float(v) for v in values]
+    import torch
+    t = torch.tensor([float(v) for v in values], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return t.tolist()
+
+
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the kernel behind each stage at cfg2, from the
+# committed ncu --set full capture profiles/r01b_cfg2.md (constants of that capture, not measured by this run).
+NCU_TRAFFIC_CFG2 = {"pc_update": 1570e6, "pc_overlap": 675e6, "k1x_accumulate": 1540e6, "fwd_plane": 316e6,
+                    "inv_plane": 526e6, "fwd_stick": 102e6, "inv_stick": 65e6, "pdep_project": 63e6,
+                    "pdep_backproject": 67e6, "screen_syrk": 138e6}
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -255,10 +273,7 @@ def main():
     prof_counts = bse.bse_profile_get(h)
     P = bse.bse_num_pairs(h)
     tb_ms, ta_ms = float(np.mean(t_build)), float(np.mean(t_apply))
-    if world > 1:
-        t = torch.tensor([tb_ms, ta_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        tb_ms, ta_ms = t.tolist()
+    tb_ms, ta_ms = max_over_ranks([tb_ms, ta_ms], dist if world > 1 else None, dev)
     launches = sum(prof_counts[s][1] * k for s, k in zip(bse.STAGES, bse.KERNELS_PER_STAGE))
 
     # ---- per-stage device times (CUDA events on the library's stream, one extra profiled pass per step) ----
@@ -301,7 +316,9 @@ def main():
     roof["kernel"] = top
     roof["launches_per_step"] = n_launch_top
     roof["ms_per_launch"] = ms_top / n_launch_top
-    roof["traffic"] = None
+    roof["traffic"] = NCU_TRAFFIC_CFG2.get(top) if (args.config == 2 and args.tau == "real" and args.vec == "real") else None
+    roof["traffic_source"] = "profiles/r01b_cfg2.md (ncu --set full, per launch)" if roof["traffic"] else None
+    roof["algorithmic_bytes_per_launch"] = mt["bytes"] / n_launch_top
     tot_f = sum(m["flops"] for m in model.values())
     tot_b = sum(m["bytes"] for m in model.values())
     pipe_roof_ms = 1e3 * max(tot_f / (dmma_tf * 1e12), tot_b / (hbm_gbs * 1e9))
@@ -328,10 +345,7 @@ def main():
                 e2e_build.append(t1 - t0)
                 e2e_apply.append(t2 - t1)
         e2e_b, e2e_a = float(np.mean(e2e_build)), float(np.mean(e2e_apply))
-        if world > 1:
-            t = torch.tensor([e2e_b, e2e_a], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_b, e2e_a = t.tolist()
+        e2e_b, e2e_a = max_over_ranks([e2e_b, e2e_a], dist if world > 1 else None, dev)
         h2d = u_host.numel() * 8 + phi_host.numel() * 8 + a_host.numel() * 8
         d2h = out_host.numel() * 8 + 8
         e2e = {"value": world * P / e2e_b, "unit": "pairs/s", "k1x_applies_per_s": world * B / e2e_a,

@@ -11,7 +11,8 @@
  *                                                               (eq. 5 and PAPER.md:67; the paper's K^1d)
  *
  * Conventions (normative)
- *   grid n1 x n2 x n3 (this version: n1 = n2 = n3 = n even, cubic cell of edge L, else BSE_EUNSUPPORTED),
+ *   grid n1 x n2 x n3 (this version: n1 = n2 = n3 = n in {12 16 20 24 30 32 36 40 48 60 64 72 80 96 100 108 120 128 144
+ *   160}, cubic cell of edge L, else BSE_EUNSUPPORTED),
  *   linear index (i1*n + i2)*n + i3;  r = (L/n) i;  G = (2 pi/L) m;  Hartree atomic units.
  *   sphere S = { m : |m|^2 <= floor(2 ecut (L/2pi)^2 (1+1e-12)) };  R = floor(sqrt(max)) must be < n/2.
  *   half sphere H = { m in S : m3>0 } U { m3=0, m2>0 } U { m3=m2=0, m1>=0 }, sorted by ascending
@@ -43,10 +44,13 @@ enum { BSE_OK = 0, BSE_EINVAL = -1, BSE_ENOMEM = -2, BSE_ECUDA = -3, BSE_ESTATE 
 /* flags of bse_create */
 #define BSE_TAU_REAL   0x0u   /* tau_vv'(r) stored on the real-space grid, [P][N] doubles (default)          */
 #define BSE_TAU_PW     0x1u   /* tau_vv'(G) stored on H, [P][Npw_h] complex; inverse FFT inside the apply     */
-#define BSE_TAU_STREAM 0x2u   /* nothing stored: tau rebuilt in pair batches inside every bse_apply_k1x       */
+#define BSE_TAU_STREAM 0x2u   /* nothing kept between calls: every bse_apply_k1x rebuilds tau(G) in pair batches into
+                                 a transient buffer and streams tau(r) from it in row batches                    */
 #define BSE_TAU_MASK   0x3u
 #define BSE_VEC_REAL   0x0u   /* a/out = [B][Nv][N] real (default)                                            */
-#define BSE_VEC_PW     0x4u   /* a/out = [B][Nv][Npw_h] complex on H ("of length N_pw")         */
+#define BSE_VEC_PW     0x4u   /* a/out = [B][Nv][Npw_h] complex on H ("of length N_pw"); a(0) must be
+                                 real; out = P_c of (sum_v' tau a) truncated to S.  With BSE_TAU_PW/STREAM the products
+                                 are formed on the smallest supported grid n_a >= 3R+1 (alias-free inside S)     */
 #define BSE_PTR_HOST   0x8u   /* u and phi passed to bse_create are HOST pointers (copied to the device)      */
 
 /* Create a problem instance.  Builds the sphere/stick tables, twiddles and v_c^{1/2} on the host and uploads
@@ -68,7 +72,9 @@ int bse_create(bse_handle **h, const int grid[3], const double cell[9], double e
 int bse_build_tau(bse_handle *h);
 
 /* out[b,v] = P_c sum_v' tau_vv' a[b,v'] for B trial blocks.  a, out: DEVICE pointers, layout per
- * BSE_VEC_* flag.  BSE_ESTATE if bse_build_tau has not run. */
+ * BSE_VEC_* flag.  BSE_ESTATE if bse_build_tau has not run.  The first call plans its staging buffers from the device
+ * memory that is free then (up to 92 % of it: tau(r) row batches, real-space copies of a group of trial blocks) and keeps
+ * them; BSE_ENOMEM if one trial block plus one row of pairs does not fit. */
 int bse_apply_k1x(bse_handle *h, const double *a, double *out, int B);
 
 /* Same with HOST pointers: copies a to the device, applies, copies out back, synchronises (the end-to-end
