@@ -218,12 +218,24 @@ int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb,
     const int tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
     const long long ksteps = (K + BK - 1) / BK;
     const long long tiles = (squareA && squareB) ? (long long)tm * (tm + 1) / 2 : (long long)tm * tn;   // SYRK: v <= w tiles
-    long long splits = (2LL * 148 + tiles - 1) / tiles;
-    if (splits > ksteps / 8) splits = ksteps / 8;
-    if (splits < 1) splits = 1;
+    // split K so that the CTAs come in whole waves of 148 (one per SM) and there are at least two per SM: the DMMA pipe
+    // saturates at ~8 warps per SM, while a few CTAs over a multiple of 148 leave most SMs idle for a whole CTA time
+    // (304 CTAs ran 1.5x longer than 288).  More, shorter CTAs only add prologue and partial-sum traffic.
+    const long long sms = 148;
+    long long smax = ksteps / 8;
     const long long cap = (long long)(part_bytes / ((size_t)M * N * 8));
     if (cap < 1) { bse_set_error("bse_gemm_dot: split-K workspace too small"); return BSE_ENOMEM; }
-    if (splits > cap) splits = cap;
+    if (smax > cap) smax = cap;
+    if (smax < 1) smax = 1;
+    long long splits = 1;
+    double best = -1.0;
+    for (long long sp = 1; sp <= smax; ++sp) {
+        const long long ctas = tiles * sp;
+        double eff = (double)ctas / (double)(((ctas + sms - 1) / sms) * sms);
+        if (ctas < 2 * sms) eff *= 0.5 * (double)ctas / (double)sms;          // under two per SM: scaled down
+        if (eff > best + 0.02) { best = eff; splits = sp; }
+        if (ctas >= 8 * sms) break;
+    }
     long long kchunk = ((ksteps + splits - 1) / splits) * BK;
     splits = (K + kchunk - 1) / kchunk;
     dim3 grid(tn, tm, (unsigned)splits);

@@ -126,7 +126,7 @@ accumulate_kernel(const double *__restrict__ tau, long long p_first, long long p
         if (p < 0 || p >= p_count) continue;
         any = true;
         if (r < N) {
-            const double2 t = *reinterpret_cast<const double2 *>(tau + p * N + r);
+            const double2 t = *reinterpret_cast<const double2 *>(tau + p * N + r);   // re-used by row w: keep in L2
 #pragma unroll
             for (int b = 0; b < BB; ++b) {
                 const double2 x = *reinterpret_cast<const double2 *>(a + ((long long)(b0 + b) * Nv + wp.x) * N + r);
@@ -169,7 +169,8 @@ accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict
     for (int b = 0; b < BB; ++b) s[b] = make_double2(0.0, 0.0);
     for (int e = ea; e < eb; ++e) {
         const int w = adj[e].x;
-        const double2 t = *reinterpret_cast<const double2 *>(tau_dir + (long long)eslot[e] * N + r);
+        // tau is read once per use: streaming load, so that it does not push the re-used a tiles out of L2
+        const double2 t = __ldcs(reinterpret_cast<const double2 *>(tau_dir + (long long)eslot[e] * N + r));
 #pragma unroll
         for (int b = 0; b < BB; ++b) {
             const double2 x = *reinterpret_cast<const double2 *>(a + ((long long)(b0 + b) * Nv + w) * N + r);
@@ -179,7 +180,7 @@ accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict
     }
 #pragma unroll
     for (int b = 0; b < BB; ++b)
-        *reinterpret_cast<double2 *>(acc + ((long long)(b0 + b) * acc_ld + (v - v_base)) * N + r) = s[b];
+        __stcs(reinterpret_cast<double2 *>(acc + ((long long)(b0 + b) * acc_ld + (v - v_base)) * N + r), s[b]);
 }
 
 __global__ void weight_pw_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst, long long npw_h,
