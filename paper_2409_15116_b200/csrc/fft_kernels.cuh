@@ -42,7 +42,7 @@ struct Geo {
     static constexpr int R2p = R2 + 1;
     static constexpr int LD = R1 * R2p + ((R2 % 8) ? ((R2 - R1 * R2p) % 8 + 8) % 8 : 0);   // plane line stride (complex)
     static constexpr int LDS = (R1 * R2p) | 1;                                            // stick line stride
-    static constexpr int TS = 16;                                                          // sticks per CTA
+    static constexpr int TS = 32;                                                          // sticks per CTA
     static __host__ __device__ constexpr int natslot(int e) { return (e / R2) * R2p + e % R2; }
     static __host__ __device__ constexpr int fwdslot(int k) { return (k % R1) * R2p + k / R1; }
     static constexpr int plane_smem = (n / 2) * LD * 16 + n * 16 + 3 * n * 4;

@@ -212,9 +212,12 @@ int bse_launch_pairlist(bse_handle *h) {
     BSE_CUDA(cudaStreamSynchronize(h->stream));
     h->P = P;
     h->nadj = nadj = h->adj_ptr_h[Nv];
-    h->adj_h.resize((size_t)nadj * 2);         // (w, pair) of every directed entry: row batches are planned on the host
-    BSE_CUDA(cudaMemcpyAsync(h->adj_h.data(), h->adj, (size_t)nadj * 8, cudaMemcpyDeviceToHost, h->stream));
-    BSE_CUDA(cudaStreamSynchronize(h->stream));
+    h->adj_h.clear();
+    if ((h->flags & BSE_TAU_MASK) != BSE_TAU_REAL) {   // (w, pair) of every directed entry: row batches are planned on the host
+        h->adj_h.resize((size_t)nadj * 2);
+        BSE_CUDA(cudaMemcpyAsync(h->adj_h.data(), h->adj, (size_t)nadj * 8, cudaMemcpyDeviceToHost, h->stream));
+        BSE_CUDA(cudaStreamSynchronize(h->stream));
+    }
     return BSE_OK;
 }
 
