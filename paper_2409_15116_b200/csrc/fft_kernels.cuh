@@ -46,15 +46,18 @@ struct Geo {
     static __host__ __device__ constexpr int natslot(int e) { return (e / R2) * R2p + e % R2; }
     static __host__ __device__ constexpr int fwdslot(int k) { return (k % R1) * R2p + k / R1; }
     static constexpr int plane_smem = (n / 2) * LD * 16 + n * 16 + 3 * n * 4;
-    // plane kernels: threads per CTA (one sweep of the rows pass per <= 512 threads) and the CTAs per SM to compile for
+    // plane kernels: as many CTAs per SM as shared memory allows (they are the only overlap of one plane's load / store
+    // phases with another's butterflies), and per CTA the threads that leave each of them >= ~112 registers
     static constexpr int plane_tasks = (n / 2) * R2;
-    static constexpr int plane_iters = (plane_tasks + 511) / 512;
+    static constexpr int smem_ctas = 232448 / (plane_smem + 1024) < 1 ? 1 : 232448 / (plane_smem + 1024);
+    static constexpr int thr_cap0 = 65536 / (112 * (smem_ctas > 6 ? 6 : smem_ctas)) / 32 * 32;
+    static constexpr int thr_cap = thr_cap0 > 512 ? 512 : (thr_cap0 < 64 ? 64 : thr_cap0);
+    static constexpr int plane_iters = (plane_tasks + thr_cap - 1) / thr_cap;
     static constexpr int plane_thr = (((plane_tasks + plane_iters - 1) / plane_iters + 31) / 32 * 32) < 64
                                          ? 64 : ((plane_tasks + plane_iters - 1) / plane_iters + 31) / 32 * 32;
-    static constexpr int smem_ctas = 232448 / (plane_smem + 1024);
     static constexpr int reg_ctas = 65536 / (plane_thr * 100);          // keep >= 100 registers per thread
     static constexpr int plane_minb = smem_ctas < reg_ctas ? (smem_ctas < 1 ? 1 : smem_ctas) : (reg_ctas < 1 ? 1 : reg_ctas);
-    static constexpr int stick_smem = TS * LDS * 16 + n * 16;
+    static constexpr int stick_smem = TS * LDS * 16;
 };
 
 // shared memory carve-up of the plane kernels: C[(n/2)*LD] | tw[n] | soff[n] | wmax[n] | wmin[n]
@@ -272,7 +275,7 @@ inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// stick passes.  grid = (ceil(NS/TS), count), 256 threads.  smem: C[TS*LDS] | tw[n]
+// stick passes.  grid = (ceil(NS/TS), count), 256 threads.  smem: C[TS*LDS]
 template <int R1, int R2>
 __global__ void __launch_bounds__(256)
 fwd_stick_kernel(PlanDev P, const double2 *__restrict__ Z, double2 *__restrict__ X, long long npw_h,
@@ -281,13 +284,11 @@ fwd_stick_kernel(PlanDev P, const double2 *__restrict__ Z, double2 *__restrict__
     constexpr int n = G::n, LDS = G::LDS, R2p = G::R2p, TS = G::TS;
     extern __shared__ __align__(16) unsigned char smem[];
     double2 *C = reinterpret_cast<double2 *>(smem);
-    double2 *tw = C + TS * LDS;
-    for (int i = threadIdx.x; i < n; i += blockDim.x) tw[i] = P.tw[i];
+    const double2 *tw = P.tw;                 // read through L1: no table copy, no barrier before the first load
     const int NS = P.NS;
     const int s0 = blockIdx.x * TS;
     const long long p = blockIdx.y;
     const double2 *z = Z + p * n * (long long)NS;
-    __syncthreads();
     for (int task = threadIdx.x; task < TS * R2; task += blockDim.x) {
         const int j = task / TS, sl = task - j * TS;
         const int s = s0 + sl;
@@ -330,13 +331,11 @@ inv_stick_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, doub
     constexpr int n = G::n, LDS = G::LDS, R2p = G::R2p, TS = G::TS;
     extern __shared__ __align__(16) unsigned char smem[];
     double2 *C = reinterpret_cast<double2 *>(smem);
-    double2 *tw = C + TS * LDS;
-    for (int i = threadIdx.x; i < n; i += blockDim.x) tw[i] = P.tw[i];
+    const double2 *tw = P.tw;                 // read through L1: no table copy, no barrier before the first load
     const int NS = P.NS;
     const int s0 = blockIdx.x * TS;
     const long long p = blockIdx.y;
     const double2 *tg = T + (gather ? (long long)gather[g0 + p] : p) * npw_h;
-    __syncthreads();
     for (int task = threadIdx.x; task < TS * R2; task += blockDim.x) {
         const int j = task / TS, sl = task - j * TS;
         const int s = s0 + sl;
