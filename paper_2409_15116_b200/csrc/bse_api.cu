@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -416,6 +417,19 @@ int plan_apply_memory(bse_handle *h, int B) {
         while (bg > 1 && (B + bg - 2) / (bg - 1) == groups) --bg;
         pacc = pacc_of(bg);
         rows_cap = std::min<long long>(h->Nv, std::max<long long>(1, (long long)(2.0 * pacc / avgdeg)));
+    }
+    // test hooks: BSE_MAX_GROUP / BSE_MAX_BATCH cap B_g / the row batch so that small cases exercise several groups
+    // and several row batches (tests/test_gpu_parity.py); they never raise a limit
+    if (const char *e = std::getenv("BSE_MAX_GROUP")) {
+        const long long cap_g = std::atoll(e);
+        if (cap_g >= 1 && bg > cap_g) { bg = cap_g; }
+    }
+    if (const char *e = std::getenv("BSE_MAX_BATCH")) {
+        const long long cap_p = std::max<long long>(std::atoll(e), maxdeg);
+        if (pacc > cap_p) {
+            pacc = cap_p;
+            if (pw && batched) rows_cap = std::min<long long>(h->Nv, std::max<long long>(1, (long long)(2.0 * pacc / avgdeg)));
+        }
     }
     if (pacc) BSE_CUDA(cudaMalloc(&h->tau_batch, (size_t)pacc * h->ap->N * 8));
     if (bg) {

@@ -127,6 +127,7 @@ dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restri
         issue(kt + STAGES - 1);
         const double *as = As + (kt % STAGES) * A_TILE;
         const double *bs = Bs + (kt % STAGES) * B_TILE;
+        if (SQA && SQB && m0 == (int)n0 && wm > wn) continue;    // diagonal SYRK tile: the warp below the diagonal idles
 #pragma unroll
         for (int kk = 0; kk < BK; kk += 4) {
             double af[4], bf[4];

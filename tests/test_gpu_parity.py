@@ -135,6 +135,24 @@ def test_pw_layout_all_tau_modes():
     _check_pw(wl.make(2, Nv=12, Npdep=40, B=2), bse.BSE_TAU_PW)
 
 
+def test_several_groups_and_row_batches(monkeypatch):
+    """Small case forced through the large-config machinery: trial blocks in groups of 2 (B = 5: ragged last group) and
+    row batches of at most 7 pairs (several batches, pairs shared between batches re-inverted)."""
+    bse = _bse()
+    monkeypatch.setenv("BSE_MAX_GROUP", "2")
+    monkeypatch.setenv("BSE_MAX_BATCH", "7")
+    cfg = wl.Config("grp", 10.0, 24, 9, 20, 8.0, 1.2, 0.8, 3.0, 0.02, 5, "random", seed=77)
+    w = wl.make(cfg=cfg)
+    o1 = _check_pw(w, bse.BSE_TAU_PW)
+    o2 = _check_pw(w, bse.BSE_TAU_STREAM)
+    assert rel(o2, o1) < 1e-12
+    _check_full(w, bse.BSE_TAU_PW, check_g=False)
+    monkeypatch.delenv("BSE_MAX_GROUP")
+    monkeypatch.delenv("BSE_MAX_BATCH")
+    o3 = _check_pw(w, bse.BSE_TAU_PW)
+    assert rel(o3, o1) < 1e-12
+
+
 def test_cfg1_full_all_modes():
     w = wl.make(1)
     bse = _bse()
