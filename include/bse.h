@@ -78,8 +78,14 @@ int bse_build_tau(bse_handle *h);
 int bse_apply_k1x(bse_handle *h, const double *a, double *out, int B);
 
 /* Same with HOST pointers: copies a to the device, applies, copies out back, synchronises (the end-to-end
- * call bench.py times as `e2e`). */
+ * call bench.py times as `e2e`).  With BSE_TAU_REAL the blocks are pipelined: block b+1 is copied in and block b-1
+ * copied out (two copy streams) while block b is applied.  Pinned host memory is needed for the overlap. */
 int bse_apply_k1x_host(bse_handle *h, const double *a_host, double *out_host, int B);
+
+/* Replace u and/or phi (either may be NULL) of a handle created with BSE_PTR_HOST by new HOST arrays of the same sizes:
+ * host-to-device copy into the buffers the handle owns, enqueued on its stream, nothing reallocated.  tau is invalidated
+ * (call bse_build_tau again).  BSE_ESTATE if the handle borrows device arrays. */
+int bse_set_inputs_host(bse_handle *h, const double *u_host, const double *phi_host);
 
 int bse_destroy(bse_handle *h);
 

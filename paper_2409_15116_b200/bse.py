@@ -32,6 +32,7 @@ _sig = {
     "bse_build_tau": [_vp],
     "bse_apply_k1x": [_vp, _vp, _vp, _i],
     "bse_apply_k1x_host": [_vp, _vp, _vp, _i],
+    "bse_set_inputs_host": [_vp, _vp, _vp],
     "bse_destroy": [_vp],
     "bse_npw_half": [_vp, C.POINTER(_ll)],
     "bse_gvectors": [_vp, _vp],
@@ -97,6 +98,10 @@ def bse_apply_k1x(h, a, out, B):
 
 def bse_apply_k1x_host(h, a_host, out_host, B):
     _check(lib.bse_apply_k1x_host(h, _ptr(a_host), _ptr(out_host), int(B)), "bse_apply_k1x_host")
+
+
+def bse_set_inputs_host(h, u_host=None, phi_host=None):
+    _check(lib.bse_set_inputs_host(h, _ptr(u_host), _ptr(phi_host)), "bse_set_inputs_host")
 
 
 def bse_destroy(h):

@@ -636,6 +636,9 @@ extern "C" int bse_destroy(bse_handle *h) {
     cudaFree(h->part); cudaFree(h->Sov); cudaFree(h->tau_batch); cudaFree(h->a_dev); cudaFree(h->out_dev);
     cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->a_r); cudaFree(h->acc_r);
     cudaFree(h->batch_pairs); cudaFree(h->eslot);
+    for (cudaEvent_t e : h->ev_pipe) cudaEventDestroy(e);
+    if (h->s_in) cudaStreamDestroy(h->s_in);
+    if (h->s_out) cudaStreamDestroy(h->s_out);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
     delete h;
@@ -685,11 +688,54 @@ extern "C" int bse_apply_k1x_host(bse_handle *h, const double *a_host, double *o
         BSE_CUDA(cudaMalloc(&h->out_dev, bytes));
         h->a_dev_bytes = bytes;
     }
+    if ((h->flags & BSE_TAU_MASK) == BSE_TAU_REAL && B > 1) {
+        // tau(r) is resident, so blocks are independent: copy block b+1 in and block b-1 out (two copy streams, PCIe is full
+        // duplex) while block b is applied; the call ends ~one block after the last input byte arrives
+        if (!h->s_in) {
+            BSE_CUDA(cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
+            BSE_CUDA(cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
+        }
+        while ((int)h->ev_pipe.size() < 2 * B + 1) {
+            cudaEvent_t e;
+            BSE_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            h->ev_pipe.push_back(e);
+        }
+        const size_t per = bytes / B, per_d = per / 8;
+        BSE_CUDA(cudaEventRecord(h->ev_pipe[2 * B], h->stream));             // earlier work on the library's stream first
+        BSE_CUDA(cudaStreamWaitEvent(h->s_in, h->ev_pipe[2 * B], 0));
+        for (int b = 0; b < B; ++b) {
+            BSE_CUDA(cudaMemcpyAsync(h->a_dev + b * per_d, a_host + b * per_d, per, cudaMemcpyHostToDevice, h->s_in));
+            BSE_CUDA(cudaEventRecord(h->ev_pipe[b], h->s_in));
+        }
+        for (int b = 0; b < B; ++b) {
+            BSE_CUDA(cudaStreamWaitEvent(h->stream, h->ev_pipe[b], 0));
+            const int rc = bse_apply_k1x(h, h->a_dev + b * per_d, h->out_dev + b * per_d, 1);
+            if (rc) return rc;
+            BSE_CUDA(cudaEventRecord(h->ev_pipe[B + b], h->stream));
+            BSE_CUDA(cudaStreamWaitEvent(h->s_out, h->ev_pipe[B + b], 0));
+            BSE_CUDA(cudaMemcpyAsync(out_host + b * per_d, h->out_dev + b * per_d, per, cudaMemcpyDeviceToHost, h->s_out));
+        }
+        BSE_CUDA(cudaStreamSynchronize(h->s_out));
+        BSE_CUDA(cudaStreamSynchronize(h->stream));
+        return BSE_OK;
+    }
     BSE_CUDA(cudaMemcpyAsync(h->a_dev, a_host, bytes, cudaMemcpyHostToDevice, h->stream));
     const int rc = bse_apply_k1x(h, h->a_dev, h->out_dev, B);
     if (rc) return rc;
     BSE_CUDA(cudaMemcpyAsync(out_host, h->out_dev, bytes, cudaMemcpyDeviceToHost, h->stream));
     BSE_CUDA(cudaStreamSynchronize(h->stream));
+    return BSE_OK;
+}
+
+// New orbitals / PDEP vectors of the same sizes from HOST memory into the buffers a BSE_PTR_HOST handle owns (no
+// reallocation): the per-step input refresh of a caller whose orbitals change (bench.py's e2e step).  Invalidates tau.
+extern "C" int bse_set_inputs_host(bse_handle *h, const double *u_host, const double *phi_host) {
+    if (!h || (!u_host && !phi_host)) { bse_set_error("null pointer"); return BSE_EINVAL; }
+    if (!h->u_owned || !h->phi_owned) { bse_set_error("bse_set_inputs_host needs a handle created with BSE_PTR_HOST"); return BSE_ESTATE; }
+    if (u_host) BSE_CUDA(cudaMemcpyAsync(h->u_owned, u_host, (size_t)h->Nv * h->N * 8, cudaMemcpyHostToDevice, h->stream));
+    if (phi_host) BSE_CUDA(cudaMemcpyAsync(h->phi_owned, phi_host, (size_t)h->Npdep * h->fft.npw_h * 16, cudaMemcpyHostToDevice, h->stream));
+    h->built = false;
+    if (u_host) { cudaFree(h->uG); cudaFree(h->uGw); h->uG = h->uGw = nullptr; }
     return BSE_OK;
 }
 

@@ -87,6 +87,8 @@ struct bse_handle {
     long long Pacc = 0;                            // capacity of tau_batch in directed entries                         // Bg is already the most that fits
     double *a_dev = nullptr, *out_dev = nullptr;   // staging for the host-pointer entry point
     size_t a_dev_bytes = 0;
+    cudaStream_t s_in = nullptr, s_out = nullptr;  // copy streams of the pipelined host-pointer apply
+    std::vector<cudaEvent_t> ev_pipe;
     // profiling
     bool prof = false;
     double st_ms[BSE_ST_COUNT] = {0};

@@ -267,6 +267,28 @@ def test_host_pointer_entry_points():
         out = np.empty_like(a)
         bse.bse_apply_k1x_host(h, a, out, a.shape[0])
         tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs, want="r")
-        assert rel(out, orc.apply_k1x_real(tab, w.u, pairs, tau_ref, a)) <= TOL
+        assert rel(out, orc.apply_k1x_real(tab, w.u, pairs, tau_ref, a)) <= TOL       # B = 2: the pipelined path
+        # new inputs into the same handle: tau is invalidated, a rebuild gives the new problem's result
+        w2 = wl.make(cfg=wl.Config("h", 9.0, 12, 4, 6, 3.0, 1.3, 0.8, 3.0, 0.0, 2, "random", seed=5))
+        phi2 = np.ascontiguousarray(w2.phi).view(np.float64)
+        bse.bse_set_inputs_host(h, np.ascontiguousarray(w2.u), phi2)
+        with pytest.raises(bse.BseError) as e:
+            bse.bse_apply_k1x_host(h, a, out, a.shape[0])
+        assert e.value.code == bse.BSE_ESTATE
+        bse.bse_build_tau(h)
+        pairs2 = bse.bse_get_pairs(h)
+        a2 = np.ascontiguousarray(w2.a_real())
+        bse.bse_apply_k1x_host(h, a2, out, a2.shape[0])
+        tau2 = orc.build_tau(tab, w2.u, w2.phi, w2.lam, pairs2, want="r")
+        assert rel(out, orc.apply_k1x_real(tab, w2.u, pairs2, tau2, a2)) <= TOL
     finally:
         bse.bse_destroy(h)
+    u_d = torch.from_numpy(w.u).cuda()
+    phi_d = torch.from_numpy(phi).cuda()
+    hb = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u_d, w.phi.shape[0], phi_d, w.lam, w.eta, 0)
+    try:
+        with pytest.raises(bse.BseError) as e:
+            bse.bse_set_inputs_host(hb, w.u, phi)
+        assert e.value.code == bse.BSE_ESTATE                  # borrowed device arrays: nothing to copy into
+    finally:
+        bse.bse_destroy(hb)
