@@ -169,10 +169,10 @@ int st_fwd_plane(bse_handle *h, const FftPlan &pl, const double *fields, const i
     StageTimer t(h, BSE_ST_FWD_PLANE, cnt * m.plane_flops, cnt * (m.N8 + m.z));
     return bse_launch_fwd_plane(pl, fields, pairs, p0, cnt, pl.N, h->Z, h->stream);
 }
-int st_fwd_stick(bse_handle *h, const FftPlan &pl, int cnt, double2 *X, const double *scale) {
+int st_fwd_stick(bse_handle *h, const FftPlan &pl, int cnt, double2 *X, const double *scale, const int *scatter = nullptr) {
     const Model m(pl);
     StageTimer t(h, BSE_ST_FWD_STICK, cnt * m.stick_flops, cnt * (m.z + m.g));
-    return bse_launch_fwd_stick(pl, h->Z, cnt, X, scale, h->stream);
+    return bse_launch_fwd_stick(pl, h->Z, cnt, X, scale, h->stream, scatter);
 }
 int st_inv_stick(bse_handle *h, const FftPlan &pl, const double2 *T, int cnt) {
     const Model m(pl);
@@ -326,41 +326,69 @@ int fill_tau_store(bse_handle *h, bool real) {
     return BSE_OK;
 }
 
-// Row batches of the batched tau modes: consecutive rows are added while the pairs they touch (each counted once: a pair
-// with both ends in the batch serves both rows) fit the tau(r) batch buffer and the rows fit acc_r.
+// Row batches of the batched tau modes.  A batch is a CLUSTER of rows grown greedily over the pair graph: starting from
+// the lowest row not yet placed, the row with the most neighbours already inside the batch is added while the pairs the
+// batch touches (each counted once: a pair with both ends inside serves both rows) fit the tau(r) batch buffer and the
+// rows fit acc_r.  Compact clusters share pairs (fewer tau(r) inversions than rows in list order) and touch few
+// distinct neighbours (fewer re-reads of a).  rowlist holds the rows of all batches, batch after batch.
 int plan_row_batches(bse_handle *h, int rows_cap) {
     const std::vector<int> &ap = h->adj_ptr_h;
     const int Nv = h->Nv;
     h->batches.clear();
-    std::vector<int> pairs_all, eslot((size_t)h->nadj), mark((size_t)std::max<long long>(h->P, 1), -1);
-    std::vector<int> cur;
-    for (int v0 = 0; v0 < Nv;) {
+    std::vector<int> pairs_all, eslot((size_t)h->nadj), mark((size_t)std::max<long long>(h->P, 1), -1), rowlist;
+    std::vector<int> cur, score((size_t)Nv, 0), touched;
+    std::vector<char> placed((size_t)Nv, 0);
+    rowlist.reserve(Nv);
+    int next_seed = 0, tag = 0;
+    while ((int)rowlist.size() < Nv) {
+        while (placed[next_seed]) ++next_seed;
         cur.clear();
-        int v1 = v0;
-        while (v1 < Nv && v1 - v0 < rows_cap) {
+        touched.clear();
+        const int r0 = (int)rowlist.size();
+        int v = next_seed;
+        for (;;) {
             int fresh = 0;
-            for (int e = ap[v1]; e < ap[v1 + 1]; ++e) fresh += mark[h->adj_h[2 * e + 1]] != v0 ? 1 : 0;
-            if (v1 > v0 && (long long)cur.size() + fresh > h->Pacc) break;
-            for (int e = ap[v1]; e < ap[v1 + 1]; ++e) {
-                const int pidx = h->adj_h[2 * e + 1];
-                if (mark[pidx] != v0) { mark[pidx] = v0; cur.push_back(pidx); }
+            for (int e = ap[v]; e < ap[v + 1]; ++e) fresh += mark[h->adj_h[2 * e + 1]] != tag ? 1 : 0;
+            if ((int)rowlist.size() > r0 && (long long)cur.size() + fresh > h->Pacc) break;
+            placed[v] = 1;
+            rowlist.push_back(v);
+            for (int e = ap[v]; e < ap[v + 1]; ++e) {
+                const int pidx = h->adj_h[2 * e + 1], u = h->adj_h[2 * e];
+                if (mark[pidx] != tag) { mark[pidx] = tag; cur.push_back(pidx); }
+                if (!placed[u]) { if (score[u]++ == 0) touched.push_back(u); }
             }
-            ++v1;
+            if ((int)rowlist.size() - r0 >= rows_cap || (int)rowlist.size() >= Nv) break;
+            int best = -1, bs = 0;                              // most neighbours already in the batch; ties: lowest row
+            for (int u : touched)
+                if (!placed[u] && (score[u] > bs || (score[u] == bs && u < best))) { bs = score[u]; best = u; }
+            if (best < 0) {                                     // the component is exhausted: continue with the next unplaced row
+                int s2 = next_seed;
+                while (s2 < Nv && placed[s2]) ++s2;
+                if (s2 >= Nv) break;
+                best = s2;
+            }
+            v = best;
         }
+        for (int u : touched) score[u] = 0;
         std::sort(cur.begin(), cur.end());                     // ascending pair index: sequential reads of the tau(G) store
-        for (int e = ap[v0]; e < ap[v1]; ++e)
-            eslot[e] = (int)(std::lower_bound(cur.begin(), cur.end(), h->adj_h[2 * e + 1]) - cur.begin());
-        h->batches.push_back({v0, v1, (int)pairs_all.size(), (int)cur.size()});
+        for (int i = r0; i < (int)rowlist.size(); ++i) {
+            const int row = rowlist[i];
+            for (int e = ap[row]; e < ap[row + 1]; ++e)
+                eslot[e] = (int)(std::lower_bound(cur.begin(), cur.end(), h->adj_h[2 * e + 1]) - cur.begin());
+        }
+        h->batches.push_back({r0, (int)rowlist.size(), (int)pairs_all.size(), (int)cur.size()});
         pairs_all.insert(pairs_all.end(), cur.begin(), cur.end());
-        v0 = v1;
+        ++tag;
     }
     h->uniq_share = (double)h->P / (double)std::max<size_t>(pairs_all.size(), 1);
-    cudaFree(h->batch_pairs); cudaFree(h->eslot);
-    h->batch_pairs = h->eslot = nullptr;
+    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist);
+    h->batch_pairs = h->eslot = h->rowlist = nullptr;
     BSE_CUDA(cudaMalloc(&h->batch_pairs, std::max<size_t>(pairs_all.size(), 1) * 4));
     BSE_CUDA(cudaMalloc(&h->eslot, std::max<size_t>(eslot.size(), 1) * 4));
+    BSE_CUDA(cudaMalloc(&h->rowlist, (size_t)Nv * 4));
     BSE_CUDA(cudaMemcpyAsync(h->batch_pairs, pairs_all.data(), pairs_all.size() * 4, cudaMemcpyHostToDevice, h->stream));
     BSE_CUDA(cudaMemcpyAsync(h->eslot, eslot.data(), eslot.size() * 4, cudaMemcpyHostToDevice, h->stream));
+    BSE_CUDA(cudaMemcpyAsync(h->rowlist, rowlist.data(), (size_t)Nv * 4, cudaMemcpyHostToDevice, h->stream));
     BSE_CUDA(cudaStreamSynchronize(h->stream));                // the host vectors go out of scope
     return BSE_OK;
 }
@@ -447,7 +475,7 @@ int plan_apply_memory(bse_handle *h, int B) {
 }
 
 // forward transform of `rows` accumulated fields of each of nb blocks into the PW output (a12): acc(G) on H
-int rows_to_pw(bse_handle *h, const double *acc, long long acc_ld, int rows, int nb, double2 *out_pw, int v0) {
+int rows_to_pw(bse_handle *h, const double *acc, long long acc_ld, int rows, int nb, double2 *out_pw, const int *dest) {
     const FftPlan &pl = *h->ap;
     const long long npw_h = pl.npw_h;
     int rc;
@@ -455,7 +483,9 @@ int rows_to_pw(bse_handle *h, const double *acc, long long acc_ld, int rows, int
         for (int r0 = 0; r0 < rows; r0 += (int)h->Pb) {
             const int cnt = (int)std::min<long long>(h->Pb, rows - r0);
             if ((rc = st_fwd_plane(h, pl, acc + (long long)b * acc_ld * pl.N, nullptr, r0, cnt))) return rc;
-            if ((rc = st_fwd_stick(h, pl, cnt, out_pw + ((long long)b * h->Nv + v0 + r0) * npw_h, pl.inv2n))) return rc;
+            // field p of the launch is row dest[r0 + p] (device array; nullptr: row r0 + p) of block b
+            if ((rc = st_fwd_stick(h, pl, cnt, out_pw + (long long)b * h->Nv * npw_h + (dest ? 0 : r0 * npw_h), pl.inv2n,
+                                   dest ? dest + r0 : nullptr))) return rc;
         }
     return BSE_OK;
 }
@@ -471,14 +501,14 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
     if (mode == BSE_TAU_REAL) {
         double *acc = acc_real ? acc_real : h->acc_r;
         if ((rc = st_accumulate(h, h->tau_r, 0, h->P, a, acc, nb, true))) return rc;
-        return out_pw ? rows_to_pw(h, acc, h->Nv, h->Nv, nb, out_pw, 0) : BSE_OK;
+        return out_pw ? rows_to_pw(h, acc, h->Nv, h->Nv, nb, out_pw, nullptr) : BSE_OK;
     }
     const FftPlan &pl = *h->ap;
     const Model m(pl);
     const std::vector<int> &ap = h->adj_ptr_h;
     const double uniq = h->uniq_share;        // share of the inverted fields that is algorithmic work (each pair once)
     for (const bse_handle::RowBatch &bt : h->batches) {
-        const int v0 = bt.v0, rows = bt.v1 - bt.v0, cnt = ap[bt.v1] - ap[bt.v0];
+        const int r0 = bt.v0, rows = bt.v1 - bt.v0;               // rows rowlist[r0 .. r0 + rows)
         for (int c0 = 0; c0 < bt.nu; c0 += (int)h->Pb) {              // tau(G) -> tau(r) of the batch's pairs
             const int c = (int)std::min<long long>(h->Pb, bt.nu - c0);
             { StageTimer t(h, BSE_ST_INV_STICK, uniq * c * m.stick_flops, uniq * c * (m.z + m.g));
@@ -486,12 +516,12 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
             { StageTimer t(h, BSE_ST_INV_PLANE, uniq * c * m.plane_flops, uniq * c * (m.N8 + m.z));
               if ((rc = bse_launch_inv_plane(pl, h->Z, c, pl.N, h->tau_batch + (long long)c0 * pl.N, h->stream))) return rc; }
         }
-        { StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)pl.N * cnt,
-                       m.N8 * (uniq * bt.nu + nb * rows + (v0 == 0 ? (double)nb * h->Nv : 0.0)));
-          if (acc_real) rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, v0, rows, a, acc_real, h->Nv, 0, nb);
-          else rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, v0, rows, a, h->acc_r, h->rows_cap, v0, nb);
+        { StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)pl.N * (double)h->nadj * rows / h->Nv,
+                       m.N8 * (uniq * bt.nu + nb * rows + (r0 == 0 ? (double)nb * h->Nv : 0.0)));
+          if (acc_real) rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, h->rowlist + r0, rows, a, acc_real, h->Nv, false, nb);
+          else rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, h->rowlist + r0, rows, a, h->acc_r, h->rows_cap, true, nb);
           if (rc) return rc; }
-        if (out_pw && (rc = rows_to_pw(h, h->acc_r, h->rows_cap, rows, nb, out_pw, v0))) return rc;
+        if (out_pw && (rc = rows_to_pw(h, h->acc_r, h->rows_cap, rows, nb, out_pw, h->rowlist + r0))) return rc;
     }
     return BSE_OK;
 }
@@ -635,7 +665,7 @@ extern "C" int bse_destroy(bse_handle *h) {
     cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);
     cudaFree(h->part); cudaFree(h->Sov); cudaFree(h->tau_batch); cudaFree(h->a_dev); cudaFree(h->out_dev);
     cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->a_r); cudaFree(h->acc_r);
-    cudaFree(h->batch_pairs); cudaFree(h->eslot);
+    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist);
     for (cudaEvent_t e : h->ev_pipe) cudaEventDestroy(e);
     if (h->s_in) cudaStreamDestroy(h->s_in);
     if (h->s_out) cudaStreamDestroy(h->s_out);

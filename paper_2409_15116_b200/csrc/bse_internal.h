@@ -56,10 +56,11 @@ struct bse_handle {
     int2 *adj = nullptr;             // device [nadj] (w, pair index), sorted by w within a row
     long long P = -1, nadj = 0;
     std::vector<int> adj_h;          // host copy of adj, flattened (w, pair)
-    struct RowBatch { int v0, v1, u0, nu; };   // rows [v0, v1); its unique pairs are batch_pairs[u0, u0 + nu)
+    struct RowBatch { int v0, v1, u0, nu; };   // rows rowlist[v0 .. v1); its unique pairs are batch_pairs[u0, u0 + nu)
     std::vector<RowBatch> batches;
     int *batch_pairs = nullptr;      // device: pair indices of every batch, concatenated
     int *eslot = nullptr;            // device [nadj]: slot of directed entry e inside its batch
+    int *rowlist = nullptr;          // device [Nv]: rows in batch order (clusters of the pair graph)
     double uniq_share = 1.0;         // P / (sum of nu): share of the inverted fields that is algorithmic work
     std::vector<int> adj_ptr_h;      // host copy of adj_ptr (row batches of the batched tau modes)
     bool built = false;
@@ -110,10 +111,11 @@ int bse_cuda_fail(cudaError_t e, const char *what);
 // fft_kernels.cu
 int bse_fft_select(FftPlan &pl);     // sets R1, R2, ops for pl.n; BSE_EUNSUPPORTED if there is no kernel for n
 // fields: [.][N]; pairs == nullptr: plain transform of field p0+p.  scale: [npw_h] table applied in the stick pass.
+// fwd_stick: scatter != nullptr (device array): field p is written to X + scatter[p] * npw_h instead of X + p * npw_h.
 int bse_launch_fwd_plane(const FftPlan &pl, const double *fields, const int2 *pairs, long long p0, int count,
                          long long N, double2 *Z, cudaStream_t s);
 int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2 *X, const double *scale,
-                         cudaStream_t s);
+                         cudaStream_t s, const int *scatter = nullptr);
 // gather != nullptr: field p is read from T + gather[g0 + p] * npw_h (pair indices of a row batch)
 int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2 *Z, cudaStream_t s,
                          const int *gather = nullptr, int g0 = 0);
@@ -131,9 +133,10 @@ int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, 
 
 // k1x_kernels.cu
 int bse_launch_pairlist(bse_handle *h);                 // M -> rowcnt,rowptr,pid,pairs (count only if pairs==nullptr)
-// row-complete accumulation of rows [v0, v0+nrows): tau_b[eslot[e]] for every directed entry e of those rows
-int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_b, const int *eslot, int v0, int nrows, const double *a,
-                               double *acc, long long acc_ld, int v_base, int B);
+// row-complete accumulation of the rows rows[0 .. nrows) (device array): tau_b[eslot[e]] for every directed entry e of
+// those rows; local: acc row index = position in the batch instead of the row id
+int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_b, const int *eslot, const int *rows,
+                               int nrows, const double *a, double *acc, long long acc_ld, bool local, int B);
 // dst[w][k] = Omega * wt * src[w][k], wt = 2 for G != 0 and (1, 0) on (re, im) of G = 0 (entry 0 of H)
 int bse_launch_weight_pw(const double2 *src, double2 *dst, long long npw_h, long long rows, double Omega,
                          cudaStream_t s);

@@ -49,9 +49,9 @@ int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long lo
     return ((const FftOps *)pl.ops)->inv_plane(to_dev(pl), Z, count, N, out, s);
 }
 int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2 *X, const double *scale,
-                         cudaStream_t s) {
+                         cudaStream_t s, const int *scatter) {
     if (count <= 0) return BSE_OK;
-    return ((const FftOps *)pl.ops)->fwd_stick(to_dev(pl), Z, count, X, pl.npw_h, scale, s);
+    return ((const FftOps *)pl.ops)->fwd_stick(to_dev(pl), Z, count, X, pl.npw_h, scale, s, scatter);
 }
 int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2 *Z, cudaStream_t s,
                          const int *gather, int g0) {

@@ -279,7 +279,7 @@ inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *
 template <int R1, int R2>
 __global__ void __launch_bounds__(256)
 fwd_stick_kernel(PlanDev P, const double2 *__restrict__ Z, double2 *__restrict__ X, long long npw_h,
-                 const double *__restrict__ scale) {
+                 const double *__restrict__ scale, const int *__restrict__ scatter, int s_off) {
     using G = Geo<R1, R2>;
     constexpr int n = G::n, LDS = G::LDS, R2p = G::R2p, TS = G::TS;
     extern __shared__ __align__(16) unsigned char smem[];
@@ -303,7 +303,7 @@ fwd_stick_kernel(PlanDev P, const double2 *__restrict__ Z, double2 *__restrict__
     }
     __syncthreads();
     // a4: x(G) = scale(G) * rho(G), gathered to H  (scale = v_c^{1/2}/(2N) for tau, 1/(2N) for the PW wrapper)
-    double2 *xo = X + p * npw_h;
+    double2 *xo = X + (scatter ? (long long)scatter[s_off + p] : p) * npw_h;
     for (int task = threadIdx.x; task < TS * R1; task += blockDim.x) {
         const int blk = task / TS, sl = task - blk * TS;
         const int s = s0 + sl;
@@ -375,7 +375,7 @@ struct FftOps {
     int n, R1, R2, plane_smem;
     int (*fwd_plane)(const PlanDev &, const double *, const int2 *, long long, int, long long, double2 *, cudaStream_t);
     int (*inv_plane)(const PlanDev &, const double2 *, int, long long, double *, cudaStream_t);
-    int (*fwd_stick)(const PlanDev &, const double2 *, int, double2 *, long long, const double *, cudaStream_t);
+    int (*fwd_stick)(const PlanDev &, const double2 *, int, double2 *, long long, const double *, cudaStream_t, const int *);
     int (*inv_stick)(const PlanDev &, const double2 *, int, long long, double2 *, cudaStream_t, const int *, int);
 };
 
@@ -420,13 +420,13 @@ struct Launch {
         return BSE_OK;
     }
     static int fwd_stick(const PlanDev &P, const double2 *Z, int count, double2 *X, long long npw_h, const double *scale,
-                         cudaStream_t s) {
+                         cudaStream_t s, const int *scatter) {
         int rc = set_smem((const void *)fwd_stick_kernel<R1, R2>, G::stick_smem);
         if (rc) return rc;
         for (int c0 = 0; c0 < count; c0 += 65535) {
             const int c = count - c0 < 65535 ? count - c0 : 65535;
             fwd_stick_kernel<R1, R2><<<dim3((P.NS + G::TS - 1) / G::TS, c), 256, G::stick_smem, s>>>(
-                P, Z + (long long)c0 * G::n * P.NS, X + (long long)c0 * npw_h, npw_h, scale);
+                P, Z + (long long)c0 * G::n * P.NS, scatter ? X : X + (long long)c0 * npw_h, npw_h, scale, scatter, c0);
         }
         BSE_CUDA(cudaGetLastError());
         return BSE_OK;

@@ -149,18 +149,19 @@ accumulate_kernel(const double *__restrict__ tau, long long p_first, long long p
     }
 }
 
-// Row-complete form used with the batched tau modes: the batch holds tau(r) of every pair that rows
-// [v0, v0 + gridDim.x) touch, once (a pair with both ends in the batch serves both rows); eslot[e] is the slot of
+// Row-complete form used with the batched tau modes: the batch holds tau(r) of every pair that its rows
+// rows[0 .. gridDim.x) touch, once (a pair with both ends in the batch serves both rows); eslot[e] is the slot of
 // directed entry e in the batch.  Each output row is written once, never re-read:
-//   acc[(b * acc_ld + v - v_base)][r] = sum_{e in row v} tau_b[eslot[e]][r] * a[b][adj[e].x][r]
+//   acc[b * acc_ld + (local ? i : v)][r] = sum_{e in row v} tau_b[eslot[e]][r] * a[b][adj[e].x][r],  v = rows[i]
 // grid = (rows, ceil(N / (2*blockDim))); rows vary fastest across resident CTAs, so they share the r-tile of a in L2.
 template <int BB>
 __global__ void __launch_bounds__(256)
-accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict__ eslot, int v0,
-                       const int *__restrict__ adj_ptr,
+accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict__ eslot,
+                       const int *__restrict__ rows, const int *__restrict__ adj_ptr,
                        const int2 *__restrict__ adj, const double *__restrict__ a, double *__restrict__ acc, int Nv,
-                       long long N, int b0, long long acc_ld, int v_base) {
-    const int v = v0 + blockIdx.x;
+                       long long N, int b0, long long acc_ld, int local) {
+    const int v = rows[blockIdx.x];                  // the batch is a cluster of rows, not a range
+    const int arow = local ? (int)blockIdx.x : v;    // acc_r of the PW layout holds the batch's rows in batch order
     const long long r = 2 * ((long long)blockIdx.y * blockDim.x + threadIdx.x);
     if (r >= N) return;
     const int ea = adj_ptr[v], eb = adj_ptr[v + 1];
@@ -180,7 +181,7 @@ accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict
     }
 #pragma unroll
     for (int b = 0; b < BB; ++b)
-        __stcs(reinterpret_cast<double2 *>(acc + ((long long)(b0 + b) * acc_ld + (v - v_base)) * N + r), s[b]);
+        __stcs(reinterpret_cast<double2 *>(acc + ((long long)(b0 + b) * acc_ld + arow) * N + r), s[b]);
 }
 
 __global__ void weight_pw_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst, long long npw_h,
@@ -251,15 +252,15 @@ int bse_launch_accumulate(bse_handle *h, const double *tau, long long p_first, l
     return BSE_OK;
 }
 
-int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_dir, const int *eslot, int v0, int nrows, const double *a,
-                               double *acc, long long acc_ld, int v_base, int B) {
+int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_dir, const int *eslot, const int *rows,
+                               int nrows, const double *a, double *acc, long long acc_ld, bool local, int B) {
     const int threads = 256;
     const long long tiles = (N / 2 + threads - 1) / threads;
     dim3 grid(nrows, (unsigned)tiles);
     int b0 = 0;
 #define BSE_ROWS(BB)                                                                                              \
-    accumulate_rows_kernel<BB><<<grid, threads, 0, h->stream>>>(tau_dir, eslot, v0, h->adj_ptr, h->adj, a, acc, h->Nv, \
-                                                                N, b0, acc_ld, v_base)
+    accumulate_rows_kernel<BB><<<grid, threads, 0, h->stream>>>(tau_dir, eslot, rows, h->adj_ptr, h->adj, a, acc, h->Nv, \
+                                                                N, b0, acc_ld, local ? 1 : 0)
     while (b0 < B) {
         const int left = B - b0;
         if (left >= 8) { BSE_ROWS(8); b0 += 8; }
