@@ -262,3 +262,40 @@ def p_c_pw(tab: Tables, uS: np.ndarray, accS: np.ndarray) -> np.ndarray:
     uS: [Nv][Npw] orbital coefficients on S; accS: [Npw]."""
     ov = tab.Omega * (np.conj(uS) @ accS)                        # <u_w|acc>, real up to rounding
     return accS - ov.real @ uS
+
+
+# ===================================================================== K1e, eq. 4 (the bare exchange-like Hartree term)
+def hartree_r(tab: Tables, n_r: np.ndarray) -> np.ndarray:
+    """v_H(r) = int v_c(r, r') n(r') dr' = sum_{G in S} v_c(G) n(G) e^{iG.r},  v_c(G) = 4 pi / |G|^2 = vc12^2, v_c(0) := 0
+    (readings S2, S4, S5: the density is truncated to S like every reciprocal-space object)."""
+    return tab.to_r(tab.vc12 * tab.vc12 * tab.to_G(n_r))
+
+
+def apply_k1e_real(tab: Tables, u: np.ndarray, a: np.ndarray) -> np.ndarray:
+    """K1e a = { 2 P_c [ psi_v(r) * int v_c(r, r') sum_v' psi_v'(r') a_v'(r') dr' ] : v }   (eq. 4; real orbitals).
+    a: [B][Nv][N] real; returns [B][Nv][N]."""
+    B, Nv, N = a.shape
+    out = np.empty_like(a)
+    for b in range(B):
+        n_r = np.zeros(N)
+        for v in range(Nv):
+            n_r += u[v] * a[b, v]                    # sum_v' psi*_v' a_v'
+        vH = hartree_r(tab, n_r)
+        for v in range(Nv):
+            out[b, v] = p_c_real(tab, u, 2.0 * u[v] * vH)
+    return out
+
+
+def apply_k1e_pw(tab: Tables, u: np.ndarray, a_pw: np.ndarray) -> np.ndarray:
+    """PW layout of K1e: a_pw [B][Nv][Npw_h] on H; psi_v * v_H is truncated to S before P_c (S15)."""
+    B, Nv, _ = a_pw.shape
+    uS = np.array([tab.to_G(u[w]) for w in range(Nv)])
+    out = np.empty((B, Nv, tab.npw_h), dtype=np.complex128)
+    for b in range(B):
+        n_r = np.zeros(tab.N)
+        for v in range(Nv):
+            n_r += u[v] * tab.to_r(tab.expand_H_to_S(a_pw[b, v]))
+        vH = hartree_r(tab, n_r)
+        for v in range(Nv):
+            out[b, v] = S_to_H(tab, p_c_pw(tab, uS, tab.to_G(2.0 * u[v] * vH)))
+    return out

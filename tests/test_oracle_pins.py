@@ -276,3 +276,72 @@ def test_P11b_overlap_rows_equals_overlap_matrix_rows():
     rows = [0, 5, 7]
     Or = orc.overlap_rows(lambda v: w.u[v], w.Nv, rows)
     assert np.abs(Or - O[rows]).max() < 1e-15
+
+
+# ------------------------------------------------------------------ P13-P16: K1e (eq. 4)
+def test_P13_k1e_dense_coulomb_operator_tiny_grid():
+    """K1e from a dense real-space Coulomb matrix built from brute-force plane waves, by loops (eq. 4 written out)."""
+    cfg = _small_cfg(n=6, L=5.0, ecut=2.5, Nv=3, Npdep=4, B=2, sigma=1.1)
+    w = wl.make(cfg=cfg)
+    n, N, L = w.n, w.N, w.L
+    Omega, dV = L ** 3, L ** 3 / N
+    mx = wl.msq_max(L, w.ecut)
+    rng_m = range(-n // 2, n // 2)
+    S = [(a, b, c) for a in rng_m for b in rng_m for c in rng_m if a * a + b * b + c * c <= mx]
+    r = np.stack(np.meshgrid(*(np.arange(n),) * 3, indexing="ij"), -1).reshape(-1, 3)
+    E = np.array([np.exp(1j * TWO_PI * (r @ np.array(m)) / n) for m in S])
+    vc = np.array([0.0 if m == (0, 0, 0) else 4 * math.pi / ((TWO_PI / L) ** 2 * (m[0] ** 2 + m[1] ** 2 + m[2] ** 2)) for m in S])
+    Vr = ((E.T * vc) @ np.conj(E)).real / Omega                  # v_c(r, r') restricted to S
+    tab = orc.Tables(n, L, w.ecut)
+    a = w.a_real()
+    got = orc.apply_k1e_real(tab, w.u, a)
+    Pc = np.eye(N) - dV * (w.u.T @ w.u)
+    for b in range(a.shape[0]):
+        dens = sum(w.u[x] * a[b, x] for x in range(w.Nv))
+        vH = dV * (Vr @ dens)
+        for v in range(w.Nv):
+            want = Pc @ (2.0 * w.u[v] * vH)
+            assert np.linalg.norm(got[b, v] - want) <= 1e-11 * np.linalg.norm(want)
+
+
+def test_P14_hartree_of_gaussian_density_is_analytic():
+    """v_H(G) = 4 pi n(G) / G^2 for a periodised Gaussian density given analytically in reciprocal space."""
+    n, L, ecut, sig = 20, 12.0, 4.0, 1.4
+    tab = orc.Tables(n, L, ecut)
+    Rc = np.array([5.3, 6.1, 6.8])
+    G = (TWO_PI / L) * tab.S.astype(float)
+    G2 = (G ** 2).sum(1)
+    nG = (2 * math.pi * sig ** 2) ** 1.5 / L ** 3 * np.exp(-0.5 * sig ** 2 * G2) * np.exp(-1j * (G @ Rc))
+    n_r = tab.to_r(nG)                                            # band-limited density on the grid
+    got = tab.to_G(orc.hartree_r(tab, n_r))
+    want = np.zeros(tab.npw, complex)
+    nz = G2 > 0
+    want[nz] = 4 * math.pi * nG[nz] / G2[nz]
+    assert np.linalg.norm(got - want) <= 1e-12 * np.linalg.norm(want)
+
+
+def test_P15_k1e_symmetric_and_projected():
+    w = wl.make(cfg=_small_cfg(n=12, Nv=4, B=2))
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    a = w.a_real()
+    out = orc.apply_k1e_real(tab, w.u, a)
+    ov = tab.dV * np.einsum("wr,bvr->bvw", w.u, out)
+    assert np.abs(ov).max() < 1e-12                               # P_c: <u_w|out> = 0
+    A, Bv = a[0], a[1]
+    KA, KB = out[0], out[1]
+    lhs = tab.dV * np.sum(Bv * KA)
+    rhs = tab.dV * np.sum(A * KB)
+    assert abs(lhs - rhs) <= 1e-12 * max(abs(lhs), abs(rhs), 1e-30)   # K1e symmetric on the projected space
+    # positive semi-definite (Coulomb energy of the transition density): <a|K1e a> = 2 int n v_H >= 0
+    assert tab.dV * np.sum(A * KA) > 0
+
+
+def test_P16_k1e_pw_equals_gathered_real():
+    w = wl.make(cfg=_small_cfg(n=12, Nv=4, B=2))
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    real = orc.apply_k1e_real(tab, w.u, w.a_real())
+    pw = orc.apply_k1e_pw(tab, w.u, w.a_pw)
+    for b in range(real.shape[0]):
+        for v in range(w.Nv):
+            want = orc.S_to_H(tab, tab.to_G(real[b, v]))
+            assert np.linalg.norm(pw[b, v] - want) <= 1e-11 * np.linalg.norm(want)
