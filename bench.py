@@ -96,7 +96,7 @@ class ClockSampler:
 
 BOUND = {"screen_syrk": "tensor", "pair_list": "hbm", "fwd_plane": "hbm", "fwd_stick": "hbm", "pdep_project": "tensor",
          "pdep_backproject": "tensor", "inv_stick": "hbm", "inv_plane": "hbm", "k1x_accumulate": "hbm",
-         "pc_overlap": "tensor", "pc_update": "tensor"}
+         "pc_overlap": "tensor", "pc_update": "tensor", "k1e_density": "hbm", "k1e_product": "hbm"}
 
 
 def w_cols(w):
@@ -326,6 +326,21 @@ def main():
                 "frac": round(pipe_roof_ms / (tb_ms + ta_ms), 4), "gflop": round(tot_f / 1e9, 2),
                 "mbytes": round(tot_b / 1e6, 1), "fp64_dmma_tflops": round(dmma_tf, 2), "fp64_dfma_tflops": round(dfma_tf, 2)}
 
+    # ---- K1e (eq. 4) timed beside the step: not part of `value` ----
+    k1e_ms = None
+    if not large or args.vec == "pw":
+        for _ in range(2):
+            bse.bse_apply_k1e(h, a_d, out_d, B)
+        torch.cuda.synchronize()
+        ke0, ke1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 1 if large else 10
+        ke0.record()
+        for _ in range(reps):
+            bse.bse_apply_k1e(h, a_d, out_d, B)
+        ke1.record()
+        ke1.synchronize()
+        k1e_ms = ke0.elapsed_time(ke1) / reps
+
     # ---- end to end through the C ABI with host (pinned) buffers ----
     e2e = None
     if not args.no_e2e:
@@ -378,7 +393,8 @@ def main():
                                f"Npdep={n_pdep}, Npw_h={npw_h}, eta={w.eta}, P={P} surviving pairs, B={B}",
                    "tau_storage": args.tau, "vec_layout": args.vec, "parallelism": "replicas" if world > 1 else "1gpu",
                    "l2": "512 MB buffer written between timed steps (L2 flush); inputs also exceed L2"},
-        "k1x_applies_per_s": world * B / (ta_ms * 1e-3), "build_ms": tb_ms, "apply_ms": ta_ms, "pairs": P,
+        "k1x_applies_per_s": world * B / (ta_ms * 1e-3),
+        "k1e_applies_per_s": (world * B / (k1e_ms * 1e-3)) if k1e_ms else None, "k1e_ms": k1e_ms, "build_ms": tb_ms, "apply_ms": ta_ms, "pairs": P,
         "gpu_launches": int(launches), "wall_s_timed_region": wall,
         "clocks": clocks,
         "e2e": e2e,

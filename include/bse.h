@@ -77,6 +77,12 @@ int bse_build_tau(bse_handle *h);
  * them; BSE_ENOMEM if one trial block plus one row of pairs does not fit. */
 int bse_apply_k1x(bse_handle *h, const double *a, double *out, int B);
 
+/* K1e term of the Liouville operator (eq. 4), same layouts and conventions as bse_apply_k1x:
+ *   out[b,v] = 2 P_c [ u_v(r) v_H[b](r) ],  v_H[b](G) = v_c(G) n_b(G) on S (v_c(0) := 0),  n_b(r) = sum_v' u_v'(r) a[b,v'](r).
+ * Needs no pair list (may be called before bse_build_tau).  REAL layout: the product u_v v_H is not truncated; PW layout: it
+ * is truncated to S before P_c and formed on the apply grid.  K1e - K1x (the caller's sign) is the two-body kernel of eq. 1. */
+int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B);
+
 /* Same with HOST pointers: copies a to the device, applies, copies out back, synchronises (the end-to-end
  * call bench.py times as `e2e`).  With BSE_TAU_REAL the blocks are pipelined: block b+1 is copied in and block b-1
  * copied out (two copy streams) while block b is applied.  Pinned host memory is needed for the overlap. */
@@ -104,7 +110,8 @@ int bse_get_tau(bse_handle *h, long long first, long long count, double *dst, un
  * host sync per call).  Stage indices: BSE_ST_*; ms and launches are arrays of BSE_ST_COUNT, accumulated since
  * the last bse_profile_reset. */
 enum { BSE_ST_SCREEN = 0, BSE_ST_PAIRLIST, BSE_ST_FWD_PLANE, BSE_ST_FWD_STICK, BSE_ST_PROJECT, BSE_ST_BACKPROJECT,
-       BSE_ST_INV_STICK, BSE_ST_INV_PLANE, BSE_ST_ACCUM, BSE_ST_PC_OVERLAP, BSE_ST_PC_UPDATE, BSE_ST_COUNT };
+       BSE_ST_INV_STICK, BSE_ST_INV_PLANE, BSE_ST_ACCUM, BSE_ST_PC_OVERLAP, BSE_ST_PC_UPDATE, BSE_ST_K1E_DENSITY,
+       BSE_ST_K1E_PRODUCT, BSE_ST_COUNT };
 int bse_profile_enable(bse_handle *h, int enable);
 int bse_profile_reset(bse_handle *h);
 int bse_profile_get(const bse_handle *h, double *ms /* [BSE_ST_COUNT] */, long long *launches /* [BSE_ST_COUNT] */);

@@ -22,9 +22,9 @@ BSE_OK, BSE_EINVAL, BSE_ENOMEM, BSE_ECUDA, BSE_ESTATE, BSE_EUNSUPPORTED = 0, -1,
 BSE_TAU_REAL, BSE_TAU_PW, BSE_TAU_STREAM = 0x0, 0x1, 0x2
 BSE_VEC_REAL, BSE_VEC_PW, BSE_PTR_HOST = 0x0, 0x4, 0x8
 STAGES = ["screen_syrk", "pair_list", "fwd_plane", "fwd_stick", "pdep_project", "pdep_backproject",
-          "inv_stick", "inv_plane", "k1x_accumulate", "pc_overlap", "pc_update"]
+          "inv_stick", "inv_plane", "k1x_accumulate", "pc_overlap", "pc_update", "k1e_density", "k1e_product"]
 # kernels launched per stage invocation (bse_api.cu): split-K GEMMs launch GEMM + reduce, pair list 1 kernel
-KERNELS_PER_STAGE = [2, 1, 1, 1, 2, 1, 1, 1, 1, 2, 1]
+KERNELS_PER_STAGE = [2, 1, 1, 1, 2, 1, 1, 1, 1, 2, 1, 1, 1]
 
 _vp, _i, _d, _u, _ll = C.c_void_p, C.c_int, C.c_double, C.c_uint, C.c_longlong
 _sig = {
@@ -32,6 +32,7 @@ _sig = {
     "bse_build_tau": [_vp],
     "bse_apply_k1x": [_vp, _vp, _vp, _i],
     "bse_apply_k1x_host": [_vp, _vp, _vp, _i],
+    "bse_apply_k1e": [_vp, _vp, _vp, _i],
     "bse_set_inputs_host": [_vp, _vp, _vp],
     "bse_destroy": [_vp],
     "bse_npw_half": [_vp, C.POINTER(_ll)],
@@ -94,6 +95,10 @@ def bse_build_tau(h):
 
 def bse_apply_k1x(h, a, out, B):
     _check(lib.bse_apply_k1x(h, _ptr(a), _ptr(out), int(B)), "bse_apply_k1x")
+
+
+def bse_apply_k1e(h, a, out, B):
+    _check(lib.bse_apply_k1e(h, _ptr(a), _ptr(out), int(B)), "bse_apply_k1e")
 
 
 def bse_apply_k1x_host(h, a_host, out_host, B):

@@ -22,7 +22,7 @@ extern "C" const char *bse_version(void) { return "bse_b200 0.1 (sm_100a, fp64)"
 
 static const char *k_stage_names[BSE_ST_COUNT] = {
     "screen_syrk", "pair_list", "fwd_plane", "fwd_stick", "pdep_project", "pdep_backproject",
-    "inv_stick", "inv_plane", "k1x_accumulate", "pc_overlap", "pc_update"};
+    "inv_stick", "inv_plane", "k1x_accumulate", "pc_overlap", "pc_update", "k1e_density", "k1e_product"};
 extern "C" const char *bse_stage_name(int s) { return (s >= 0 && s < BSE_ST_COUNT) ? k_stage_names[s] : "?"; }
 
 namespace {
@@ -83,7 +83,7 @@ int build_fft_plan(bse_handle *h, FftPlan &pl, int n) {
     std::vector<int> hidx((size_t)D * D * D, -1);
     auto hid = [&](int m1, int m2, int m3) -> int & { return hidx[((size_t)(m1 + R) * D + (m2 + R)) * D + (m3 + R)]; };
     h->mill.resize(H.size() * 3);
-    std::vector<double> vc12(H.size()), vc12n(H.size()), inv2n(H.size());
+    std::vector<double> vc12(H.size()), vc12n(H.size()), inv2n(H.size()), vcn(H.size());
     const double twopi_L = 2.0 * M_PI / h->L;
     for (size_t i = 0; i < H.size(); ++i) {
         hid(H[i].m1, H[i].m2, H[i].m3) = (int)i;
@@ -92,6 +92,7 @@ int build_fft_plan(bse_handle *h, FftPlan &pl, int n) {
         vc12[i] = q == 0 ? 0.0 : std::sqrt(4.0 * M_PI) / (twopi_L * std::sqrt((double)q));
         vc12n[i] = vc12[i] / (2.0 * (double)pl.N);
         inv2n[i] = 1.0 / (2.0 * (double)pl.N);
+        vcn[i] = vc12[i] * vc12[i] / (2.0 * (double)pl.N);
     }
     // half sticks ordered by (t2 = m2 mod n, m3): stick index = soff[t2] + m3 for wmin[t2] <= m3 <= wmax[t2]
     std::vector<int> soff(n, 0), wmax(n, -1), wmin(n, 0);
@@ -136,12 +137,13 @@ int build_fft_plan(bse_handle *h, FftPlan &pl, int n) {
     if ((rc = upload(pl.vc12, vc12))) return rc;
     if ((rc = upload(pl.vc12n, vc12n))) return rc;
     if ((rc = upload(pl.inv2n, inv2n))) return rc;
+    if ((rc = upload(pl.vcn, vcn))) return rc;
     return BSE_OK;
 }
 
 void free_plan(FftPlan &pl) {
     cudaFree(pl.tw); cudaFree(pl.soff); cudaFree(pl.wmax); cudaFree(pl.wmin); cudaFree(pl.hmapT);
-    cudaFree(pl.vc12); cudaFree(pl.vc12n); cudaFree(pl.inv2n);
+    cudaFree(pl.vc12); cudaFree(pl.vc12n); cudaFree(pl.inv2n); cudaFree(pl.vcn);
 }
 
 inline long long ldD(const bse_handle *h) { return (h->Npdep + 1) & ~1; }
@@ -665,7 +667,7 @@ extern "C" int bse_destroy(bse_handle *h) {
     cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);
     cudaFree(h->part); cudaFree(h->Sov); cudaFree(h->tau_batch); cudaFree(h->a_dev); cudaFree(h->out_dev);
     cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->a_r); cudaFree(h->acc_r);
-    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist);
+    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist); cudaFree(h->k1e_ws); cudaFree(h->u_a);
     for (cudaEvent_t e : h->ev_pipe) cudaEventDestroy(e);
     if (h->s_in) cudaStreamDestroy(h->s_in);
     if (h->s_out) cudaStreamDestroy(h->s_out);
@@ -765,8 +767,114 @@ extern "C" int bse_set_inputs_host(bse_handle *h, const double *u_host, const do
     if (u_host) BSE_CUDA(cudaMemcpyAsync(h->u_owned, u_host, (size_t)h->Nv * h->N * 8, cudaMemcpyHostToDevice, h->stream));
     if (phi_host) BSE_CUDA(cudaMemcpyAsync(h->phi_owned, phi_host, (size_t)h->Npdep * h->fft.npw_h * 16, cudaMemcpyHostToDevice, h->stream));
     h->built = false;
-    if (u_host) { cudaFree(h->uG); cudaFree(h->uGw); h->uG = h->uGw = nullptr; }
+    if (u_host) { cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->u_a); h->uG = h->uGw = nullptr; h->u_a = nullptr; }
     return BSE_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ K1e (eq. 4)
+namespace {
+
+int ensure_k1e_ws(bse_handle *h, size_t bytes) {
+    if (h->k1e_bytes >= bytes) return BSE_OK;
+    cudaFree(h->k1e_ws);
+    h->k1e_ws = nullptr; h->k1e_bytes = 0;
+    BSE_CUDA(cudaMalloc(&h->k1e_ws, bytes));
+    h->k1e_bytes = bytes;
+    return BSE_OK;
+}
+
+// n -> v_H in place for cnt fields held at buf ([cnt][pl.N]): forward transform with the v_c / N scaling (a3 + a4 with
+// v_c instead of v_c^{1/2}), inverse transform (a9)
+int hartree_in_place(bse_handle *h, const FftPlan &pl, double *buf, int nfields) {
+    int rc;
+    for (int c0 = 0; c0 < nfields; c0 += (int)h->Pb) {
+        const int cnt = (int)std::min<long long>(h->Pb, nfields - c0);
+        if ((rc = st_fwd_plane(h, pl, buf, nullptr, c0, cnt))) return rc;
+        if ((rc = st_fwd_stick(h, pl, cnt, h->X, pl.vcn))) return rc;
+        if ((rc = st_inv_stick(h, pl, h->X, cnt))) return rc;
+        if ((rc = st_inv_plane(h, pl, cnt, buf + (long long)c0 * pl.N))) return rc;
+    }
+    return BSE_OK;
+}
+
+// orbitals on the apply grid of the PW layout: u_a = inverse transform of u(G) on n_a (u is band-limited to S)
+int ensure_u_apply(bse_handle *h) {
+    if (h->ap == &h->fft || h->u_a) return BSE_OK;
+    const FftPlan &pl = *h->ap;
+    int rc;
+    if ((rc = ensure_u_pw(h))) return rc;
+    if (cudaMalloc(&h->u_a, (size_t)h->Nv * pl.N * 8) != cudaSuccess) {
+        // the K1x apply plan holds the free memory: drop it (the next K1x apply plans again, with u_a in place)
+        (void)cudaGetLastError();
+        h->u_a = nullptr;
+        BSE_CUDA(cudaStreamSynchronize(h->stream));
+        cudaFree(h->tau_batch); cudaFree(h->a_r); cudaFree(h->acc_r);
+        h->tau_batch = h->a_r = h->acc_r = nullptr;
+        h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
+        BSE_CUDA(cudaMalloc(&h->u_a, (size_t)h->Nv * pl.N * 8));
+    }
+    for (long long v0 = 0; v0 < h->Nv; v0 += h->Pb) {
+        const int cnt = (int)std::min<long long>(h->Pb, h->Nv - v0);
+        if ((rc = st_inv_stick(h, pl, h->uG + v0 * pl.npw_h, cnt))) return rc;
+        if ((rc = st_inv_plane(h, pl, cnt, h->u_a + v0 * pl.N))) return rc;
+    }
+    return BSE_OK;
+}
+
+}  // namespace
+
+extern "C" int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B) {
+    if (!h || !a || !out || B <= 0) { bse_set_error("null pointer or B <= 0"); return BSE_EINVAL; }
+    if (a == out) { bse_set_error("out must not alias a"); return BSE_EINVAL; }
+    int rc;
+    const long long Nv = h->Nv;
+    if (!(h->flags & BSE_VEC_PW)) {
+        const FftPlan &pl = h->fft;
+        const double N8 = 8.0 * (double)pl.N;
+        if ((rc = ensure_k1e_ws(h, (size_t)B * pl.N * 8))) return rc;
+        { StageTimer t(h, BSE_ST_K1E_DENSITY, 2.0 * B * Nv * (double)pl.N, N8 * (B * Nv + Nv + B));
+          if ((rc = bse_launch_k1e_density(h->u, a, h->k1e_ws, h->Nv, pl.N, B, h->stream))) return rc; }
+        if ((rc = hartree_in_place(h, pl, h->k1e_ws, B))) return rc;
+        { StageTimer t(h, BSE_ST_K1E_PRODUCT, 2.0 * B * Nv * (double)pl.N, N8 * (B * Nv + Nv + B));
+          if ((rc = bse_launch_k1e_product(h->u, h->k1e_ws, out, 0, h->Nv, Nv, pl.N, B, h->stream))) return rc; }
+        return p_c_rows(h, out, (long long)B * Nv, pl.N, h->u, h->u, h->dV);
+    }
+    // PW layout: one block at a time on the apply grid: a(G) -> a(r), density, Hartree, products in row chunks -> out(G)
+    const FftPlan &pl = *h->ap;
+    const double N8 = 8.0 * (double)pl.N;
+    const long long npw_h = pl.npw_h;
+    if ((rc = ensure_u_pw(h))) return rc;
+    if ((rc = ensure_u_apply(h))) return rc;
+    const double *ua = h->u_a ? h->u_a : h->u;
+    // staging: the K1x plan's buffers when they exist (they took the free memory), else own workspace
+    double *a_r = h->a_r, *dens = (h->tau_batch && h->Pacc >= h->Pb + 1) ? h->tau_batch : nullptr;
+    if (!a_r || !dens) {
+        if ((rc = ensure_k1e_ws(h, (size_t)((a_r ? 0 : Nv) + (dens ? 0 : 1 + h->Pb)) * pl.N * 8))) return rc;
+        double *ws = h->k1e_ws;
+        if (!a_r) { a_r = ws; ws += Nv * pl.N; }
+        if (!dens) dens = ws;
+    }
+    double *prod = dens + pl.N;
+    const double2 *ag = (const double2 *)a;
+    double2 *og = (double2 *)out;
+    for (int b = 0; b < B; ++b) {
+        for (long long v0 = 0; v0 < Nv; v0 += h->Pb) {
+            const int cnt = (int)std::min<long long>(h->Pb, Nv - v0);
+            if ((rc = st_inv_stick(h, pl, ag + ((long long)b * Nv + v0) * npw_h, cnt))) return rc;
+            if ((rc = st_inv_plane(h, pl, cnt, a_r + v0 * pl.N))) return rc;
+        }
+        { StageTimer t(h, BSE_ST_K1E_DENSITY, 2.0 * Nv * (double)pl.N, N8 * (2.0 * Nv + 1));
+          if ((rc = bse_launch_k1e_density(ua, a_r, dens, h->Nv, pl.N, 1, h->stream))) return rc; }
+        if ((rc = hartree_in_place(h, pl, dens, 1))) return rc;
+        for (long long v0 = 0; v0 < Nv; v0 += h->Pb) {
+            const int cnt = (int)std::min<long long>(h->Pb, Nv - v0);
+            { StageTimer t(h, BSE_ST_K1E_PRODUCT, 2.0 * cnt * (double)pl.N, N8 * (2.0 * cnt + 1));
+              if ((rc = bse_launch_k1e_product(ua, dens, prod, (int)v0, cnt, h->Pb, pl.N, 1, h->stream))) return rc; }
+            if ((rc = st_fwd_plane(h, pl, prod, nullptr, 0, cnt))) return rc;
+            if ((rc = st_fwd_stick(h, pl, cnt, og + ((long long)b * Nv + v0) * npw_h, pl.inv2n))) return rc;
+        }
+    }
+    return p_c_rows(h, (double *)out, (long long)B * Nv, 2 * npw_h, (const double *)h->uGw, (const double *)h->uG, 1.0);
 }
 
 // ------------------------------------------------------------------------------------------------ accessors

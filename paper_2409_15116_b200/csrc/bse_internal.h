@@ -28,6 +28,7 @@ struct FftPlan {
     double *vc12 = nullptr;       // [npw_h] sqrt(4 pi)/|G|, 0 at G = 0
     double *vc12n = nullptr;      // [npw_h] vc12 / (2N)  (forward normalisation and the untangling 1/2 folded in)
     double *inv2n = nullptr;      // [npw_h] 1 / (2N)     (forward transform without the Coulomb factor, PW wrapper)
+    double *vcn = nullptr;        // [npw_h] v_c / (2N) = vc12^2 / (2N)  (Hartree potential of K1e)
 };
 
 // ---------------------------------------------------------------------------------------------------------
@@ -86,6 +87,10 @@ struct bse_handle {
     bool Bg_final = false, plan_ok = false;
     long long plan_nadj = -1;
     long long Pacc = 0;                            // capacity of tau_batch in directed entries                         // Bg is already the most that fits
+    // K1e workspaces (grow-only): dens / vH [B][N] (REAL) or one block's a(r) [Nv][Na] + [1][Na] + product rows [Pb][Na] (PW)
+    double *k1e_ws = nullptr;
+    size_t k1e_bytes = 0;
+    double *u_a = nullptr;                         // [Nv][Na] orbitals on the apply grid (PW layout with a coarser grid)
     double *a_dev = nullptr, *out_dev = nullptr;   // staging for the host-pointer entry point
     size_t a_dev_bytes = 0;
     cudaStream_t s_in = nullptr, s_out = nullptr;  // copy streams of the pipelined host-pointer apply
@@ -137,6 +142,10 @@ int bse_launch_pairlist(bse_handle *h);                 // M -> rowcnt,rowptr,pi
 // those rows; local: acc row index = position in the batch instead of the row id
 int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_b, const int *eslot, const int *rows,
                                int nrows, const double *a, double *acc, long long acc_ld, bool local, int B);
+// K1e (eq. 4): dens[b][r] = sum_v u[v][r] a[b][v][r];  out[b * out_ld + i][r] = 2 u[v0 + i][r] vH[b][r], i < nrows
+int bse_launch_k1e_density(const double *u, const double *a, double *dens, int Nv, long long N, int B, cudaStream_t s);
+int bse_launch_k1e_product(const double *u, const double *vH, double *out, int v0, int nrows, long long out_ld,
+                           long long N, int B, cudaStream_t s);
 // dst[w][k] = Omega * wt * src[w][k], wt = 2 for G != 0 and (1, 0) on (re, im) of G = 0 (entry 0 of H)
 int bse_launch_weight_pw(const double2 *src, double2 *dst, long long npw_h, long long rows, double Omega,
                          cudaStream_t s);

@@ -184,6 +184,49 @@ accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict
         __stcs(reinterpret_cast<double2 *>(acc + ((long long)(b0 + b) * acc_ld + arow) * N + r), s[b]);
 }
 
+// K1e (eq. 4): transition density n[b][r] = sum_v u[v][r] a[b][v][r] and the product 2 u[v][r] vH[b][r].
+// grid = (ceil(N / (2*blockDim)), ceil(B / BB)); u[v] tiles are shared by the BB blocks of a CTA.
+template <int BB>
+__global__ void __launch_bounds__(256)
+k1e_density_kernel(const double *__restrict__ u, const double *__restrict__ a, double *__restrict__ dens, int Nv,
+                   long long N, int B) {
+    const long long r = 2 * ((long long)blockIdx.x * blockDim.x + threadIdx.x);
+    if (r >= N) return;
+    const int b0 = blockIdx.y * BB;
+    double2 s[BB];
+#pragma unroll
+    for (int b = 0; b < BB; ++b) s[b] = make_double2(0.0, 0.0);
+    for (int v = 0; v < Nv; ++v) {
+        const double2 x = *reinterpret_cast<const double2 *>(u + (long long)v * N + r);
+#pragma unroll
+        for (int b = 0; b < BB; ++b) {
+            if (b0 + b < B) {
+                const double2 y = __ldcs(reinterpret_cast<const double2 *>(a + ((long long)(b0 + b) * Nv + v) * N + r));
+                s[b].x = fma(x.x, y.x, s[b].x);
+                s[b].y = fma(x.y, y.y, s[b].y);
+            }
+        }
+    }
+#pragma unroll
+    for (int b = 0; b < BB; ++b)
+        if (b0 + b < B) *reinterpret_cast<double2 *>(dens + (long long)(b0 + b) * N + r) = s[b];
+}
+
+// out[(b * out_ld + v - v0)][r] = 2 u[v][r] vH[b][r] for v in [v0, v0 + gridDim.y), b < B
+__global__ void __launch_bounds__(256)
+k1e_product_kernel(const double *__restrict__ u, const double *__restrict__ vH, double *__restrict__ out, int v0,
+                   long long out_ld, long long N, int B) {
+    const long long r = 2 * ((long long)blockIdx.x * blockDim.x + threadIdx.x);
+    if (r >= N) return;
+    const int v = v0 + blockIdx.y;
+    const double2 x = *reinterpret_cast<const double2 *>(u + (long long)v * N + r);
+    for (int b = 0; b < B; ++b) {
+        const double2 y = *reinterpret_cast<const double2 *>(vH + (long long)b * N + r);
+        __stcs(reinterpret_cast<double2 *>(out + ((long long)b * out_ld + blockIdx.y) * N + r),
+               make_double2(2.0 * x.x * y.x, 2.0 * x.y * y.y));
+    }
+}
+
 __global__ void weight_pw_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst, long long npw_h,
                                  long long total, double Omega) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -269,6 +312,23 @@ int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_dir
         else { BSE_ROWS(1); b0 += 1; }
     }
 #undef BSE_ROWS
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+int bse_launch_k1e_density(const double *u, const double *a, double *dens, int Nv, long long N, int B, cudaStream_t s) {
+    const int threads = 256;
+    const unsigned tiles = (unsigned)((N / 2 + threads - 1) / threads);
+    k1e_density_kernel<4><<<dim3(tiles, (B + 3) / 4), threads, 0, s>>>(u, a, dens, Nv, N, B);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+int bse_launch_k1e_product(const double *u, const double *vH, double *out, int v0, int nrows, long long out_ld,
+                           long long N, int B, cudaStream_t s) {
+    const int threads = 256;
+    const unsigned tiles = (unsigned)((N / 2 + threads - 1) / threads);
+    k1e_product_kernel<<<dim3(tiles, nrows), threads, 0, s>>>(u, vH, out, v0, out_ld, N, B);
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }

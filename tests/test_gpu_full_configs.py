@@ -5,7 +5,8 @@ pair integral takes ~10 s), so each test checks, against oracle values computed 
   * the surviving-pair list restricted to sampled rows v (every w, both orders) - bit-exact, with the S10 guard band asserted
     on those rows - and the GPU's O rows to 1e-12;
   * tau_vw(r) for every pair of one complete row v* (the row with the fewest neighbours, >= 3) - 1e-10 relative L2 each;
-  * the K1x output row out[b, v*] for sampled blocks b in the layout the config uses (PW on H for cfg 4-5) - 1e-10.
+  * the K1x output row out[b, v*] for sampled blocks b in the layout the config uses (PW on H for cfg 4-5) - 1e-10;
+  * (cfg 3, 4) one K1e output row (eq. 4) in the PW layout - 1e-10.
 Inputs come from workloads.make_device (seeded, built on the GPU with torch: input preparation only).
 Launch configuration = the one bench.py uses for that config (tau storage / vector layout per SURVEY.md 8(d) item 7).
 """
@@ -33,7 +34,34 @@ def _need_memory(gb):
         pytest.skip(f"needs {gb} GB of free device memory, {free / 1e9:.0f} GB available")
 
 
-def _sampled_full_check(cfg_id, tau_flag, vec_pw, screen_rows, blocks, need_gb):
+def _k1e_row_check(bse, h, w, u_pw_host, row):
+    """K1e (eq. 4) at full size in the PW layout, block 0, one output row against the oracle.  The oracle's PW form needs
+    a_v(r) of every orbital by its own FFT (hours at this size), so it is evaluated through its REAL form on
+    a(r) = inverse transform of the input coefficients (input preparation, torch) and gathered to H, which pin P16 shows is
+    the same thing."""
+    Nv, N = w.Nv, w.N
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    a0 = torch.view_as_real(w.a_pw[0:1]).contiguous()
+    out0 = torch.empty_like(a0)
+    bse.bse_apply_k1e(h, a0, out0, 1)
+    torch.cuda.synchronize()
+    got = torch.view_as_complex(out0[0, row]).cpu().numpy()
+    tabs = _scatter_tables(w)
+    n_r = np.zeros(N)
+    for v0 in range(0, Nv, 16):
+        ar = _to_real(w, w.a_pw[0, v0:v0 + 16], tabs)
+        n_r += np.einsum("vr,vr->r", w.u[v0:v0 + 16].cpu().numpy(), ar.cpu().numpy())      # sum_v u_v a_v, in numpy
+    vH = orc.hartree_r(tab, n_r)
+    uS = tab.expand_H_to_S(u_pw_host)
+    ref = orc.S_to_H(tab, orc.p_c_pw(tab, uS, tab.to_G(2.0 * w.u[row].cpu().numpy() * vH)))
+    wt = np.full(tab.npw_h, 2.0)
+    wt[0] = 1.0
+    e = float(np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum()))
+    assert e <= TOL, e
+    return e
+
+
+def _sampled_full_check(cfg_id, tau_flag, vec_pw, screen_rows, blocks, need_gb, k1e_row=None):
     from paper_2409_15116_b200 import bse
     _need_memory(need_gb)
     t0 = time.time()
@@ -72,6 +100,11 @@ def _sampled_full_check(cfg_id, tau_flag, vec_pw, screen_rows, blocks, need_gb):
             ref = sorted(x for x in range(Nv) if x == v or Or[i, x] >= w.eta)
             assert sorted(nbr[v]) == ref, f"pair list differs from the oracle on row {v}"
             assert np.abs(O_gpu[v] - Or[i]).max() < 1e-12
+
+        if k1e_row is not None:
+            e1 = _k1e_row_check(bse, h, w, u_pw_host, k1e_row)
+            print(f"cfg{cfg_id}: K1e row {k1e_row}, block 0: error {e1:.2e}")
+            torch.cuda.empty_cache()
 
         # ---- apply on the GPU
         if vec_pw:
@@ -158,12 +191,12 @@ def test_cfg3_full_size_real_layout():
 
 def test_cfg3_full_size_pw_layout():
     from paper_2409_15116_b200 import bse
-    _sampled_full_check(3, bse.BSE_TAU_PW, True, screen_rows=[17], blocks=[5], need_gb=40)
+    _sampled_full_check(3, bse.BSE_TAU_PW, True, screen_rows=[17], blocks=[5], need_gb=40, k1e_row=200)
 
 
 def test_cfg4_full_size():
     from paper_2409_15116_b200 import bse
-    _sampled_full_check(4, bse.BSE_TAU_PW, True, screen_rows=[777], blocks=[7], need_gb=120)
+    _sampled_full_check(4, bse.BSE_TAU_PW, True, screen_rows=[777], blocks=[7], need_gb=120, k1e_row=513)
 
 
 def test_cfg5_full_size_streamed():

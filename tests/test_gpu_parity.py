@@ -292,3 +292,50 @@ def test_host_pointer_entry_points():
         assert e.value.code == bse.BSE_ESTATE                  # borrowed device arrays: nothing to copy into
     finally:
         bse.bse_destroy(hb)
+
+
+@pytest.mark.parametrize("cfg", [
+    None,                                                                        # BASELINE config 1
+    wl.Config("k1e", 9.0, 12, 5, 7, 3.0, 1.3, 0.8, 3.0, 0.05, 3, "random", seed=112),     # odd Nv, B; apply grid = grid
+    wl.Config("k1e", 12.0, 20, 6, 9, 4.0, 1.3, 0.8, 3.0, 0.0, 1, "random", seed=120),     # radix 5
+])
+def test_k1e_real_and_pw_layouts(cfg):
+    """K1e (eq. 4; SURVEY 8(f) #1) against the oracle in both layouts; needs no pair list."""
+    bse = _bse()
+    w = wl.make(1) if cfg is None else wl.make(cfg=cfg)
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    B = w.a_pw.shape[0]
+    g = Gpu(w, bse.BSE_TAU_PW)
+    try:
+        a = w.a_real()
+        ref = orc.apply_k1e_real(tab, w.u, a)
+        a_d = torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+        out = torch.empty_like(a_d)
+        bse.bse_apply_k1e(g.h, a_d, out, B)                     # before bse_build_tau: allowed
+        torch.cuda.synchronize()
+        assert rel(out.cpu().numpy(), ref) <= TOL
+    finally:
+        g.close()
+    g = Gpu(w, bse.BSE_TAU_PW | bse.BSE_VEC_PW)
+    try:
+        ref = orc.apply_k1e_pw(tab, w.u, w.a_pw)
+        a_d = torch.from_numpy(np.ascontiguousarray(w.a_pw).view(np.float64)).to("cuda:0")
+        out = torch.empty_like(a_d)
+        bse.bse_apply_k1e(g.h, a_d, out, B)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy().view(np.complex128).reshape(ref.shape)
+        wt = np.full(tab.npw_h, 2.0)
+        wt[0] = 1.0
+        err = np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum())
+        assert err <= TOL, err
+        # K1x on the same handle afterwards still matches (shared workspaces)
+        g.build()
+        pairs_ref, _ = orc.screen_pairs(w.u, w.eta)
+        tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs_ref, want="r")
+        refx = orc.apply_k1x_pw(tab, w.u, pairs_ref, tau_ref, w.a_pw)
+        bse.bse_apply_k1x(g.h, a_d, out, B)
+        torch.cuda.synchronize()
+        gotx = out.cpu().numpy().view(np.complex128).reshape(refx.shape)
+        assert np.sqrt((wt * np.abs(gotx - refx) ** 2).sum() / (wt * np.abs(refx) ** 2).sum()) <= TOL
+    finally:
+        g.close()
