@@ -162,7 +162,10 @@ def run_reference(args, rank):
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "pairs/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * info["P"] / v, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{args.config - 1}] (cfg{args.config})"},
+            "config": {"workload": f"BASELINE.json configs[{args.config - 1}] (cfg{args.config}): grid {w.n}^3, Nv={w.Nv}, "
+                                   f"Npdep={w.phi.shape[0]}, Npw_h={w.mill.shape[0]}, eta={w.eta}, P={info['P']} surviving pairs, "
+                                   f"B={w.a_pw.shape[0]}",
+                       "tau_storage": "oracle", "vec_layout": "real", "parallelism": "host cores"},
             "cpu_baseline": {"value": v, "unit": "pairs/s", "cores": info["cores"], "kind": "oracle", "sample": sample},
             "e2e": {"value": v, "unit": "pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
