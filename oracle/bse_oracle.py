@@ -299,3 +299,16 @@ def apply_k1e_pw(tab: Tables, u: np.ndarray, a_pw: np.ndarray) -> np.ndarray:
         for v in range(Nv):
             out[b, v] = S_to_H(tab, p_c_pw(tab, uS, tab.to_G(2.0 * u[v] * vH)))
     return out
+
+
+# ===================================================== KS <-> localised representation, eq. 12
+def rotate(U: np.ndarray, x: np.ndarray, transpose: bool = False) -> np.ndarray:
+    """y[b, v, :] = sum_v' U[v, v'] x[b, v', :]  (eq. 12 applied to the orbitals of A_s), or with U^T (the way back;
+    U is real orthogonal at the Gamma point).  x: [B][Nv][K], any K (real-space points or PW coefficients)."""
+    M = U.T if transpose else U
+    out = np.zeros_like(x)
+    for b in range(x.shape[0]):
+        for v in range(M.shape[0]):
+            for w in range(M.shape[1]):
+                out[b, v] += M[v, w] * x[b, w]
+    return out

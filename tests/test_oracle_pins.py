@@ -345,3 +345,26 @@ def test_P16_k1e_pw_equals_gathered_real():
         for v in range(w.Nv):
             want = orc.S_to_H(tab, tab.to_G(real[b, v]))
             assert np.linalg.norm(pw[b, v] - want) <= 1e-11 * np.linalg.norm(want)
+
+
+# ------------------------------------------------------------------ P17: rotation of the representation (eq. 12)
+def test_P17_rotation_covariance_of_k1x_and_k1e():
+    """With every pair kept (eta = 0), K1x and K1e are covariant under an orthogonal mixing of the occupied orbitals:
+    K(U u, U a) = U K(u, a).  Pins `rotate` (index order, transpose) through the whole chain, not against itself."""
+    w = wl.make(cfg=_small_cfg(n=12, Nv=4, Npdep=6, B=2, eta=0.0))
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    rng = np.random.default_rng(5)
+    U, _ = np.linalg.qr(rng.normal(size=(w.Nv, w.Nv)))
+    a = w.a_real()
+    u2 = U @ w.u
+    a2 = orc.rotate(U, a)
+    assert np.allclose(orc.rotate(U, a2, transpose=True), a, atol=1e-14)
+    assert np.allclose(a2, np.einsum("vw,bwr->bvr", U, a), atol=1e-14)
+    pairs, _ = orc.screen_pairs(w.u, 0.0)
+    pairs2, _ = orc.screen_pairs(u2, 0.0)
+    k = orc.apply_k1x_real(tab, w.u, pairs, orc.build_tau(tab, w.u, w.phi, w.lam, pairs), a)
+    k2 = orc.apply_k1x_real(tab, u2, pairs2, orc.build_tau(tab, u2, w.phi, w.lam, pairs2), a2)
+    assert np.linalg.norm(k2 - orc.rotate(U, k)) <= 1e-11 * np.linalg.norm(k)
+    e = orc.apply_k1e_real(tab, w.u, a)
+    e2 = orc.apply_k1e_real(tab, u2, a2)
+    assert np.linalg.norm(e2 - orc.rotate(U, e)) <= 1e-11 * np.linalg.norm(e)
