@@ -83,6 +83,12 @@ int bse_apply_k1x(bse_handle *h, const double *a, double *out, int B);
  * is truncated to S before P_c and formed on the apply grid.  K1e - K1x (the caller's sign) is the two-body kernel of eq. 1. */
 int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B);
 
+/* Change of representation of trial blocks between the Kohn-Sham and the localised orbitals (eq. 12, PAPER.md:104-106;
+ * "a transformation of A_s between the two spaces is necessary"):
+ *   transpose == 0: y[b,v,:] = sum_v' U[v][v'] x[b,v',:]      transpose != 0: y[b,v,:] = sum_v' U[v'][v] x[b,v',:]
+ * U: DEVICE [Nv][Nv] row-major real orthogonal (Gamma point); x, y: DEVICE, layout per BSE_VEC_* flag; y must not alias x. */
+int bse_rotate(bse_handle *h, const double *U, int transpose, const double *x, double *y, int B);
+
 /* Same with HOST pointers: copies a to the device, applies, copies out back, synchronises (the end-to-end
  * call bench.py times as `e2e`).  With BSE_TAU_REAL the blocks are pipelined: block b+1 is copied in and block b-1
  * copied out (two copy streams) while block b is applied.  Pinned host memory is needed for the overlap. */

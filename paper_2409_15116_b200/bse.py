@@ -33,6 +33,7 @@ _sig = {
     "bse_apply_k1x": [_vp, _vp, _vp, _i],
     "bse_apply_k1x_host": [_vp, _vp, _vp, _i],
     "bse_apply_k1e": [_vp, _vp, _vp, _i],
+    "bse_rotate": [_vp, _vp, _i, _vp, _vp, _i],
     "bse_set_inputs_host": [_vp, _vp, _vp],
     "bse_destroy": [_vp],
     "bse_npw_half": [_vp, C.POINTER(_ll)],
@@ -99,6 +100,10 @@ def bse_apply_k1x(h, a, out, B):
 
 def bse_apply_k1e(h, a, out, B):
     _check(lib.bse_apply_k1e(h, _ptr(a), _ptr(out), int(B)), "bse_apply_k1e")
+
+
+def bse_rotate(h, U, x, y, B, transpose=False):
+    _check(lib.bse_rotate(h, _ptr(U), 1 if transpose else 0, _ptr(x), _ptr(y), int(B)), "bse_rotate")
 
 
 def bse_apply_k1x_host(h, a_host, out_host, B):

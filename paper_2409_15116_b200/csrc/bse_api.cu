@@ -667,7 +667,7 @@ extern "C" int bse_destroy(bse_handle *h) {
     cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);
     cudaFree(h->part); cudaFree(h->Sov); cudaFree(h->tau_batch); cudaFree(h->a_dev); cudaFree(h->out_dev);
     cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->a_r); cudaFree(h->acc_r);
-    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist); cudaFree(h->k1e_ws); cudaFree(h->u_a);
+    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist); cudaFree(h->k1e_ws); cudaFree(h->u_a); cudaFree(h->Ut);
     for (cudaEvent_t e : h->ev_pipe) cudaEventDestroy(e);
     if (h->s_in) cudaStreamDestroy(h->s_in);
     if (h->s_out) cudaStreamDestroy(h->s_out);
@@ -875,6 +875,36 @@ extern "C" int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B)
         }
     }
     return p_c_rows(h, (double *)out, (long long)B * Nv, 2 * npw_h, (const double *)h->uGw, (const double *)h->uG, 1.0);
+}
+
+// KS <-> localised representation of the trial blocks (eq. 12): y[b] = U x[b] or U^T x[b]
+extern "C" int bse_rotate(bse_handle *h, const double *U, int transpose, const double *x, double *y, int B) {
+    if (!h || !U || !x || !y || B <= 0) { bse_set_error("null pointer or B <= 0"); return BSE_EINVAL; }
+    if (x == y) { bse_set_error("y must not alias x"); return BSE_EINVAL; }
+    const long long K = (h->flags & BSE_VEC_PW) ? 2 * h->fft.npw_h : h->N;
+    const long long lds = ldS(h);
+    const double *A = U;
+    long long lda = h->Nv;
+    int rc;
+    if (transpose) {
+        if (!h->Ut) BSE_CUDA(cudaMalloc(&h->Ut, (size_t)h->Nv * lds * 8));
+        if ((rc = bse_launch_transpose(U, h->Nv, h->Ut, lds, h->Nv, h->stream))) return rc;
+        A = h->Ut;
+        lda = lds;
+    }
+    if (h->Nv & 1) {                       // the tile loader copies 16 B at a time: odd row lengths go through a padded copy
+        if (!transpose) {
+            if (!h->Ut) BSE_CUDA(cudaMalloc(&h->Ut, (size_t)h->Nv * lds * 8));
+            BSE_CUDA(cudaMemcpy2DAsync(h->Ut, (size_t)lds * 8, U, (size_t)h->Nv * 8, (size_t)h->Nv * 8, h->Nv,
+                                       cudaMemcpyDeviceToDevice, h->stream));
+            A = h->Ut;
+            lda = lds;
+        }
+    }
+    for (int b = 0; b < B; ++b)
+        if ((rc = bse_gemm_nn(A, lda, x + (long long)b * h->Nv * K, K, h->Nv, K, h->Nv, EPI_STORE, nullptr, nullptr,
+                              y + (long long)b * h->Nv * K, K, h->stream))) return rc;
+    return BSE_OK;
 }
 
 // ------------------------------------------------------------------------------------------------ accessors

@@ -90,6 +90,7 @@ struct bse_handle {
     // K1e workspaces (grow-only): dens / vH [B][N] (REAL) or one block's a(r) [Nv][Na] + [1][Na] + product rows [Pb][Na] (PW)
     double *k1e_ws = nullptr;
     size_t k1e_bytes = 0;
+    double *Ut = nullptr;                          // [Nv][ldS] transposed copy of the rotation matrix (bse_rotate)
     double *u_a = nullptr;                         // [Nv][Na] orbitals on the apply grid (PW layout with a coarser grid)
     double *a_dev = nullptr, *out_dev = nullptr;   // staging for the host-pointer entry point
     size_t a_dev_bytes = 0;
@@ -127,12 +128,12 @@ int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2
 int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long long N, double *out, cudaStream_t s);
 
 // gemm_dmma.cu
-enum { EPI_PARTIAL = 0, EPI_TAU = 1, EPI_SUB = 2 };
+enum { EPI_PARTIAL = 0, EPI_TAU = 1, EPI_SUB = 2, EPI_STORE = 3 };
 // C[M][N] (+)= A[M][K] * B[N][K]^T, split-K partials into `part` then reduced: C = alpha * colscale[n] * sum
 int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb, int M, int N, long long K,
                  bool squareA, bool squareB, double *part, size_t part_bytes, double *C, long long ldc,
                  double alpha, const double *colscale, cudaStream_t s);
-// NN form: acc = A[M][K] * B[K][N];  EPI_TAU: C = colscale2[n>>1] * (Xin + acc);  EPI_SUB: C = C - acc
+// NN form: acc = A[M][K] * B[K][N];  EPI_TAU: C = colscale2[n>>1] * (Xin + acc);  EPI_SUB: C = C - acc;  EPI_STORE: C = acc
 int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, int M, long long N, int K,
                 int epi, const double *Xin, const double *colscale2, double *C, long long ldc, cudaStream_t s);
 
@@ -146,6 +147,8 @@ int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_b, 
 int bse_launch_k1e_density(const double *u, const double *a, double *dens, int Nv, long long N, int B, cudaStream_t s);
 int bse_launch_k1e_product(const double *u, const double *vH, double *out, int v0, int nrows, long long out_ld,
                            long long N, int B, cudaStream_t s);
+// dst[j][i] = src[i][j], n x n, leading dimensions lds / ldd
+int bse_launch_transpose(const double *src, long long lds, double *dst, long long ldd, int n, cudaStream_t s);
 // dst[w][k] = Omega * wt * src[w][k], wt = 2 for G != 0 and (1, 0) on (re, im) of G = 0 (entry 0 of H)
 int bse_launch_weight_pw(const double2 *src, double2 *dst, long long npw_h, long long rows, double Omega,
                          cudaStream_t s);

@@ -64,6 +64,7 @@ __device__ __forceinline__ void load_tile_n(double *sm, const double *g, long lo
 // EPI_PARTIAL: store raw accumulators to part[z][M][Ntot]  (split-K, K range per blockIdx.z)
 // EPI_TAU    : C[m][n] = cs2[n>>1] * (Xin[m][n] + acc)
 // EPI_SUB    : C[m][n] = C[m][n] - acc
+// EPI_STORE  : C[m][n] = acc
 template <bool BN_MAJOR, int EPI, bool SQA, bool SQB>
 __global__ void __launch_bounds__(THREADS)
 dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restrict__ B, long long ldb, int M,
@@ -271,6 +272,10 @@ int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, 
         k<<<grid, THREADS, SMEM_NN, s>>>(A, lda, B, ldb, M, N, K, K, C, ldc, Xin, colscale2);
     } else if (epi == EPI_SUB) {
         auto k = dgemm_kernel<true, EPI_SUB, false, false>;
+        if ((rc = prep(k, SMEM_NN))) return rc;
+        k<<<grid, THREADS, SMEM_NN, s>>>(A, lda, B, ldb, M, N, K, K, C, ldc, nullptr, nullptr);
+    } else if (epi == EPI_STORE) {
+        auto k = dgemm_kernel<true, EPI_STORE, false, false>;
         if ((rc = prep(k, SMEM_NN))) return rc;
         k<<<grid, THREADS, SMEM_NN, s>>>(A, lda, B, ldb, M, N, K, K, C, ldc, nullptr, nullptr);
     } else {

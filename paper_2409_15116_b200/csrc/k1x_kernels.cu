@@ -227,6 +227,11 @@ k1e_product_kernel(const double *__restrict__ u, const double *__restrict__ vH, 
     }
 }
 
+__global__ void transpose_kernel(const double *__restrict__ src, long long lds, double *__restrict__ dst, long long ldd, int n) {
+    const int i = blockIdx.y * blockDim.y + threadIdx.y, j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n && j < n) dst[(long long)j * ldd + i] = src[(long long)i * lds + j];
+}
+
 __global__ void weight_pw_kernel(const double2 *__restrict__ src, double2 *__restrict__ dst, long long npw_h,
                                  long long total, double Omega) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -329,6 +334,13 @@ int bse_launch_k1e_product(const double *u, const double *vH, double *out, int v
     const int threads = 256;
     const unsigned tiles = (unsigned)((N / 2 + threads - 1) / threads);
     k1e_product_kernel<<<dim3(tiles, nrows), threads, 0, s>>>(u, vH, out, v0, out_ld, N, B);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+int bse_launch_transpose(const double *src, long long lds, double *dst, long long ldd, int n, cudaStream_t s) {
+    dim3 blk(32, 8), grd((n + 31) / 32, (n + 7) / 8);
+    transpose_kernel<<<grd, blk, 0, s>>>(src, lds, dst, ldd, n);
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }

@@ -339,3 +339,47 @@ def test_k1e_real_and_pw_layouts(cfg):
         assert np.sqrt((wt * np.abs(gotx - refx) ** 2).sum() / (wt * np.abs(refx) ** 2).sum()) <= TOL
     finally:
         g.close()
+
+
+@pytest.mark.parametrize("Nv", [5, 8])
+def test_rotate_between_representations(Nv):
+    """bse_rotate (eq. 12) against the oracle's triple loop, both directions, both layouts; then the
+    covariance K(U u, U a) = U K(u, a) of K1x and K1e with every pair kept, end to end on the GPU."""
+    bse = _bse()
+    cfg = wl.Config("rot", 9.0, 12, Nv, 7, 3.0, 1.3, 0.8, 3.0, 0.0, 2, "random", seed=200 + Nv)
+    w = wl.make(cfg=cfg)
+    rng = np.random.default_rng(9)
+    U, _ = np.linalg.qr(rng.normal(size=(Nv, Nv)))
+    U_d = torch.from_numpy(np.ascontiguousarray(U)).to("cuda:0")
+    B = w.a_pw.shape[0]
+    for vec, x in ((bse.BSE_VEC_REAL, w.a_real()), (bse.BSE_VEC_PW, np.ascontiguousarray(w.a_pw).view(np.float64))):
+        g = Gpu(w, vec)
+        try:
+            x_d = torch.from_numpy(np.ascontiguousarray(x)).to("cuda:0")
+            y_d = torch.empty_like(x_d)
+            for tr in (False, True):
+                bse.bse_rotate(g.h, U_d, x_d, y_d, B, transpose=tr)
+                torch.cuda.synchronize()
+                ref = orc.rotate(U, x.reshape(B, Nv, -1), transpose=tr)
+                assert rel(y_d.cpu().numpy().reshape(ref.shape), ref) <= 1e-13
+        finally:
+            g.close()
+    # covariance on the GPU (REAL layout): handle 1 = (u, a), handle 2 = (U u, U a)
+    a = w.a_real()
+    outs = []
+    for uu, aa in ((w.u, a), (U @ w.u, orc.rotate(U, a))):
+        u_d = torch.from_numpy(np.ascontiguousarray(uu)).to("cuda:0")
+        phi_d = torch.from_numpy(np.ascontiguousarray(w.phi).view(np.float64)).to("cuda:0")
+        h = bse.bse_create([w.n] * 3, w.cell, w.ecut, Nv, u_d, w.phi.shape[0], phi_d, w.lam, 0.0, 0)
+        try:
+            bse.bse_build_tau(h)
+            a_d = torch.from_numpy(np.ascontiguousarray(aa)).to("cuda:0")
+            kx, ke = torch.empty_like(a_d), torch.empty_like(a_d)
+            bse.bse_apply_k1x(h, a_d, kx, B)
+            bse.bse_apply_k1e(h, a_d, ke, B)
+            torch.cuda.synchronize()
+            outs.append((kx.cpu().numpy(), ke.cpu().numpy()))
+        finally:
+            bse.bse_destroy(h)
+    assert rel(outs[1][0], orc.rotate(U, outs[0][0])) <= 1e-10
+    assert rel(outs[1][1], orc.rotate(U, outs[0][1])) <= 1e-10
