@@ -50,7 +50,7 @@ struct Geo {
     // phases with another's butterflies), and per CTA the threads that leave each of them >= ~112 registers
     static constexpr int plane_tasks = (n / 2) * R2;
     static constexpr int smem_ctas = 232448 / (plane_smem + 1024) < 1 ? 1 : 232448 / (plane_smem + 1024);
-    static constexpr int thr_cap0 = 65536 / (112 * (smem_ctas > 6 ? 6 : smem_ctas)) / 32 * 32;
+    static constexpr int thr_cap0 = 65536 / (100 * (smem_ctas > 6 ? 6 : smem_ctas)) / 32 * 32;
     static constexpr int thr_cap = thr_cap0 > 512 ? 512 : (thr_cap0 < 64 ? 64 : thr_cap0);
     static constexpr int plane_iters = (plane_tasks + thr_cap - 1) / thr_cap;
     static constexpr int plane_thr = (((plane_tasks + plane_iters - 1) / plane_iters + 31) / 32 * 32) < 64
