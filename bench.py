@@ -330,7 +330,7 @@ def main():
                 "mbytes": round(tot_b / 1e6, 1), "fp64_dmma_tflops": round(dmma_tf, 2), "fp64_dfma_tflops": round(dfma_tf, 2)}
 
     # ---- K1e (eq. 4) timed beside the step: not part of `value` ----
-    k1e_ms = None
+    k1e_ms = k1_ms = None
     if not large or args.vec == "pw":
         for _ in range(2):
             bse.bse_apply_k1e(h, a_d, out_d, B)
@@ -343,6 +343,15 @@ def main():
         ke1.record()
         ke1.synchronize()
         k1e_ms = ke0.elapsed_time(ke1) / reps
+        for _ in range(2):
+            bse.bse_apply_k1(h, a_d, out_d, B, 1.0, -1.0)     # eq. 1: K1e - K1d with one P_c
+        torch.cuda.synchronize()
+        ke0.record()
+        for _ in range(reps):
+            bse.bse_apply_k1(h, a_d, out_d, B, 1.0, -1.0)
+        ke1.record()
+        ke1.synchronize()
+        k1_ms = ke0.elapsed_time(ke1) / reps
 
     # ---- end to end through the C ABI with host (pinned) buffers ----
     e2e = None
@@ -397,7 +406,9 @@ def main():
                    "tau_storage": args.tau, "vec_layout": args.vec, "parallelism": "replicas" if world > 1 else "1gpu",
                    "l2": "512 MB buffer written between timed steps (L2 flush); inputs also exceed L2"},
         "k1x_applies_per_s": world * B / (ta_ms * 1e-3),
-        "k1e_applies_per_s": (world * B / (k1e_ms * 1e-3)) if k1e_ms else None, "k1e_ms": k1e_ms, "build_ms": tb_ms, "apply_ms": ta_ms, "pairs": P,
+        "k1e_applies_per_s": (world * B / (k1e_ms * 1e-3)) if k1e_ms else None, "k1e_ms": k1e_ms,
+        "k1_combined_ms": k1_ms, "k1_combined_applies_per_s": (world * B / (k1_ms * 1e-3)) if k1_ms else None,
+        "build_ms": tb_ms, "apply_ms": ta_ms, "pairs": P,
         "gpu_launches": int(launches), "wall_s_timed_region": wall,
         "clocks": clocks,
         "e2e": e2e,

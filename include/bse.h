@@ -83,6 +83,12 @@ int bse_apply_k1x(bse_handle *h, const double *a, double *out, int B);
  * is truncated to S before P_c and formed on the apply grid.  K1e - K1x (the caller's sign) is the two-body kernel of eq. 1. */
 int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B);
 
+/* Both two-body terms in one call, sharing the transforms of a, the accumulated rows and ONE P_c:
+ *   out[b,v] = P_c ( ce * 2 u_v v_H[b]  +  cd * sum_v' tau_vv' a[b,v'] );   eq. 1 uses ce = 1, cd = -1.
+ * Equals ce * bse_apply_k1e + cd * bse_apply_k1x (P_c is linear) at about the cost of bse_apply_k1x alone.
+ * BSE_ESTATE if bse_build_tau has not run. */
+int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, double ce, double cd);
+
 /* Change of representation of trial blocks between the Kohn-Sham and the localised orbitals (eq. 12, PAPER.md:104-106;
  * "a transformation of A_s between the two spaces is necessary"):
  *   transpose == 0: y[b,v,:] = sum_v' U[v][v'] x[b,v',:]      transpose != 0: y[b,v,:] = sum_v' U[v'][v] x[b,v',:]

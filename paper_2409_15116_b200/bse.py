@@ -34,6 +34,7 @@ _sig = {
     "bse_apply_k1x_host": [_vp, _vp, _vp, _i],
     "bse_apply_k1e": [_vp, _vp, _vp, _i],
     "bse_rotate": [_vp, _vp, _i, _vp, _vp, _i],
+    "bse_apply_k1": [_vp, _vp, _vp, _i, _d, _d],
     "bse_set_inputs_host": [_vp, _vp, _vp],
     "bse_destroy": [_vp],
     "bse_npw_half": [_vp, C.POINTER(_ll)],
@@ -100,6 +101,10 @@ def bse_apply_k1x(h, a, out, B):
 
 def bse_apply_k1e(h, a, out, B):
     _check(lib.bse_apply_k1e(h, _ptr(a), _ptr(out), int(B)), "bse_apply_k1e")
+
+
+def bse_apply_k1(h, a, out, B, ce=1.0, cd=-1.0):
+    _check(lib.bse_apply_k1(h, _ptr(a), _ptr(out), int(B), float(ce), float(cd)), "bse_apply_k1")
 
 
 def bse_rotate(h, U, x, y, B, transpose=False):

@@ -476,6 +476,63 @@ int plan_apply_memory(bse_handle *h, int B) {
     return BSE_OK;
 }
 
+// ---- K1e helpers (eq. 4): workspace, Hartree potential in place, orbitals on the apply grid
+int ensure_k1e_ws(bse_handle *h, size_t bytes) {
+    if (h->k1e_bytes >= bytes) return BSE_OK;
+    cudaFree(h->k1e_ws);
+    h->k1e_ws = nullptr; h->k1e_bytes = 0;
+    if (cudaMalloc(&h->k1e_ws, bytes) != cudaSuccess) {
+        // the K1x apply plan holds the free memory: drop it (the next apply plans again around this workspace)
+        (void)cudaGetLastError();
+        h->k1e_ws = nullptr;
+        BSE_CUDA(cudaStreamSynchronize(h->stream));
+        cudaFree(h->tau_batch); cudaFree(h->a_r); cudaFree(h->acc_r);
+        h->tau_batch = h->a_r = h->acc_r = nullptr;
+        h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
+        BSE_CUDA(cudaMalloc(&h->k1e_ws, bytes));
+    }
+    h->k1e_bytes = bytes;
+    return BSE_OK;
+}
+
+// n -> v_H in place for cnt fields held at buf ([cnt][pl.N]): forward transform with the v_c / N scaling (a3 + a4 with
+// v_c instead of v_c^{1/2}), inverse transform (a9)
+int hartree_in_place(bse_handle *h, const FftPlan &pl, double *buf, int nfields) {
+    int rc;
+    for (int c0 = 0; c0 < nfields; c0 += (int)h->Pb) {
+        const int cnt = (int)std::min<long long>(h->Pb, nfields - c0);
+        if ((rc = st_fwd_plane(h, pl, buf, nullptr, c0, cnt))) return rc;
+        if ((rc = st_fwd_stick(h, pl, cnt, h->X, pl.vcn))) return rc;
+        if ((rc = st_inv_stick(h, pl, h->X, cnt))) return rc;
+        if ((rc = st_inv_plane(h, pl, cnt, buf + (long long)c0 * pl.N))) return rc;
+    }
+    return BSE_OK;
+}
+
+// orbitals on the apply grid of the PW layout: u_a = inverse transform of u(G) on n_a (u is band-limited to S)
+int ensure_u_apply(bse_handle *h) {
+    if (h->ap == &h->fft || h->u_a) return BSE_OK;
+    const FftPlan &pl = *h->ap;
+    int rc;
+    if ((rc = ensure_u_pw(h))) return rc;
+    if (cudaMalloc(&h->u_a, (size_t)h->Nv * pl.N * 8) != cudaSuccess) {
+        // the K1x apply plan holds the free memory: drop it (the next K1x apply plans again, with u_a in place)
+        (void)cudaGetLastError();
+        h->u_a = nullptr;
+        BSE_CUDA(cudaStreamSynchronize(h->stream));
+        cudaFree(h->tau_batch); cudaFree(h->a_r); cudaFree(h->acc_r);
+        h->tau_batch = h->a_r = h->acc_r = nullptr;
+        h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
+        BSE_CUDA(cudaMalloc(&h->u_a, (size_t)h->Nv * pl.N * 8));
+    }
+    for (long long v0 = 0; v0 < h->Nv; v0 += h->Pb) {
+        const int cnt = (int)std::min<long long>(h->Pb, h->Nv - v0);
+        if ((rc = st_inv_stick(h, pl, h->uG + v0 * pl.npw_h, cnt))) return rc;
+        if ((rc = st_inv_plane(h, pl, cnt, h->u_a + v0 * pl.N))) return rc;
+    }
+    return BSE_OK;
+}
+
 // forward transform of `rows` accumulated fields of each of nb blocks into the PW output (a12): acc(G) on H
 int rows_to_pw(bse_handle *h, const double *acc, long long acc_ld, int rows, int nb, double2 *out_pw, const int *dest) {
     const FftPlan &pl = *h->ap;
@@ -503,6 +560,11 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
     if (mode == BSE_TAU_REAL) {
         double *acc = acc_real ? acc_real : h->acc_r;
         if ((rc = st_accumulate(h, h->tau_r, 0, h->P, a, acc, nb, true))) return rc;
+        if (h->mix_on) {
+            StageTimer t(h, BSE_ST_K1E_PRODUCT, 3.0 * nb * h->Nv * (double)h->ap->N, 8.0 * h->ap->N * (2.0 * nb * h->Nv + h->Nv + nb));
+            if ((rc = bse_launch_k1_mix(h->mix_u, h->mix_vH, acc, nullptr, h->Nv, h->Nv, false, h->ap->N, nb, h->mix_ce,
+                                        h->mix_cd, h->stream))) return rc;
+        }
         return out_pw ? rows_to_pw(h, acc, h->Nv, h->Nv, nb, out_pw, nullptr) : BSE_OK;
     }
     const FftPlan &pl = *h->ap;
@@ -523,6 +585,14 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
           if (acc_real) rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, h->rowlist + r0, rows, a, acc_real, h->Nv, false, nb);
           else rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, h->rowlist + r0, rows, a, h->acc_r, h->rows_cap, true, nb);
           if (rc) return rc; }
+        if (h->mix_on) {
+            StageTimer t(h, BSE_ST_K1E_PRODUCT, 3.0 * nb * rows * (double)pl.N, m.N8 * (2.0 * nb * rows + rows + nb));
+            if (acc_real) rc = bse_launch_k1_mix(h->mix_u, h->mix_vH, acc_real, h->rowlist + r0, rows, h->Nv, false, pl.N, nb,
+                                                 h->mix_ce, h->mix_cd, h->stream);
+            else rc = bse_launch_k1_mix(h->mix_u, h->mix_vH, h->acc_r, h->rowlist + r0, rows, h->rows_cap, true, pl.N, nb,
+                                        h->mix_ce, h->mix_cd, h->stream);
+            if (rc) return rc;
+        }
         if (out_pw && (rc = rows_to_pw(h, h->acc_r, h->rows_cap, rows, nb, out_pw, h->rowlist + r0))) return rc;
     }
     return BSE_OK;
@@ -542,6 +612,13 @@ int apply_pw(bse_handle *h, const double2 *a, double2 *out, int B) {
             const int cnt = (int)std::min<long long>(h->Pb, fields - f0);
             if ((rc = st_inv_stick(h, pl, ag + f0 * npw_h, cnt))) return rc;
             if ((rc = st_inv_plane(h, pl, cnt, h->a_r + f0 * pl.N))) return rc;
+        }
+        if (h->mix_on) {                                              // v_H of this group's blocks (K1e part of bse_apply_k1)
+            double *vH = h->k1e_ws;
+            { StageTimer t(h, BSE_ST_K1E_DENSITY, 2.0 * nb * Nv * (double)pl.N, 8.0 * pl.N * (double)(nb * Nv + Nv + nb));
+              if ((rc = bse_launch_k1e_density(h->mix_u, h->a_r, vH, h->Nv, pl.N, nb, h->stream))) return rc; }
+            if ((rc = hartree_in_place(h, pl, vH, nb))) return rc;
+            h->mix_vH = vH;
         }
         if ((rc = accumulate_all(h, h->a_r, nb, nullptr, out + (long long)b0 * Nv * npw_h))) return rc;
     }
@@ -772,57 +849,6 @@ extern "C" int bse_set_inputs_host(bse_handle *h, const double *u_host, const do
 }
 
 // ------------------------------------------------------------------------------------------------ K1e (eq. 4)
-namespace {
-
-int ensure_k1e_ws(bse_handle *h, size_t bytes) {
-    if (h->k1e_bytes >= bytes) return BSE_OK;
-    cudaFree(h->k1e_ws);
-    h->k1e_ws = nullptr; h->k1e_bytes = 0;
-    BSE_CUDA(cudaMalloc(&h->k1e_ws, bytes));
-    h->k1e_bytes = bytes;
-    return BSE_OK;
-}
-
-// n -> v_H in place for cnt fields held at buf ([cnt][pl.N]): forward transform with the v_c / N scaling (a3 + a4 with
-// v_c instead of v_c^{1/2}), inverse transform (a9)
-int hartree_in_place(bse_handle *h, const FftPlan &pl, double *buf, int nfields) {
-    int rc;
-    for (int c0 = 0; c0 < nfields; c0 += (int)h->Pb) {
-        const int cnt = (int)std::min<long long>(h->Pb, nfields - c0);
-        if ((rc = st_fwd_plane(h, pl, buf, nullptr, c0, cnt))) return rc;
-        if ((rc = st_fwd_stick(h, pl, cnt, h->X, pl.vcn))) return rc;
-        if ((rc = st_inv_stick(h, pl, h->X, cnt))) return rc;
-        if ((rc = st_inv_plane(h, pl, cnt, buf + (long long)c0 * pl.N))) return rc;
-    }
-    return BSE_OK;
-}
-
-// orbitals on the apply grid of the PW layout: u_a = inverse transform of u(G) on n_a (u is band-limited to S)
-int ensure_u_apply(bse_handle *h) {
-    if (h->ap == &h->fft || h->u_a) return BSE_OK;
-    const FftPlan &pl = *h->ap;
-    int rc;
-    if ((rc = ensure_u_pw(h))) return rc;
-    if (cudaMalloc(&h->u_a, (size_t)h->Nv * pl.N * 8) != cudaSuccess) {
-        // the K1x apply plan holds the free memory: drop it (the next K1x apply plans again, with u_a in place)
-        (void)cudaGetLastError();
-        h->u_a = nullptr;
-        BSE_CUDA(cudaStreamSynchronize(h->stream));
-        cudaFree(h->tau_batch); cudaFree(h->a_r); cudaFree(h->acc_r);
-        h->tau_batch = h->a_r = h->acc_r = nullptr;
-        h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
-        BSE_CUDA(cudaMalloc(&h->u_a, (size_t)h->Nv * pl.N * 8));
-    }
-    for (long long v0 = 0; v0 < h->Nv; v0 += h->Pb) {
-        const int cnt = (int)std::min<long long>(h->Pb, h->Nv - v0);
-        if ((rc = st_inv_stick(h, pl, h->uG + v0 * pl.npw_h, cnt))) return rc;
-        if ((rc = st_inv_plane(h, pl, cnt, h->u_a + v0 * pl.N))) return rc;
-    }
-    return BSE_OK;
-}
-
-}  // namespace
-
 extern "C" int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B) {
     if (!h || !a || !out || B <= 0) { bse_set_error("null pointer or B <= 0"); return BSE_EINVAL; }
     if (a == out) { bse_set_error("out must not alias a"); return BSE_EINVAL; }
@@ -875,6 +901,43 @@ extern "C" int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B)
         }
     }
     return p_c_rows(h, (double *)out, (long long)B * Nv, 2 * npw_h, (const double *)h->uGw, (const double *)h->uG, 1.0);
+}
+
+// Two-body kernel in one call (eq. 1: K1e and K1d enter with one P_c): out = P_c( ce * 2 u_v v_H + cd * sum_v' tau_vv' a_v' )
+extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, double ce, double cd) {
+    if (!h || !a || !out || B <= 0) { bse_set_error("null pointer or B <= 0"); return BSE_EINVAL; }
+    if (!h->built) { bse_set_error("bse_apply_k1 before bse_build_tau"); return BSE_ESTATE; }
+    if (a == out) { bse_set_error("out must not alias a"); return BSE_EINVAL; }
+    int rc;
+    const bool pw = (h->flags & BSE_VEC_PW) != 0;
+    if (pw) {                                                   // K1e needs u on the apply grid: before the plan sizes itself
+        if ((rc = ensure_u_pw(h))) return rc;
+        if ((rc = ensure_u_apply(h))) return rc;
+    }
+    if ((rc = ensure_k1e_ws(h, (size_t)B * h->ap->N * 8))) return rc;
+    if ((h->flags & BSE_TAU_MASK) == BSE_TAU_STREAM) {
+        if ((rc = ensure_tau_store(h, false))) return rc;
+        if ((rc = fill_tau_store(h, false))) return rc;
+    }
+    if ((rc = plan_apply_memory(h, B))) return rc;
+    h->mix_ce = ce; h->mix_cd = cd;
+    h->mix_u = (pw && h->u_a) ? h->u_a : h->u;
+    if (pw) {
+        h->mix_on = true;
+        rc = apply_pw(h, (const double2 *)a, (double2 *)out, B);
+        h->mix_on = false;
+        return rc;
+    }
+    const FftPlan &pl = h->fft;
+    { StageTimer t(h, BSE_ST_K1E_DENSITY, 2.0 * B * h->Nv * (double)pl.N, 8.0 * pl.N * (double)(B * h->Nv + h->Nv + B));
+      if ((rc = bse_launch_k1e_density(h->u, a, h->k1e_ws, h->Nv, pl.N, B, h->stream))) return rc; }
+    if ((rc = hartree_in_place(h, pl, h->k1e_ws, B))) return rc;
+    h->mix_vH = h->k1e_ws;
+    h->mix_on = true;
+    rc = accumulate_all(h, a, B, out, nullptr);
+    h->mix_on = false;
+    if (rc) return rc;
+    return p_c_rows(h, out, (long long)B * h->Nv, h->N, h->u, h->u, h->dV);
 }
 
 // KS <-> localised representation of the trial blocks (eq. 12): y[b] = U x[b] or U^T x[b]

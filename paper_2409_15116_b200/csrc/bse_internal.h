@@ -90,6 +90,11 @@ struct bse_handle {
     // K1e workspaces (grow-only): dens / vH [B][N] (REAL) or one block's a(r) [Nv][Na] + [1][Na] + product rows [Pb][Na] (PW)
     double *k1e_ws = nullptr;
     size_t k1e_bytes = 0;
+    // combined K1e / K1x call (bse_apply_k1): while mix_on, accumulate_all folds ce * 2 u_v vH[b] into the accumulated rows
+    bool mix_on = false;
+    double mix_ce = 0.0, mix_cd = 1.0;
+    const double *mix_u = nullptr;                 // orbitals on the grid the apply runs on
+    const double *mix_vH = nullptr;                // [nb][N] Hartree potentials of the blocks being accumulated
     double *Ut = nullptr;                          // [Nv][ldS] transposed copy of the rotation matrix (bse_rotate)
     double *u_a = nullptr;                         // [Nv][Na] orbitals on the apply grid (PW layout with a coarser grid)
     double *a_dev = nullptr, *out_dev = nullptr;   // staging for the host-pointer entry point
@@ -147,6 +152,9 @@ int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_b, 
 int bse_launch_k1e_density(const double *u, const double *a, double *dens, int Nv, long long N, int B, cudaStream_t s);
 int bse_launch_k1e_product(const double *u, const double *vH, double *out, int v0, int nrows, long long out_ld,
                            long long N, int B, cudaStream_t s);
+// acc row <- cd * acc row + 2 ce * u[v] * vH[b] on nrows rows (rows: device row ids or nullptr = identity)
+int bse_launch_k1_mix(const double *u, const double *vH, double *acc, const int *rows, int nrows, long long acc_ld,
+                      bool local, long long N, int nb, double ce, double cd, cudaStream_t s);
 // dst[j][i] = src[i][j], n x n, leading dimensions lds / ldd
 int bse_launch_transpose(const double *src, long long lds, double *dst, long long ldd, int n, cudaStream_t s);
 // dst[w][k] = Omega * wt * src[w][k], wt = 2 for G != 0 and (1, 0) on (re, im) of G = 0 (entry 0 of H)

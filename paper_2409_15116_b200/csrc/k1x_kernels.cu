@@ -227,6 +227,25 @@ k1e_product_kernel(const double *__restrict__ u, const double *__restrict__ vH, 
     }
 }
 
+// Combined two-body kernel (eq. 1: K1e - K1d share one P_c): acc row <- cd * acc row + ce2 * u[v][r] * vH[b][r] on the rows of
+// a batch (rows == nullptr: row i = i); acc row index = position in the batch (local) or the row id.
+__global__ void __launch_bounds__(256)
+k1_mix_kernel(const double *__restrict__ u, const double *__restrict__ vH, double *__restrict__ acc,
+              const int *__restrict__ rows, long long acc_ld, int local, long long N, int nb, double ce2, double cd) {
+    const long long r = 2 * ((long long)blockIdx.x * blockDim.x + threadIdx.x);
+    if (r >= N) return;
+    const int i = blockIdx.y;
+    const int v = rows ? rows[i] : i;
+    const int arow = local ? i : v;
+    const double2 x = *reinterpret_cast<const double2 *>(u + (long long)v * N + r);
+    for (int b = 0; b < nb; ++b) {
+        const double2 y = *reinterpret_cast<const double2 *>(vH + (long long)b * N + r);
+        double2 *dst = reinterpret_cast<double2 *>(acc + ((long long)b * acc_ld + arow) * N + r);
+        const double2 p = *dst;
+        *dst = make_double2(fma(ce2 * x.x, y.x, cd * p.x), fma(ce2 * x.y, y.y, cd * p.y));
+    }
+}
+
 __global__ void transpose_kernel(const double *__restrict__ src, long long lds, double *__restrict__ dst, long long ldd, int n) {
     const int i = blockIdx.y * blockDim.y + threadIdx.y, j = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n && j < n) dst[(long long)j * ldd + i] = src[(long long)i * lds + j];
@@ -341,6 +360,15 @@ int bse_launch_k1e_product(const double *u, const double *vH, double *out, int v
 int bse_launch_transpose(const double *src, long long lds, double *dst, long long ldd, int n, cudaStream_t s) {
     dim3 blk(32, 8), grd((n + 31) / 32, (n + 7) / 8);
     transpose_kernel<<<grd, blk, 0, s>>>(src, lds, dst, ldd, n);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+int bse_launch_k1_mix(const double *u, const double *vH, double *acc, const int *rows, int nrows, long long acc_ld,
+                      bool local, long long N, int nb, double ce, double cd, cudaStream_t s) {
+    const int threads = 256;
+    const unsigned tiles = (unsigned)((N / 2 + threads - 1) / threads);
+    k1_mix_kernel<<<dim3(tiles, nrows), threads, 0, s>>>(u, vH, acc, rows, acc_ld, local ? 1 : 0, N, nb, 2.0 * ce, cd);
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }

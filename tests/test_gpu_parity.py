@@ -383,3 +383,49 @@ def test_rotate_between_representations(Nv):
             bse.bse_destroy(h)
     assert rel(outs[1][0], orc.rotate(U, outs[0][0])) <= 1e-10
     assert rel(outs[1][1], orc.rotate(U, outs[0][1])) <= 1e-10
+
+
+@pytest.mark.parametrize("tau", ["real", "pw", "stream"])
+def test_combined_two_body_call(tau, monkeypatch):
+    """bse_apply_k1 = ce * K1e + cd * K1x with one P_c (eq. 1), against the oracle's two terms, both layouts, every tau mode;
+    the PW case is also forced through several block groups and row batches."""
+    bse = _bse()
+    flag = {"real": bse.BSE_TAU_REAL, "pw": bse.BSE_TAU_PW, "stream": bse.BSE_TAU_STREAM}[tau]
+    cfg = wl.Config("k1", 10.0, 24, 9, 20, 8.0, 1.2, 0.8, 3.0, 0.02, 3, "random", seed=78)
+    w = wl.make(cfg=cfg)
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    B = w.a_pw.shape[0]
+    pairs, _ = orc.screen_pairs(w.u, w.eta)
+    tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs, want="r")
+    ce, cd = 1.0, -1.0
+    a = w.a_real()
+    ref_r = ce * orc.apply_k1e_real(tab, w.u, a) + cd * orc.apply_k1x_real(tab, w.u, pairs, tau_ref, a)
+    ref_g = ce * orc.apply_k1e_pw(tab, w.u, w.a_pw) + cd * orc.apply_k1x_pw(tab, w.u, pairs, tau_ref, w.a_pw)
+    g = Gpu(w, flag)
+    try:
+        g.build()
+        a_d = torch.from_numpy(np.ascontiguousarray(a)).to("cuda:0")
+        out = torch.empty_like(a_d)
+        bse.bse_apply_k1(g.h, a_d, out, B, ce, cd)
+        torch.cuda.synchronize()
+        assert rel(out.cpu().numpy(), ref_r) <= TOL
+    finally:
+        g.close()
+    wt = np.full(tab.npw_h, 2.0)
+    wt[0] = 1.0
+    for forced in (False, True):
+        if forced:
+            monkeypatch.setenv("BSE_MAX_GROUP", "2")
+            monkeypatch.setenv("BSE_MAX_BATCH", "7")
+        g = Gpu(w, flag | bse.BSE_VEC_PW)
+        try:
+            g.build()
+            a_d = torch.from_numpy(np.ascontiguousarray(w.a_pw).view(np.float64)).to("cuda:0")
+            out = torch.empty_like(a_d)
+            bse.bse_apply_k1(g.h, a_d, out, B, ce, cd)
+            torch.cuda.synchronize()
+            got = out.cpu().numpy().view(np.complex128).reshape(ref_g.shape)
+            err = np.sqrt((wt * np.abs(got - ref_g) ** 2).sum() / (wt * np.abs(ref_g) ** 2).sum())
+            assert err <= TOL, (forced, err)
+        finally:
+            g.close()
