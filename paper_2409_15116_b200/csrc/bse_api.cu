@@ -589,8 +589,18 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
             StageTimer t(h, BSE_ST_K1E_PRODUCT, 3.0 * nb * rows * (double)pl.N, m.N8 * (2.0 * nb * rows + rows + nb));
             if (acc_real) rc = bse_launch_k1_mix(h->mix_u, h->mix_vH, acc_real, h->rowlist + r0, rows, h->Nv, false, pl.N, nb,
                                                  h->mix_ce, h->mix_cd, h->stream);
-            else rc = bse_launch_k1_mix(h->mix_u, h->mix_vH, h->acc_r, h->rowlist + r0, rows, h->rows_cap, true, pl.N, nb,
-                                        h->mix_ce, h->mix_cd, h->stream);
+            else if (h->mix_u) rc = bse_launch_k1_mix(h->mix_u, h->mix_vH, h->acc_r, h->rowlist + r0, rows, h->rows_cap, true, pl.N,
+                                                      nb, h->mix_ce, h->mix_cd, h->stream);
+            else {                                                    // the rows' orbitals on the apply grid, on the fly
+                double *ub = h->k1e_ws + (long long)h->mix_B * pl.N;
+                for (int c0 = 0; c0 < rows && !rc; c0 += (int)h->Pb) {
+                    const int c = (int)std::min<long long>(h->Pb, rows - c0);
+                    if ((rc = bse_launch_inv_stick(pl, h->uG, c, h->Z, h->stream, h->rowlist, r0 + c0))) break;
+                    if ((rc = bse_launch_inv_plane(pl, h->Z, c, pl.N, ub, h->stream))) break;
+                    rc = bse_launch_k1_mix(ub, h->mix_vH, h->acc_r + (long long)c0 * pl.N, nullptr, c, h->rows_cap, true, pl.N, nb,
+                                           h->mix_ce, h->mix_cd, h->stream);
+                }
+            }
             if (rc) return rc;
         }
         if (out_pw && (rc = rows_to_pw(h, h->acc_r, h->rows_cap, rows, nb, out_pw, h->rowlist + r0))) return rc;
@@ -615,8 +625,19 @@ int apply_pw(bse_handle *h, const double2 *a, double2 *out, int B) {
         }
         if (h->mix_on) {                                              // v_H of this group's blocks (K1e part of bse_apply_k1)
             double *vH = h->k1e_ws;
-            { StageTimer t(h, BSE_ST_K1E_DENSITY, 2.0 * nb * Nv * (double)pl.N, 8.0 * pl.N * (double)(nb * Nv + Nv + nb));
-              if ((rc = bse_launch_k1e_density(h->mix_u, h->a_r, vH, h->Nv, pl.N, nb, h->stream))) return rc; }
+            if (h->mix_u) {
+                StageTimer t(h, BSE_ST_K1E_DENSITY, 2.0 * nb * Nv * (double)pl.N, 8.0 * pl.N * (double)(nb * Nv + Nv + nb));
+                if ((rc = bse_launch_k1e_density(h->mix_u, h->a_r, vH, h->Nv, pl.N, nb, h->stream))) return rc;
+            } else {                                                  // u on the apply grid made on the fly, Pb orbitals at a time
+                double *ub = h->k1e_ws + (long long)B * pl.N;
+                for (long long v0 = 0; v0 < Nv; v0 += h->Pb) {
+                    const int cnt = (int)std::min<long long>(h->Pb, Nv - v0);
+                    if ((rc = st_inv_stick(h, pl, h->uG + v0 * npw_h, cnt))) return rc;
+                    if ((rc = st_inv_plane(h, pl, cnt, ub))) return rc;
+                    StageTimer t(h, BSE_ST_K1E_DENSITY, 2.0 * nb * cnt * (double)pl.N, 8.0 * pl.N * (double)(nb * cnt + cnt + nb));
+                    if ((rc = bse_launch_k1e_density(ub, h->a_r, vH, h->Nv, pl.N, nb, h->stream, (int)v0, cnt, v0 > 0))) return rc;
+                }
+            }
             if ((rc = hartree_in_place(h, pl, vH, nb))) return rc;
             h->mix_vH = vH;
         }
@@ -910,18 +931,23 @@ extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, 
     if (a == out) { bse_set_error("out must not alias a"); return BSE_EINVAL; }
     int rc;
     const bool pw = (h->flags & BSE_VEC_PW) != 0;
-    if (pw) {                                                   // K1e needs u on the apply grid: before the plan sizes itself
-        if ((rc = ensure_u_pw(h))) return rc;
-        if ((rc = ensure_u_apply(h))) return rc;
+    const bool fly = pw && h->ap != &h->fft && (h->flags & BSE_TAU_MASK) != BSE_TAU_REAL;   // u on the apply grid is made on
+    if (pw && (rc = ensure_u_pw(h))) return rc;                 // the fly from u(G), Pb orbitals at a time: no [Nv][Na] copy
+    if (pw && !fly && (rc = ensure_u_apply(h))) return rc;
+    if (fly && h->u_a) {                                        // a copy left by bse_apply_k1e: give its memory to the plan
+        BSE_CUDA(cudaStreamSynchronize(h->stream));
+        cudaFree(h->u_a);
+        h->u_a = nullptr;
+        h->plan_ok = false;
     }
-    if ((rc = ensure_k1e_ws(h, (size_t)B * h->ap->N * 8))) return rc;
+    if ((rc = ensure_k1e_ws(h, (size_t)(B + (fly ? h->Pb : 0)) * h->ap->N * 8))) return rc;
     if ((h->flags & BSE_TAU_MASK) == BSE_TAU_STREAM) {
         if ((rc = ensure_tau_store(h, false))) return rc;
         if ((rc = fill_tau_store(h, false))) return rc;
     }
     if ((rc = plan_apply_memory(h, B))) return rc;
-    h->mix_ce = ce; h->mix_cd = cd;
-    h->mix_u = (pw && h->u_a) ? h->u_a : h->u;
+    h->mix_ce = ce; h->mix_cd = cd; h->mix_B = B;
+    h->mix_u = fly ? nullptr : ((pw && h->u_a) ? h->u_a : h->u);
     if (pw) {
         h->mix_on = true;
         rc = apply_pw(h, (const double2 *)a, (double2 *)out, B);

@@ -93,7 +93,8 @@ struct bse_handle {
     // combined K1e / K1x call (bse_apply_k1): while mix_on, accumulate_all folds ce * 2 u_v vH[b] into the accumulated rows
     bool mix_on = false;
     double mix_ce = 0.0, mix_cd = 1.0;
-    const double *mix_u = nullptr;                 // orbitals on the grid the apply runs on
+    int mix_B = 0;
+    const double *mix_u = nullptr;                 // orbitals on the grid the apply runs on; nullptr: made on the fly from uG
     const double *mix_vH = nullptr;                // [nb][N] Hartree potentials of the blocks being accumulated
     double *Ut = nullptr;                          // [Nv][ldS] transposed copy of the rotation matrix (bse_rotate)
     double *u_a = nullptr;                         // [Nv][Na] orbitals on the apply grid (PW layout with a coarser grid)
@@ -149,7 +150,9 @@ int bse_launch_pairlist(bse_handle *h);                 // M -> rowcnt,rowptr,pi
 int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_b, const int *eslot, const int *rows,
                                int nrows, const double *a, double *acc, long long acc_ld, bool local, int B);
 // K1e (eq. 4): dens[b][r] = sum_v u[v][r] a[b][v][r];  out[b * out_ld + i][r] = 2 u[v0 + i][r] vH[b][r], i < nrows
-int bse_launch_k1e_density(const double *u, const double *a, double *dens, int Nv, long long N, int B, cudaStream_t s);
+// u: the orbitals v0 .. v0 + nv (nv < 0: all Nv, v0 = 0); add: dens += instead of dens =
+int bse_launch_k1e_density(const double *u, const double *a, double *dens, int Nv, long long N, int B, cudaStream_t s,
+                           int v0 = 0, int nv = -1, bool add = false);
 int bse_launch_k1e_product(const double *u, const double *vH, double *out, int v0, int nrows, long long out_ld,
                            long long N, int B, cudaStream_t s);
 // acc row <- cd * acc row + 2 ce * u[v] * vH[b] on nrows rows (rows: device row ids or nullptr = identity)

@@ -189,19 +189,19 @@ accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict
 template <int BB>
 __global__ void __launch_bounds__(256)
 k1e_density_kernel(const double *__restrict__ u, const double *__restrict__ a, double *__restrict__ dens, int Nv,
-                   long long N, int B) {
+                   long long N, int B, int v0, int nv, int add) {
     const long long r = 2 * ((long long)blockIdx.x * blockDim.x + threadIdx.x);
     if (r >= N) return;
     const int b0 = blockIdx.y * BB;
     double2 s[BB];
 #pragma unroll
     for (int b = 0; b < BB; ++b) s[b] = make_double2(0.0, 0.0);
-    for (int v = 0; v < Nv; ++v) {
+    for (int v = 0; v < nv; ++v) {                     // u holds the orbitals v0 .. v0 + nv (a chunk), a all Nv of them
         const double2 x = *reinterpret_cast<const double2 *>(u + (long long)v * N + r);
 #pragma unroll
         for (int b = 0; b < BB; ++b) {
             if (b0 + b < B) {
-                const double2 y = __ldcs(reinterpret_cast<const double2 *>(a + ((long long)(b0 + b) * Nv + v) * N + r));
+                const double2 y = __ldcs(reinterpret_cast<const double2 *>(a + ((long long)(b0 + b) * Nv + v0 + v) * N + r));
                 s[b].x = fma(x.x, y.x, s[b].x);
                 s[b].y = fma(x.y, y.y, s[b].y);
             }
@@ -209,7 +209,11 @@ k1e_density_kernel(const double *__restrict__ u, const double *__restrict__ a, d
     }
 #pragma unroll
     for (int b = 0; b < BB; ++b)
-        if (b0 + b < B) *reinterpret_cast<double2 *>(dens + (long long)(b0 + b) * N + r) = s[b];
+        if (b0 + b < B) {
+            double2 *dst = reinterpret_cast<double2 *>(dens + (long long)(b0 + b) * N + r);
+            if (add) { const double2 o = *dst; s[b].x += o.x; s[b].y += o.y; }
+            *dst = s[b];
+        }
 }
 
 // out[(b * out_ld + v - v0)][r] = 2 u[v][r] vH[b][r] for v in [v0, v0 + gridDim.y), b < B
@@ -340,10 +344,12 @@ int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_dir
     return BSE_OK;
 }
 
-int bse_launch_k1e_density(const double *u, const double *a, double *dens, int Nv, long long N, int B, cudaStream_t s) {
+int bse_launch_k1e_density(const double *u, const double *a, double *dens, int Nv, long long N, int B, cudaStream_t s,
+                           int v0, int nv, bool add) {
     const int threads = 256;
     const unsigned tiles = (unsigned)((N / 2 + threads - 1) / threads);
-    k1e_density_kernel<4><<<dim3(tiles, (B + 3) / 4), threads, 0, s>>>(u, a, dens, Nv, N, B);
+    if (nv < 0) nv = Nv;
+    k1e_density_kernel<4><<<dim3(tiles, (B + 3) / 4), threads, 0, s>>>(u, a, dens, Nv, N, B, v0, nv, add ? 1 : 0);
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }
