@@ -429,3 +429,35 @@ def test_combined_two_body_call(tau, monkeypatch):
             assert err <= TOL, (forced, err)
         finally:
             g.close()
+
+
+def test_block_count_grows_and_stream_real_batches(monkeypatch):
+    """One handle, PW layout: B = 1 first, then B = 3 (the apply plan is re-made for the larger group) - same rows both
+    times.  Then the REAL layout with BSE_TAU_STREAM forced through several row batches."""
+    bse = _bse()
+    cfg = wl.Config("grow", 10.0, 24, 7, 12, 8.0, 1.2, 0.8, 3.0, 0.02, 3, "random", seed=79)
+    w = wl.make(cfg=cfg)
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    pairs, _ = orc.screen_pairs(w.u, w.eta)
+    tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs, want="r")
+    ref = orc.apply_k1x_pw(tab, w.u, pairs, tau_ref, w.a_pw)
+    wt = np.full(tab.npw_h, 2.0)
+    wt[0] = 1.0
+    g = Gpu(w, bse.BSE_TAU_PW | bse.BSE_VEC_PW)
+    try:
+        g.build()
+        a_all = torch.from_numpy(np.ascontiguousarray(w.a_pw).view(np.float64)).to("cuda:0")
+        for B in (1, 3, 2):
+            out = torch.empty_like(a_all[:B])
+            bse.bse_apply_k1x(g.h, a_all[:B].contiguous(), out, B)
+            torch.cuda.synchronize()
+            got = out.cpu().numpy().view(np.complex128).reshape(ref[:B].shape)
+            err = np.sqrt((wt * np.abs(got - ref[:B]) ** 2).sum() / (wt * np.abs(ref[:B]) ** 2).sum())
+            assert err <= TOL, (B, err)
+        # tau(G) of a pair range straight from the store
+        tg_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs[2:5], want="G")
+        assert rel(g.tau_g(2, 3), tg_ref) <= TOL
+    finally:
+        g.close()
+    monkeypatch.setenv("BSE_MAX_BATCH", "5")
+    _check_full(w, bse.BSE_TAU_STREAM, check_g=True)
