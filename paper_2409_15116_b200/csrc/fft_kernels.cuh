@@ -22,6 +22,7 @@
 // Stick pass (one CTA = TS sticks of one pair, all i1): S1 from global, S2 to global with the v_c^{1/2}/N scaling and the
 // gather to the half sphere H (forward) / scatter from H (inverse) fused.
 #pragma once
+#include <cstdlib>
 #include "bse_internal.h"
 #include "fft_codelets.cuh"
 
@@ -42,6 +43,7 @@ struct Geo {
     static constexpr int R2p = R2 + 1;
     static constexpr int LD = R1 * R2p + ((R2 % 8) ? ((R2 - R1 * R2p) % 8 + 8) % 8 : 0);   // plane line stride (complex)
     static constexpr int LDS = (R1 * R2p) | 1;                                            // stick line stride
+    static constexpr int LDC = (R1 * R2p) | 1;                                            // compact column stride
     static constexpr int TS = 32;                                                          // sticks per CTA
     static __host__ __device__ constexpr int natslot(int e) { return (e / R2) * R2p + e % R2; }
     static __host__ __device__ constexpr int fwdslot(int k) { return (k % R1) * R2p + k / R1; }
@@ -275,6 +277,112 @@ inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// inverse plane pass, COMPACT form for large planes.  The full-plane kernel above keeps n/2 lines of n complex in shared
+// memory (n^2 * 8 B: 115 KB at n = 120, 166 KB at 144), so one CTA per SM and every global phase exposed.  Only the W = R+1
+// columns m3 <= R carry data until the rows pass expands them, so this form keeps the columns compact, Cc[W][LDC], runs the
+// two column passes there, and expands LC lines at a time through a small line buffer Wk[LC][LD] (rows pass 1 with the
+// two-row tangle fused into its load, rows pass 2 straight to global).  82 + 25 KB at n = 120: two CTAs per SM.
+// dynamic smem: Cc[W * LDC] | Wk[LC * LD] | tables (tw, soff, wmax, wmin)
+template <int R1, int R2>
+__global__ void __launch_bounds__(256)
+inv_plane_compact_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out, int LC) {
+    using G = Geo<R1, R2>;
+    constexpr int n = G::n, LD = G::LD, R2p = G::R2p, LDC = G::LDC;
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int R = P.R, W = P.W;
+    double2 *Cc = reinterpret_cast<double2 *>(smem);
+    double2 *Wk = Cc + (size_t)W * LDC;
+    double2 *tw = Wk + (size_t)LC * LD;
+    int *soff = reinterpret_cast<int *>(tw + n);
+    int *wmax = soff + n, *wmin = wmax + n;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        tw[i] = P.tw[i]; soff[i] = P.soff[i]; wmax[i] = P.wmax[i]; wmin[i] = P.wmin[i];
+    }
+    const int i1 = blockIdx.x;
+    const long long p = blockIdx.y;
+    const double2 *z = Z + (p * n + i1) * (long long)P.NS;
+    __syncthreads();
+    // I1 (columns pass 1 from the sticks): column m3 lives at Cc[m3 * LDC + natslot(i2 index)]
+    for (int task = threadIdx.x; task < W * R2; task += blockDim.x) {
+        const int j = task / W, m3 = task - j * W;
+        double2 x[R1];
+#pragma unroll
+        for (int q = 0; q < R1; ++q) {
+            const int t2 = j + q * R2;
+            double2 v = make_double2(0.0, 0.0);
+            if (m3 <= wmax[t2]) {
+                if (m3 >= wmin[t2]) v = z[soff[t2] + m3];
+                else { v = z[soff[n - t2]]; v.y = -v.y; }
+            }
+            x[q] = v;
+        }
+        Dft<R1, +1>::run(x);
+        twiddle_powers<R1>(x, cconj(tw[j]));
+#pragma unroll
+        for (int q = 0; q < R1; ++q) Cc[m3 * LDC + q * R2p + j] = x[q];
+    }
+    __syncthreads();
+    // I2 (columns pass 2, in place): slot blk * R2p + k2 then holds row blk + R1 k2 of column m3
+    for (int task = threadIdx.x; task < W * R1; task += blockDim.x) {
+        const int blk = task / W, m3 = task - blk * W;
+        double2 *c = Cc + m3 * LDC + blk * R2p;
+        double2 x[R2];
+#pragma unroll
+        for (int q = 0; q < R2; ++q) x[q] = c[q];
+        Dft<R2, +1>::run(x);
+#pragma unroll
+        for (int q = 0; q < R2; ++q) c[q] = x[q];
+    }
+    __syncthreads();
+    double *o = out + p * N + (long long)i1 * n * n;
+    for (int l0 = 0; l0 < n / 2; l0 += LC) {
+        const int nl = min(LC, n / 2 - l0);
+        // I3 (rows pass 1): line l packs the rows at column places 2l, 2l+1:  Z_l[k] = A[k] + i B[k],
+        // Z_l[n-k] = conj(A[k]) + i conj(B[k]); everything outside |m3| <= R is zero
+        for (int task = threadIdx.x; task < nl * R2; task += blockDim.x) {
+            const int ll = task / R2, j = task - ll * R2;
+            const int l = l0 + ll;
+            const int sa = G::natslot(2 * l), sb = G::natslot(2 * l + 1);
+            double2 x[R1];
+#pragma unroll
+            for (int q = 0; q < R1; ++q) {
+                const int e = j + q * R2;
+                double2 v = make_double2(0.0, 0.0);
+                if (e <= R) {
+                    const double2 a = Cc[e * LDC + sa], b = Cc[e * LDC + sb];
+                    v = e ? make_double2(a.x - b.y, a.y + b.x) : make_double2(a.x, b.x);
+                } else if (e >= n - R) {
+                    const double2 a = Cc[(n - e) * LDC + sa], b = Cc[(n - e) * LDC + sb];
+                    v = make_double2(a.x + b.y, b.x - a.y);
+                }
+                x[q] = v;
+            }
+            Dft<R1, +1>::run(x);
+            twiddle_powers<R1>(x, cconj(tw[j]));
+#pragma unroll
+            for (int q = 0; q < R1; ++q) Wk[ll * LD + q * R2p + j] = x[q];
+        }
+        __syncthreads();
+        // I4 (rows pass 2 to global): place p holds row p / R2 + R1 (p % R2)
+        for (int task = threadIdx.x; task < nl * R1; task += blockDim.x) {
+            const int ll = task / R1, blk = task - ll * R1;
+            const int l = l0 + ll;
+            const double2 *c = Wk + ll * LD + blk * R2p;
+            double2 x[R2];
+#pragma unroll
+            for (int q = 0; q < R2; ++q) x[q] = c[q];
+            Dft<R2, +1>::run(x);
+            const int pa = 2 * l, pb = 2 * l + 1;
+            double *oa = o + (pa / R2 + R1 * (pa % R2)) * n + blk;
+            double *ob = o + (pb / R2 + R1 * (pb % R2)) * n + blk;
+#pragma unroll
+            for (int k2 = 0; k2 < R2; ++k2) { oa[R1 * k2] = x[k2].x; ob[R1 * k2] = x[k2].y; }
+        }
+        __syncthreads();
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // stick passes.  grid = (ceil(NS/TS), count), 256 threads.  smem: C[TS*LDS]
 template <int R1, int R2>
 __global__ void __launch_bounds__(256)
@@ -408,6 +516,29 @@ struct Launch {
         return BSE_OK;
     }
     static int inv_plane(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s) {
+        // large planes (one full-plane CTA per SM): the compact form, if two of its CTAs fit an SM
+        static const int force = std::getenv("BSE_COMPACT_INV") ? std::atoi(std::getenv("BSE_COMPACT_INV")) : -1;
+        const int tables = G::n * 16 + 3 * G::n * 4;
+        const int half = (232448 - 2 * 1024) / 2;
+        int LC = (half - P.W * G::LDC * 16 - tables) / (G::LD * 16);
+        if (LC > G::n / 2) LC = G::n / 2;
+        const bool fits = LC >= 4;
+        const bool use = force >= 0 ? (force != 0 && fits) : (G::smem_ctas == 1 && fits);
+        if (use) {
+            const int smem_c = (P.W * G::LDC + LC * G::LD) * 16 + tables;
+            int rc = set_smem((const void *)inv_plane_compact_kernel<R1, R2>, smem_c, true);
+            if (rc) return rc;
+            int threads = ((LC * R2 + 31) / 32) * 32;
+            if (threads > 256) threads = 256;
+            if (threads < 64) threads = 64;
+            for (int c0 = 0; c0 < count; c0 += 65535) {
+                const int c = count - c0 < 65535 ? count - c0 : 65535;
+                inv_plane_compact_kernel<R1, R2><<<dim3(G::n, c), threads, smem_c, s>>>(
+                    P, Z + (long long)c0 * G::n * P.NS, N, out + (long long)c0 * N, LC);
+            }
+            BSE_CUDA(cudaGetLastError());
+            return BSE_OK;
+        }
         int rc = set_smem((const void *)inv_plane_kernel<R1, R2>, G::plane_smem, true);
         if (rc) return rc;
         const int threads = G::plane_thr;
