@@ -120,7 +120,9 @@ int bse_get_tau(bse_handle *h, long long first, long long count, double *dst, un
 /* ---- measurement helpers ---- */
 /* Environment (test hooks, read when the apply plans its memory; they only ever lower a limit): BSE_MAX_GROUP caps the number
  * of trial blocks processed together in the PW layout, BSE_MAX_BATCH caps the pairs of one row batch, so that small cases
- * exercise the multi-group / multi-batch paths of the large configurations. */
+ * exercise the multi-group / multi-batch paths of the large configurations.  BSE_COMPACT_INV = k forces the compact
+ * inverse plane kernel (sized for k CTAs per SM; 0 = never) at every grid size instead of only where the full-plane kernel
+ * leaves one CTA per SM. */
 /* Per-stage device time (CUDA events on the library's stream).  enable != 0 switches recording on (adds a
  * host sync per call).  Stage indices: BSE_ST_*; ms and launches are arrays of BSE_ST_COUNT, accumulated since
  * the last bse_profile_reset. */

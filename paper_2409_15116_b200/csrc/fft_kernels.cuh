@@ -517,10 +517,12 @@ struct Launch {
     }
     static int inv_plane(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s) {
         // large planes (one full-plane CTA per SM): the compact form, if two of its CTAs fit an SM
+        // BSE_COMPACT_INV = k (test / tuning hook): force the compact form sized for k CTAs per SM (0: never)
         static const int force = std::getenv("BSE_COMPACT_INV") ? std::atoi(std::getenv("BSE_COMPACT_INV")) : -1;
         const int tables = G::n * 16 + 3 * G::n * 4;
-        const int half = (232448 - 2 * 1024) / 2;
-        int LC = (half - P.W * G::LDC * 16 - tables) / (G::LD * 16);
+        const int per_sm = force > 1 ? force : 2;
+        const int share = (232448 - per_sm * 1024) / per_sm;
+        int LC = (share - P.W * G::LDC * 16 - tables) / (G::LD * 16);
         if (LC > G::n / 2) LC = G::n / 2;
         const bool fits = LC >= 4;
         const bool use = force >= 0 ? (force != 0 && fits) : (G::smem_ctas == 1 && fits);

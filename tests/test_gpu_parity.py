@@ -461,3 +461,13 @@ def test_block_count_grows_and_stream_real_batches(monkeypatch):
         g.close()
     monkeypatch.setenv("BSE_MAX_BATCH", "5")
     _check_full(w, bse.BSE_TAU_STREAM, check_g=True)
+
+
+def test_compact_inverse_plane_kernel_small_grids(monkeypatch):
+    """The compact inverse plane kernel (used by default only at n = 120, 144) forced on small grids: radices 4x6, 5x4, 5x6."""
+    monkeypatch.setenv("BSE_COMPACT_INV", "2")
+    for n, L, ecut, Nv, Npdep, B in ((24, 10.0, 8.0, 8, 16, 2), (20, 12.0, 4.0, 6, 9, 1), (30, 14.0, 5.0, 4, 16, 2)):
+        cfg = wl.Config("cmp", L, n, Nv, Npdep, ecut, 1.3, 0.8, 3.0, 0.0, B, "random", seed=300 + n)
+        w = wl.make(cfg=cfg)
+        _check_full(w)
+        _check_pw(w, _bse().BSE_TAU_PW)
