@@ -518,7 +518,8 @@ struct Launch {
     static int inv_plane(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s) {
         // large planes (one full-plane CTA per SM): the compact form, if two of its CTAs fit an SM
         // BSE_COMPACT_INV = k (test / tuning hook): force the compact form sized for k CTAs per SM (0: never)
-        static const int force = std::getenv("BSE_COMPACT_INV") ? std::atoi(std::getenv("BSE_COMPACT_INV")) : -1;
+        const char *env = std::getenv("BSE_COMPACT_INV");
+        const int force = env ? std::atoi(env) : -1;
         const int tables = G::n * 16 + 3 * G::n * 4;
         const int per_sm = force > 1 ? force : 2;
         const int share = (232448 - per_sm * 1024) / per_sm;
