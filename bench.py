@@ -45,9 +45,9 @@ def max_over_ranks(values, dist=None, device=None):
 
 # DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the kernel behind each stage at cfg2, from the
 # committed ncu --set full capture profiles/r01c_final.md (constants of that capture, not measured by this run).
-NCU_TRAFFIC_CFG2 = {"pc_update": 1159e6, "pc_overlap": 675e6, "k1x_accumulate": 1540e6, "fwd_plane": 314e6,
-                    "inv_plane": 523e6, "fwd_stick": 101e6, "inv_stick": 64e6, "pdep_project": 67e6,
-                    "pdep_backproject": 67e6, "screen_syrk": 138e6}
+NCU_TRAFFIC_CFG2 = {"pc_update": 1159e6, "k1x_accumulate": 1540e6,
+                    "inv_plane": 523e6, "inv_stick": 64e6, "pdep_project": 67e6, "pdep_backproject": 67e6,
+                    "screen_syrk": 138e6}
 
 
 def load_peaks():

@@ -278,6 +278,66 @@ int ensure_u_pw(bse_handle *h) {
     return bse_launch_weight_pw(h->uG, h->uGw, pl.npw_h, h->Nv, h->Omega, h->stream);
 }
 
+// Is every orbital band-limited to S?  Compares dV sum_r u_v^2 with Omega sum_S |u_v(G)|^2 (Parseval holds only then).
+// Decided once per set of inputs; costs two small Gram products.  Plane-wave orbitals are, by construction.
+int check_band_limited(bse_handle *h) {
+    if (h->u_bl >= 0) return BSE_OK;
+    int rc;
+    if ((rc = ensure_u_pw(h))) return rc;
+    const long long Nv = h->Nv, K2 = 2 * h->fft.npw_h, lds = ldS(h);
+    if ((rc = ensure_sov(h, 2 * Nv))) return rc;
+    double *Gr = h->Sov, *Gg = h->Sov + Nv * lds;
+    if ((rc = bse_gemm_dot(h->u, h->N, h->u, h->N, (int)Nv, (int)Nv, h->N, false, false, h->part, h->part_bytes, Gr, lds,
+                           h->dV, nullptr, h->stream))) return rc;
+    if ((rc = bse_gemm_dot((const double *)h->uG, K2, (const double *)h->uGw, K2, (int)Nv, (int)Nv, K2, false, false, h->part,
+                           h->part_bytes, Gg, lds, 1.0, nullptr, h->stream))) return rc;
+    std::vector<double> host((size_t)2 * Nv * lds);
+    BSE_CUDA(cudaMemcpyAsync(host.data(), h->Sov, host.size() * 8, cudaMemcpyDeviceToHost, h->stream));
+    BSE_CUDA(cudaStreamSynchronize(h->stream));
+    bool ok = true;
+    for (long long v = 0; v < Nv; ++v) {
+        const double nr = host[v * lds + v], ng = host[(Nv + v) * lds + v];
+        if (!(std::fabs(nr - ng) <= 1e-12 * std::fabs(nr))) ok = false;
+    }
+    h->u_bl = ok ? 1 : 0;
+    return BSE_OK;
+}
+
+// P_c on REAL-layout rows when u is band-limited to S: <u_w|x> = Omega sum_S conj(u_w(G)) x(G) needs x only on S, so the
+// overlaps come from one pruned forward transform per row and a GEMM over 2 N_pw_h instead of N (16x fewer flops);
+// the update x -= S u stays in real space (no truncation of x: S15).
+int p_c_rows_real(bse_handle *h, double *x, long long rows) {
+    int rc;
+    if ((rc = check_band_limited(h))) return rc;
+    if (h->u_bl != 1) return p_c_rows(h, x, rows, h->N, h->u, h->u, h->dV);
+    const FftPlan &pl = h->fft;
+    const long long npw_h = pl.npw_h, K2 = 2 * npw_h, lds = ldS(h);
+    if (h->accG_rows < rows) {
+        cudaFree(h->accG);
+        h->accG = nullptr; h->accG_rows = 0;
+        BSE_CUDA(cudaMalloc(&h->accG, (size_t)rows * npw_h * 16));
+        h->accG_rows = rows;
+    }
+    for (long long r0 = 0; r0 < rows; r0 += h->Pb) {
+        const int cnt = (int)std::min<long long>(h->Pb, rows - r0);
+        if ((rc = st_fwd_plane(h, pl, x, nullptr, r0, cnt))) return rc;
+        if ((rc = st_fwd_stick(h, pl, cnt, h->accG + r0 * npw_h, pl.inv2n))) return rc;
+    }
+    if ((rc = ensure_sov(h, rows))) return rc;
+    long long mc = rows;
+    const long long per_row = (long long)h->Nv * 8 * 2;
+    if (rows * per_row > (long long)h->part_bytes) mc = std::max<long long>(64, (long long)(h->part_bytes / per_row) / 64 * 64);
+    for (long long r0 = 0; r0 < rows; r0 += mc) {
+        const int m = (int)std::min(mc, rows - r0);
+        if ((rc = st_gemm_dot(h, BSE_ST_PC_OVERLAP, (const double *)(h->accG + r0 * npw_h), K2, (const double *)h->uGw, K2, m,
+                              h->Nv, K2, false, h->Sov + r0 * lds, lds, 1.0, nullptr))) return rc;
+        if ((rc = st_gemm_nn(h, BSE_ST_PC_UPDATE, h->Sov + r0 * lds, lds, h->u, h->N, m, h->N, h->Nv, EPI_SUB, nullptr, nullptr,
+                             x + r0 * h->N, h->N))) return rc;
+    }
+    return BSE_OK;
+}
+
+
 // pair-batch workspaces Z, X, T, Dm for `pb` fields (tau_batch follows lazily); called at create and again after the
 // pair list is known if one row of the adjacency has more entries than the batch holds
 int alloc_batch_ws(bse_handle *h, long long pb) {
@@ -765,7 +825,7 @@ extern "C" int bse_destroy(bse_handle *h) {
     cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);
     cudaFree(h->part); cudaFree(h->Sov); cudaFree(h->tau_batch); cudaFree(h->a_dev); cudaFree(h->out_dev);
     cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->a_r); cudaFree(h->acc_r);
-    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist); cudaFree(h->k1e_ws); cudaFree(h->u_a); cudaFree(h->Ut);
+    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist); cudaFree(h->k1e_ws); cudaFree(h->u_a); cudaFree(h->Ut); cudaFree(h->accG);
     for (cudaEvent_t e : h->ev_pipe) cudaEventDestroy(e);
     if (h->s_in) cudaStreamDestroy(h->s_in);
     if (h->s_out) cudaStreamDestroy(h->s_out);
@@ -805,7 +865,7 @@ extern "C" int bse_apply_k1x(bse_handle *h, const double *a, double *out, int B)
     if ((rc = plan_apply_memory(h, B))) return rc;
     if (h->flags & BSE_VEC_PW) return apply_pw(h, (const double2 *)a, (double2 *)out, B);
     if ((rc = accumulate_all(h, a, B, out, nullptr))) return rc;
-    return p_c_rows(h, out, (long long)B * h->Nv, h->N, h->u, h->u, h->dV);
+    return p_c_rows_real(h, out, (long long)B * h->Nv);
 }
 
 extern "C" int bse_apply_k1x_host(bse_handle *h, const double *a_host, double *out_host, int B) {
@@ -865,7 +925,7 @@ extern "C" int bse_set_inputs_host(bse_handle *h, const double *u_host, const do
     if (u_host) BSE_CUDA(cudaMemcpyAsync(h->u_owned, u_host, (size_t)h->Nv * h->N * 8, cudaMemcpyHostToDevice, h->stream));
     if (phi_host) BSE_CUDA(cudaMemcpyAsync(h->phi_owned, phi_host, (size_t)h->Npdep * h->fft.npw_h * 16, cudaMemcpyHostToDevice, h->stream));
     h->built = false;
-    if (u_host) { cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->u_a); h->uG = h->uGw = nullptr; h->u_a = nullptr; }
+    if (u_host) { cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->u_a); h->uG = h->uGw = nullptr; h->u_a = nullptr; h->u_bl = -1; }
     return BSE_OK;
 }
 
@@ -884,7 +944,7 @@ extern "C" int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B)
         if ((rc = hartree_in_place(h, pl, h->k1e_ws, B))) return rc;
         { StageTimer t(h, BSE_ST_K1E_PRODUCT, 2.0 * B * Nv * (double)pl.N, N8 * (B * Nv + Nv + B));
           if ((rc = bse_launch_k1e_product(h->u, h->k1e_ws, out, 0, h->Nv, Nv, pl.N, B, h->stream))) return rc; }
-        return p_c_rows(h, out, (long long)B * Nv, pl.N, h->u, h->u, h->dV);
+        return p_c_rows_real(h, out, (long long)B * Nv);
     }
     // PW layout: one block at a time on the apply grid: a(G) -> a(r), density, Hartree, products in row chunks -> out(G)
     const FftPlan &pl = *h->ap;
@@ -963,7 +1023,7 @@ extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, 
     rc = accumulate_all(h, a, B, out, nullptr);
     h->mix_on = false;
     if (rc) return rc;
-    return p_c_rows(h, out, (long long)B * h->Nv, h->N, h->u, h->u, h->dV);
+    return p_c_rows_real(h, out, (long long)B * h->Nv);
 }
 
 // KS <-> localised representation of the trial blocks (eq. 12): y[b] = U x[b] or U^T x[b]

@@ -96,6 +96,9 @@ struct bse_handle {
     int mix_B = 0;
     const double *mix_u = nullptr;                 // orbitals on the grid the apply runs on; nullptr: made on the fly from uG
     const double *mix_vH = nullptr;                // [nb][N] Hartree potentials of the blocks being accumulated
+    int u_bl = -1;                                 // 1: every orbital is band-limited to S (checked once), 0: not, -1: unknown
+    double2 *accG = nullptr;                       // [rows][npw_h] rows on H for the P_c overlaps of the REAL layout
+    long long accG_rows = 0;
     double *Ut = nullptr;                          // [Nv][ldS] transposed copy of the rotation matrix (bse_rotate)
     double *u_a = nullptr;                         // [Nv][Na] orbitals on the apply grid (PW layout with a coarser grid)
     double *a_dev = nullptr, *out_dev = nullptr;   // staging for the host-pointer entry point

@@ -471,3 +471,18 @@ def test_compact_inverse_plane_kernel_small_grids(monkeypatch):
         w = wl.make(cfg=cfg)
         _check_full(w)
         _check_pw(w, _bse().BSE_TAU_PW)
+
+
+def test_real_layout_with_orbitals_that_are_not_band_limited():
+    """The REAL layout takes any u.  With band-limited u (every generated workload) the P_c overlaps go through the pruned FFT;
+    with u that has components outside S the library must notice (Parseval check) and keep the real-space overlaps."""
+    bse = _bse()
+    cfg = wl.Config("nbl", 10.0, 24, 6, 12, 8.0, 1.2, 0.8, 3.0, 0.01, 2, "random", seed=81)
+    w = wl.make(cfg=cfg)
+    rng = np.random.default_rng(3)
+    u = w.u + 0.02 * rng.normal(size=w.u.shape) * np.abs(w.u).max()                             # grid noise: not in S
+    dV = w.L ** 3 / w.N
+    ev, V = np.linalg.eigh(dV * (u @ u.T))
+    w.u = np.ascontiguousarray(((V / np.sqrt(ev)) @ V.T) @ u)                                    # orthonormal again
+    _check_full(w, bse.BSE_TAU_REAL, check_g=True)
+    _check_full(w, bse.BSE_TAU_PW, check_g=False)
