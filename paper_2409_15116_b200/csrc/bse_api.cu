@@ -305,7 +305,8 @@ int check_band_limited(bse_handle *h) {
 
 // P_c on REAL-layout rows when u is band-limited to S: <u_w|x> = Omega sum_S conj(u_w(G)) x(G) needs x only on S, so the
 // overlaps come from one pruned forward transform per row and a GEMM over 2 N_pw_h instead of N (16x fewer flops);
-// the update x -= S u stays in real space (no truncation of x: S15).
+// and so does the correction: x -= inverse transform of (S u)(G), fused into the inverse plane pass (x itself is not
+// truncated: S15).
 int p_c_rows_real(bse_handle *h, double *x, long long rows) {
     int rc;
     if ((rc = check_band_limited(h))) return rc;
@@ -327,12 +328,27 @@ int p_c_rows_real(bse_handle *h, double *x, long long rows) {
     long long mc = rows;
     const long long per_row = (long long)h->Nv * 8 * 2;
     if (rows * per_row > (long long)h->part_bytes) mc = std::max<long long>(64, (long long)(h->part_bytes / per_row) / 64 * 64);
+    const Model m(pl);
     for (long long r0 = 0; r0 < rows; r0 += mc) {
-        const int m = (int)std::min(mc, rows - r0);
-        if ((rc = st_gemm_dot(h, BSE_ST_PC_OVERLAP, (const double *)(h->accG + r0 * npw_h), K2, (const double *)h->uGw, K2, m,
-                              h->Nv, K2, false, h->Sov + r0 * lds, lds, 1.0, nullptr))) return rc;
-        if ((rc = st_gemm_nn(h, BSE_ST_PC_UPDATE, h->Sov + r0 * lds, lds, h->u, h->N, m, h->N, h->Nv, EPI_SUB, nullptr, nullptr,
-                             x + r0 * h->N, h->N))) return rc;
+        const int mm = (int)std::min(mc, rows - r0);
+        double *ag = (double *)(h->accG + r0 * npw_h);
+        if ((rc = st_gemm_dot(h, BSE_ST_PC_OVERLAP, ag, K2, (const double *)h->uGw, K2, mm, h->Nv, K2, false,
+                              h->Sov + r0 * lds, lds, 1.0, nullptr))) return rc;
+        if (h->Nv < 160) {       // few orbitals: the real-space DGEMM update (2 Nv N flops per row) beats a transform per row
+            if ((rc = st_gemm_nn(h, BSE_ST_PC_UPDATE, h->Sov + r0 * lds, lds, h->u, h->N, mm, h->N, h->Nv, EPI_SUB, nullptr,
+                                 nullptr, x + r0 * h->N, h->N))) return rc;
+            continue;
+        }
+        // the correction sum_w S_w u_w is band-limited too: form it on H (small NN GEMM over the rows' coefficients, which
+        // are no longer needed) and subtract its inverse transform in the plane pass's store
+        if ((rc = st_gemm_nn(h, BSE_ST_PC_UPDATE, h->Sov + r0 * lds, lds, (const double *)h->uG, K2, mm, K2, h->Nv, EPI_STORE,
+                             nullptr, nullptr, ag, K2))) return rc;
+        for (long long c0 = 0; c0 < mm; c0 += h->Pb) {
+            const int cnt = (int)std::min<long long>(h->Pb, mm - c0);
+            if ((rc = st_inv_stick(h, pl, h->accG + (r0 + c0) * npw_h, cnt))) return rc;
+            StageTimer t(h, BSE_ST_PC_UPDATE, cnt * m.plane_flops, cnt * (2.0 * m.N8 + m.z));
+            if ((rc = bse_launch_inv_plane(pl, h->Z, cnt, pl.N, x + (r0 + c0) * h->N, h->stream, true))) return rc;
+        }
     }
     return BSE_OK;
 }

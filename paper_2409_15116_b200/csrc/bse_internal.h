@@ -134,7 +134,9 @@ int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2
 // gather != nullptr: field p is read from T + gather[g0 + p] * npw_h (pair indices of a row batch)
 int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2 *Z, cudaStream_t s,
                          const int *gather = nullptr, int g0 = 0);
-int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long long N, double *out, cudaStream_t s);
+// subtract: out <- out - transform instead of out <- transform (P_c update of the REAL layout)
+int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long long N, double *out, cudaStream_t s,
+                         bool subtract = false);
 
 // gemm_dmma.cu
 enum { EPI_PARTIAL = 0, EPI_TAU = 1, EPI_SUB = 2, EPI_STORE = 3 };

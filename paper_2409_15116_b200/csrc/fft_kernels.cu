@@ -44,9 +44,10 @@ int bse_launch_fwd_plane(const FftPlan &pl, const double *fields, const int2 *pa
     if (count <= 0) return BSE_OK;
     return ((const FftOps *)pl.ops)->fwd_plane(to_dev(pl), fields, pairs, p0, count, N, Z, s);
 }
-int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long long N, double *out, cudaStream_t s) {
+int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long long N, double *out, cudaStream_t s,
+                         bool subtract) {
     if (count <= 0) return BSE_OK;
-    return ((const FftOps *)pl.ops)->inv_plane(to_dev(pl), Z, count, N, out, s);
+    return ((const FftOps *)pl.ops)->inv_plane(to_dev(pl), Z, count, N, out, s, subtract ? 1 : 0);
 }
 int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2 *X, const double *scale,
                          cudaStream_t s, const int *scatter) {

@@ -187,7 +187,7 @@ fwd_plane_kernel(PlanDev P, const double *__restrict__ fields, const int2 *__res
 // inverse plane pass.  grid = (n planes, count).  Z[p][i1][NS] -> out[p][N] real.
 template <int R1, int R2>
 __global__ void __launch_bounds__(Geo<R1, R2>::plane_thr, Geo<R1, R2>::plane_minb)
-inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out) {
+inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out, int sub) {
     using G = Geo<R1, R2>;
     constexpr int n = G::n, LD = G::LD, R2p = G::R2p;
     extern __shared__ __align__(16) unsigned char smem[];
@@ -272,7 +272,10 @@ inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *
         double *oa = o + (pa / R2 + R1 * (pa % R2)) * n + blk;
         double *ob = o + (pb / R2 + R1 * (pb % R2)) * n + blk;
 #pragma unroll
-        for (int k2 = 0; k2 < R2; ++k2) { oa[R1 * k2] = x[k2].x; ob[R1 * k2] = x[k2].y; }
+        for (int k2 = 0; k2 < R2; ++k2) {
+            if (sub) { oa[R1 * k2] -= x[k2].x; ob[R1 * k2] -= x[k2].y; }          // out <- out - transform (P_c update)
+            else { oa[R1 * k2] = x[k2].x; ob[R1 * k2] = x[k2].y; }
+        }
     }
 }
 
@@ -285,7 +288,8 @@ inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *
 // dynamic smem: Cc[W * LDC] | Wk[LC * LD] | tables (tw, soff, wmax, wmin)
 template <int R1, int R2>
 __global__ void __launch_bounds__(256)
-inv_plane_compact_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out, int LC) {
+inv_plane_compact_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out, int LC,
+                         int sub) {
     using G = Geo<R1, R2>;
     constexpr int n = G::n, LD = G::LD, R2p = G::R2p, LDC = G::LDC;
     extern __shared__ __align__(16) unsigned char smem[];
@@ -376,7 +380,10 @@ inv_plane_compact_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, 
             double *oa = o + (pa / R2 + R1 * (pa % R2)) * n + blk;
             double *ob = o + (pb / R2 + R1 * (pb % R2)) * n + blk;
 #pragma unroll
-            for (int k2 = 0; k2 < R2; ++k2) { oa[R1 * k2] = x[k2].x; ob[R1 * k2] = x[k2].y; }
+            for (int k2 = 0; k2 < R2; ++k2) {
+                if (sub) { oa[R1 * k2] -= x[k2].x; ob[R1 * k2] -= x[k2].y; }      // out <- out - transform (P_c update)
+                else { oa[R1 * k2] = x[k2].x; ob[R1 * k2] = x[k2].y; }
+            }
         }
         __syncthreads();
     }
@@ -482,7 +489,7 @@ inv_stick_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, doub
 struct FftOps {
     int n, R1, R2, plane_smem;
     int (*fwd_plane)(const PlanDev &, const double *, const int2 *, long long, int, long long, double2 *, cudaStream_t);
-    int (*inv_plane)(const PlanDev &, const double2 *, int, long long, double *, cudaStream_t);
+    int (*inv_plane)(const PlanDev &, const double2 *, int, long long, double *, cudaStream_t, int);
     int (*fwd_stick)(const PlanDev &, const double2 *, int, double2 *, long long, const double *, cudaStream_t, const int *);
     int (*inv_stick)(const PlanDev &, const double2 *, int, long long, double2 *, cudaStream_t, const int *, int);
 };
@@ -515,7 +522,7 @@ struct Launch {
         BSE_CUDA(cudaGetLastError());
         return BSE_OK;
     }
-    static int inv_plane(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s) {
+    static int inv_plane(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s, int sub) {
         // large planes (one full-plane CTA per SM): the compact form, if two of its CTAs fit an SM
         // BSE_COMPACT_INV = k (test / tuning hook): force the compact form sized for k CTAs per SM (0: never)
         const char *env = std::getenv("BSE_COMPACT_INV");
@@ -537,7 +544,7 @@ struct Launch {
             for (int c0 = 0; c0 < count; c0 += 65535) {
                 const int c = count - c0 < 65535 ? count - c0 : 65535;
                 inv_plane_compact_kernel<R1, R2><<<dim3(G::n, c), threads, smem_c, s>>>(
-                    P, Z + (long long)c0 * G::n * P.NS, N, out + (long long)c0 * N, LC);
+                    P, Z + (long long)c0 * G::n * P.NS, N, out + (long long)c0 * N, LC, sub);
             }
             BSE_CUDA(cudaGetLastError());
             return BSE_OK;
@@ -548,7 +555,7 @@ struct Launch {
         for (int c0 = 0; c0 < count; c0 += 65535) {
             const int c = count - c0 < 65535 ? count - c0 : 65535;
             inv_plane_kernel<R1, R2><<<dim3(G::n, c), threads, G::plane_smem, s>>>(
-                P, Z + (long long)c0 * G::n * P.NS, N, out + (long long)c0 * N);
+                P, Z + (long long)c0 * G::n * P.NS, N, out + (long long)c0 * N, sub);
         }
         BSE_CUDA(cudaGetLastError());
         return BSE_OK;
