@@ -264,11 +264,14 @@ int p_c_rows(bse_handle *h, double *x, long long rows, long long K, const double
 // uGw = Omega * wt(G) * uG with wt = 2 (G != 0), (1, 0) on (re, im) of G = 0, so that the half-sphere real dot product
 // sum_k uGw[w][k] x[k] equals <u_w|x> = Omega sum_{G in S} conj(u_w(G)) x(G)   (S14).
 int ensure_u_pw(bse_handle *h) {
-    if (h->uG) return BSE_OK;
+    if (h->uG && h->uG_valid) return BSE_OK;
     const FftPlan &pl = h->fft;
     const size_t bytes = (size_t)h->Nv * pl.npw_h * 16;
-    BSE_CUDA(cudaMalloc(&h->uG, bytes));
-    BSE_CUDA(cudaMalloc(&h->uGw, bytes));
+    if (!h->uG) {                             // kept across bse_set_inputs_host: new orbitals are transformed into the same buffers
+        BSE_CUDA(cudaMalloc(&h->uG, bytes));
+        BSE_CUDA(cudaMalloc(&h->uGw, bytes));
+    }
+    h->uG_valid = true;
     int rc;
     for (long long v0 = 0; v0 < h->Nv; v0 += h->Pb) {
         const int cnt = (int)std::min<long long>(h->Pb, h->Nv - v0);
@@ -587,11 +590,11 @@ int hartree_in_place(bse_handle *h, const FftPlan &pl, double *buf, int nfields)
 
 // orbitals on the apply grid of the PW layout: u_a = inverse transform of u(G) on n_a (u is band-limited to S)
 int ensure_u_apply(bse_handle *h) {
-    if (h->ap == &h->fft || h->u_a) return BSE_OK;
+    if (h->ap == &h->fft || (h->u_a && h->u_a_valid)) return BSE_OK;
     const FftPlan &pl = *h->ap;
     int rc;
     if ((rc = ensure_u_pw(h))) return rc;
-    if (cudaMalloc(&h->u_a, (size_t)h->Nv * pl.N * 8) != cudaSuccess) {
+    if (!h->u_a && cudaMalloc(&h->u_a, (size_t)h->Nv * pl.N * 8) != cudaSuccess) {
         // the K1x apply plan holds the free memory: drop it (the next K1x apply plans again, with u_a in place)
         (void)cudaGetLastError();
         h->u_a = nullptr;
@@ -601,6 +604,7 @@ int ensure_u_apply(bse_handle *h) {
         h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
         BSE_CUDA(cudaMalloc(&h->u_a, (size_t)h->Nv * pl.N * 8));
     }
+    h->u_a_valid = true;
     for (long long v0 = 0; v0 < h->Nv; v0 += h->Pb) {
         const int cnt = (int)std::min<long long>(h->Pb, h->Nv - v0);
         if ((rc = st_inv_stick(h, pl, h->uG + v0 * pl.npw_h, cnt))) return rc;
@@ -941,7 +945,7 @@ extern "C" int bse_set_inputs_host(bse_handle *h, const double *u_host, const do
     if (u_host) BSE_CUDA(cudaMemcpyAsync(h->u_owned, u_host, (size_t)h->Nv * h->N * 8, cudaMemcpyHostToDevice, h->stream));
     if (phi_host) BSE_CUDA(cudaMemcpyAsync(h->phi_owned, phi_host, (size_t)h->Npdep * h->fft.npw_h * 16, cudaMemcpyHostToDevice, h->stream));
     h->built = false;
-    if (u_host) { cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->u_a); h->uG = h->uGw = nullptr; h->u_a = nullptr; h->u_bl = -1; }
+    if (u_host) { h->uG_valid = false; h->u_a_valid = false; h->u_bl = -1; }     // derived copies are refilled in place, lazily
     return BSE_OK;
 }
 
@@ -1013,7 +1017,7 @@ extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, 
     if (fly && h->u_a) {                                        // a copy left by bse_apply_k1e: give its memory to the plan
         BSE_CUDA(cudaStreamSynchronize(h->stream));
         cudaFree(h->u_a);
-        h->u_a = nullptr;
+        h->u_a = nullptr; h->u_a_valid = false;
         h->plan_ok = false;
     }
     if ((rc = ensure_k1e_ws(h, (size_t)(B + (fly ? h->Pb : 0)) * h->ap->N * 8))) return rc;

@@ -96,6 +96,7 @@ struct bse_handle {
     int mix_B = 0;
     const double *mix_u = nullptr;                 // orbitals on the grid the apply runs on; nullptr: made on the fly from uG
     const double *mix_vH = nullptr;                // [nb][N] Hartree potentials of the blocks being accumulated
+    bool uG_valid = false, u_a_valid = false;      // uG / uGw / u_a hold the current orbitals (stale after bse_set_inputs_host)
     int u_bl = -1;                                 // 1: every orbital is band-limited to S (checked once), 0: not, -1: unknown
     double2 *accG = nullptr;                       // [rows][npw_h] rows on H for the P_c overlaps of the REAL layout
     long long accG_rows = 0;
