@@ -337,7 +337,7 @@ int p_c_rows_real(bse_handle *h, double *x, long long rows) {
         double *ag = (double *)(h->accG + r0 * npw_h);
         if ((rc = st_gemm_dot(h, BSE_ST_PC_OVERLAP, ag, K2, (const double *)h->uGw, K2, mm, h->Nv, K2, false,
                               h->Sov + r0 * lds, lds, 1.0, nullptr))) return rc;
-        if (h->Nv < 160) {       // few orbitals: the real-space DGEMM update (2 Nv N flops per row) beats a transform per row
+        if (h->Nv < 48) {        // few orbitals: the real-space DGEMM update (2 Nv N flops per row) beats a transform per row
             if ((rc = st_gemm_nn(h, BSE_ST_PC_UPDATE, h->Sov + r0 * lds, lds, h->u, h->N, mm, h->N, h->Nv, EPI_SUB, nullptr,
                                  nullptr, x + r0 * h->N, h->N))) return rc;
             continue;

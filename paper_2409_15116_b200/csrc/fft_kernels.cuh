@@ -185,9 +185,9 @@ fwd_plane_kernel(PlanDev P, const double *__restrict__ fields, const int2 *__res
 
 // ---------------------------------------------------------------------------------------------------------
 // inverse plane pass.  grid = (n planes, count).  Z[p][i1][NS] -> out[p][N] real.
-template <int R1, int R2>
+template <int R1, int R2, bool SUB>
 __global__ void __launch_bounds__(Geo<R1, R2>::plane_thr, Geo<R1, R2>::plane_minb)
-inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out, int sub) {
+inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out) {
     using G = Geo<R1, R2>;
     constexpr int n = G::n, LD = G::LD, R2p = G::R2p;
     extern __shared__ __align__(16) unsigned char smem[];
@@ -264,16 +264,21 @@ inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *
     for (int task = threadIdx.x; task < (n / 2) * R1; task += blockDim.x) {
         const int l = task / R1, blk = task - l * R1;
         const double2 *c = C + l * LD + blk * R2p;
+        const int pa = 2 * l, pb = 2 * l + 1;
+        double *oa = o + (pa / R2 + R1 * (pa % R2)) * n + blk;
+        double *ob = o + (pb / R2 + R1 * (pb % R2)) * n + blk;
+        double olda[SUB ? R2 : 1], oldb[SUB ? R2 : 1];
+        if (SUB) {                             // out <- out - transform (P_c update): the old values are fetched before the
+#pragma unroll                                 // butterfly so that their latency hides behind it
+            for (int k2 = 0; k2 < R2; ++k2) { olda[k2] = oa[R1 * k2]; oldb[k2] = ob[R1 * k2]; }
+        }
         double2 x[R2];
 #pragma unroll
         for (int q = 0; q < R2; ++q) x[q] = c[q];
         Dft<R2, +1>::run(x);
-        const int pa = 2 * l, pb = 2 * l + 1;
-        double *oa = o + (pa / R2 + R1 * (pa % R2)) * n + blk;
-        double *ob = o + (pb / R2 + R1 * (pb % R2)) * n + blk;
 #pragma unroll
         for (int k2 = 0; k2 < R2; ++k2) {
-            if (sub) { oa[R1 * k2] -= x[k2].x; ob[R1 * k2] -= x[k2].y; }          // out <- out - transform (P_c update)
+            if (SUB) { oa[R1 * k2] = olda[k2] - x[k2].x; ob[R1 * k2] = oldb[k2] - x[k2].y; }
             else { oa[R1 * k2] = x[k2].x; ob[R1 * k2] = x[k2].y; }
         }
     }
@@ -286,10 +291,9 @@ inv_plane_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *
 // two column passes there, and expands LC lines at a time through a small line buffer Wk[LC][LD] (rows pass 1 with the
 // two-row tangle fused into its load, rows pass 2 straight to global).  82 + 25 KB at n = 120: two CTAs per SM.
 // dynamic smem: Cc[W * LDC] | Wk[LC * LD] | tables (tw, soff, wmax, wmin)
-template <int R1, int R2>
+template <int R1, int R2, bool SUB>
 __global__ void __launch_bounds__(256)
-inv_plane_compact_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out, int LC,
-                         int sub) {
+inv_plane_compact_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, double *__restrict__ out, int LC) {
     using G = Geo<R1, R2>;
     constexpr int n = G::n, LD = G::LD, R2p = G::R2p, LDC = G::LDC;
     extern __shared__ __align__(16) unsigned char smem[];
@@ -372,16 +376,21 @@ inv_plane_compact_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, 
             const int ll = task / R1, blk = task - ll * R1;
             const int l = l0 + ll;
             const double2 *c = Wk + ll * LD + blk * R2p;
+            const int pa = 2 * l, pb = 2 * l + 1;
+            double *oa = o + (pa / R2 + R1 * (pa % R2)) * n + blk;
+            double *ob = o + (pb / R2 + R1 * (pb % R2)) * n + blk;
+            double olda[SUB ? R2 : 1], oldb[SUB ? R2 : 1];
+            if (SUB) {
+#pragma unroll
+                for (int k2 = 0; k2 < R2; ++k2) { olda[k2] = oa[R1 * k2]; oldb[k2] = ob[R1 * k2]; }
+            }
             double2 x[R2];
 #pragma unroll
             for (int q = 0; q < R2; ++q) x[q] = c[q];
             Dft<R2, +1>::run(x);
-            const int pa = 2 * l, pb = 2 * l + 1;
-            double *oa = o + (pa / R2 + R1 * (pa % R2)) * n + blk;
-            double *ob = o + (pb / R2 + R1 * (pb % R2)) * n + blk;
 #pragma unroll
             for (int k2 = 0; k2 < R2; ++k2) {
-                if (sub) { oa[R1 * k2] -= x[k2].x; ob[R1 * k2] -= x[k2].y; }      // out <- out - transform (P_c update)
+                if (SUB) { oa[R1 * k2] = olda[k2] - x[k2].x; ob[R1 * k2] = oldb[k2] - x[k2].y; }
                 else { oa[R1 * k2] = x[k2].x; ob[R1 * k2] = x[k2].y; }
             }
         }
@@ -536,26 +545,26 @@ struct Launch {
         const bool use = force >= 0 ? (force != 0 && fits) : (G::smem_ctas == 1 && fits);
         if (use) {
             const int smem_c = (P.W * G::LDC + LC * G::LD) * 16 + tables;
-            int rc = set_smem((const void *)inv_plane_compact_kernel<R1, R2>, smem_c, true);
+            auto kern = sub ? inv_plane_compact_kernel<R1, R2, true> : inv_plane_compact_kernel<R1, R2, false>;
+            int rc = set_smem((const void *)kern, smem_c, true);
             if (rc) return rc;
             int threads = ((LC * R2 + 31) / 32) * 32;
             if (threads > 256) threads = 256;
             if (threads < 64) threads = 64;
             for (int c0 = 0; c0 < count; c0 += 65535) {
                 const int c = count - c0 < 65535 ? count - c0 : 65535;
-                inv_plane_compact_kernel<R1, R2><<<dim3(G::n, c), threads, smem_c, s>>>(
-                    P, Z + (long long)c0 * G::n * P.NS, N, out + (long long)c0 * N, LC, sub);
+                kern<<<dim3(G::n, c), threads, smem_c, s>>>(P, Z + (long long)c0 * G::n * P.NS, N, out + (long long)c0 * N, LC);
             }
             BSE_CUDA(cudaGetLastError());
             return BSE_OK;
         }
-        int rc = set_smem((const void *)inv_plane_kernel<R1, R2>, G::plane_smem, true);
+        auto kern = sub ? inv_plane_kernel<R1, R2, true> : inv_plane_kernel<R1, R2, false>;
+        int rc = set_smem((const void *)kern, G::plane_smem, true);
         if (rc) return rc;
         const int threads = G::plane_thr;
         for (int c0 = 0; c0 < count; c0 += 65535) {
             const int c = count - c0 < 65535 ? count - c0 : 65535;
-            inv_plane_kernel<R1, R2><<<dim3(G::n, c), threads, G::plane_smem, s>>>(
-                P, Z + (long long)c0 * G::n * P.NS, N, out + (long long)c0 * N, sub);
+            kern<<<dim3(G::n, c), threads, G::plane_smem, s>>>(P, Z + (long long)c0 * G::n * P.NS, N, out + (long long)c0 * N);
         }
         BSE_CUDA(cudaGetLastError());
         return BSE_OK;
