@@ -43,11 +43,11 @@ def max_over_ranks(values, dist=None, device=None):
     return t.tolist()
 
 
-# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the kernel behind each stage at cfg2, from the
-# committed ncu --set full capture profiles/r01c_final.md (constants of that capture, not measured by this run).
-NCU_TRAFFIC_CFG2 = {"pc_update": 1159e6, "k1x_accumulate": 1540e6,
-                    "inv_plane": 523e6, "inv_stick": 64e6, "pdep_project": 67e6, "pdep_backproject": 67e6,
-                    "screen_syrk": 138e6}
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the kernel(s) behind each stage at cfg2, averaged over
+# the stage's launches in one step, from the committed ncu --set full capture profiles/r01d_final.md (constants of that
+# capture, not measured by this run).
+NCU_TRAFFIC_CFG2 = {"k1x_accumulate": 1540e6, "fwd_plane": 468e6, "inv_plane": 525e6, "pc_update": 562e6, "fwd_stick": 107e6,
+                    "inv_stick": 71e6, "pdep_project": 64e6, "pdep_backproject": 67e6, "screen_syrk": 138e6, "pc_overlap": 41e6}
 
 
 def load_peaks():
@@ -339,7 +339,7 @@ def main():
     roof["launches_per_step"] = n_launch_top
     roof["ms_per_launch"] = ms_top / n_launch_top
     roof["traffic"] = NCU_TRAFFIC_CFG2.get(top) if (args.config == 2 and args.tau == "real" and args.vec == "real") else None
-    roof["traffic_source"] = "profiles/r01c_final.md (ncu --set full, per launch)" if roof["traffic"] else None
+    roof["traffic_source"] = "profiles/r01d_final.md (ncu --set full, average over the stage's launches of one step)" if roof["traffic"] else None
     roof["algorithmic_bytes_per_launch"] = mt["bytes"] / n_launch_top
     tot_f = sum(m["flops"] for m in model.values())
     tot_b = sum(m["bytes"] for m in model.values())
