@@ -164,6 +164,8 @@ int bse_launch_k1e_product(const double *u, const double *vH, double *out, int v
 // acc row <- cd * acc row + 2 ce * u[v] * vH[b] on nrows rows (rows: device row ids or nullptr = identity)
 int bse_launch_k1_mix(const double *u, const double *vH, double *acc, const int *rows, int nrows, long long acc_ld,
                       bool local, long long N, int nb, double ce, double cd, cudaStream_t s);
+// out[2 row] = sum_k x[row][k]^2, out[2 row + 1] = sum_k (x[row][k] - y[row][k])^2 (rows of len doubles)
+int bse_launch_row_sumsq(const double *x, const double *y, long long len, int rows, double *out, cudaStream_t s);
 // dst[j][i] = src[i][j], n x n, leading dimensions lds / ldd
 int bse_launch_transpose(const double *src, long long lds, double *dst, long long ldd, int n, cudaStream_t s);
 // dst[w][k] = Omega * wt * src[w][k], wt = 2 for G != 0 and (1, 0) on (re, im) of G = 0 (entry 0 of H)

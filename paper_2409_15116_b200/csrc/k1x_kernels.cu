@@ -250,6 +250,30 @@ k1_mix_kernel(const double *__restrict__ u, const double *__restrict__ vH, doubl
     }
 }
 
+// out[2 row] = sum_k x[row][k]^2, out[2 row + 1] = sum_k (x[row][k] - y[row][k])^2; one CTA per row, fixed-order tree
+__global__ void __launch_bounds__(256)
+row_sumsq_kernel(const double *__restrict__ x, const double *__restrict__ y, long long len, double *__restrict__ out) {
+    __shared__ double red[256], red2[256];
+    const double *row = x + (long long)blockIdx.x * len, *row2 = y + (long long)blockIdx.x * len;
+    double s = 0.0, d = 0.0;
+    for (long long k = threadIdx.x; k < len; k += 256) {
+        const double a = row[k], e = a - row2[k];
+        s = fma(a, a, s);
+        d = fma(e, e, d);
+    }
+    red[threadIdx.x] = s;
+    red2[threadIdx.x] = d;
+    __syncthreads();
+    for (int w = 128; w > 0; w >>= 1) {
+        if ((int)threadIdx.x < w) { red[threadIdx.x] += red[threadIdx.x + w]; red2[threadIdx.x] += red2[threadIdx.x + w]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        out[2 * blockIdx.x] = red[0];
+        out[2 * blockIdx.x + 1] = red2[0];
+    }
+}
+
 __global__ void transpose_kernel(const double *__restrict__ src, long long lds, double *__restrict__ dst, long long ldd, int n) {
     const int i = blockIdx.y * blockDim.y + threadIdx.y, j = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n && j < n) dst[(long long)j * ldd + i] = src[(long long)i * lds + j];
@@ -375,6 +399,12 @@ int bse_launch_k1_mix(const double *u, const double *vH, double *acc, const int 
     const int threads = 256;
     const unsigned tiles = (unsigned)((N / 2 + threads - 1) / threads);
     k1_mix_kernel<<<dim3(tiles, nrows), threads, 0, s>>>(u, vH, acc, rows, acc_ld, local ? 1 : 0, N, nb, 2.0 * ce, cd);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
+int bse_launch_row_sumsq(const double *x, const double *y, long long len, int rows, double *out, cudaStream_t s) {
+    row_sumsq_kernel<<<rows, 256, 0, s>>>(x, y, len, out);
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }
