@@ -118,11 +118,12 @@ int bse_get_overlap(const bse_handle *h, double *O /* HOST [Nv][Nv], eq. 16 */);
 int bse_get_tau(bse_handle *h, long long first, long long count, double *dst, unsigned layout);
 
 /* ---- measurement helpers ---- */
-/* Environment (test hooks, read when the apply plans its memory; they only ever lower a limit): BSE_MAX_GROUP caps the number
- * of trial blocks processed together in the PW layout, BSE_MAX_BATCH caps the pairs of one row batch, so that small cases
- * exercise the multi-group / multi-batch paths of the large configurations.  BSE_COMPACT_INV = k forces the compact
- * inverse plane kernel (sized for k CTAs per SM; 0 = never) at every grid size instead of only where the full-plane kernel
- * leaves one CTA per SM. */
+/* Debug / test knobs of one handle (nothing is read from the environment).  They only lower a limit or choose between
+ * equivalent kernels, never change a result:  "max_group" caps the number of trial blocks processed together in the PW
+ * layout, "max_batch" caps the pairs of one row batch (so that small cases exercise the multi-group / multi-batch paths of
+ * the large configurations; 0 = no cap);  "compact_inv" = k forces the compact inverse plane kernel sized for k CTAs per SM
+ * (0 = never, -1 = automatic).  BSE_EINVAL for an unknown key. */
+int bse_debug_set(bse_handle *h, const char *key, long long value);
 /* Per-stage device time (CUDA events on the library's stream).  enable != 0 switches recording on (adds a
  * host sync per call).  Stage indices: BSE_ST_*; ms and launches are arrays of BSE_ST_COUNT, accumulated since
  * the last bse_profile_reset. */
@@ -135,7 +136,15 @@ int bse_profile_get(const bse_handle *h, double *ms /* [BSE_ST_COUNT] */, long l
 /* Algorithmic work of the launches since the last reset (always counted): flops and compulsory HBM bytes per stage,
  * by the per-unit figures of DESIGN.md section 6 times the units each launch processed. */
 int bse_profile_model(const bse_handle *h, double *flops /* [BSE_ST_COUNT] */, double *bytes /* [BSE_ST_COUNT] */);
+/* Implementation traffic NOT in that model: bytes of the stick-plane intermediate Z handed from one pass of the 3-D transform to
+ * the other (it exists only because the transform is two kernels).  bench.py reports fractions with and without it. */
+int bse_profile_handoff(const bse_handle *h, double *bytes /* [BSE_ST_COUNT] */);
 const char *bse_stage_name(int stage);
+
+/* Device time (ms, CUDA events on the library's stream) of the most recent fill of the tau store - the pair integrals a2..a8
+ * (+a9 for BSE_TAU_REAL) of all P pairs, screen and list excluded: inside bse_build_tau for BSE_TAU_REAL / BSE_TAU_PW, inside
+ * the apply for BSE_TAU_STREAM (where bse_build_tau only screens).  Synchronises.  BSE_ESTATE if nothing was filled yet. */
+int bse_last_tau_fill_ms(bse_handle *h, double *ms);
 
 /* FP64 peak probe: runs a dependent-free DMMA (mma.sync m8n8k4 f64) chain and a DFMA chain on every SM and
  * returns the achieved TFLOP/s of each (the roofline denominators for the dense contractions). */

@@ -43,10 +43,13 @@ _sig = {
     "bse_get_pairs": [_vp, _vp],
     "bse_get_overlap": [_vp, _vp],
     "bse_get_tau": [_vp, _ll, _ll, _vp, _u],
+    "bse_debug_set": [_vp, C.c_char_p, _ll],
+    "bse_last_tau_fill_ms": [_vp, C.POINTER(_d)],
     "bse_profile_enable": [_vp, _i],
     "bse_profile_reset": [_vp],
     "bse_profile_get": [_vp, C.POINTER(_d), C.POINTER(_ll)],
     "bse_profile_model": [_vp, C.POINTER(_d), C.POINTER(_d)],
+    "bse_profile_handoff": [_vp, C.POINTER(_d)],
     "bse_probe_fp64_peak": [C.POINTER(_d), C.POINTER(_d), _vp],
 }
 for _name, _args in _sig.items():
@@ -157,6 +160,16 @@ def bse_get_tau(h, first, count, dst, layout=BSE_TAU_REAL):
     _check(lib.bse_get_tau(h, int(first), int(count), _ptr(dst), int(layout)), "bse_get_tau")
 
 
+def bse_debug_set(h, key, value):
+    _check(lib.bse_debug_set(h, str(key).encode(), int(value)), "bse_debug_set")
+
+
+def bse_last_tau_fill_ms(h):
+    v = _d()
+    _check(lib.bse_last_tau_fill_ms(h, C.byref(v)), "bse_last_tau_fill_ms")
+    return v.value
+
+
 def bse_profile_enable(h, on=True):
     _check(lib.bse_profile_enable(h, 1 if on else 0), "bse_profile_enable")
 
@@ -177,6 +190,12 @@ def bse_profile_model(h):
     by = (_d * len(STAGES))()
     _check(lib.bse_profile_model(h, fl, by), "bse_profile_model")
     return {s: (fl[i], by[i]) for i, s in enumerate(STAGES)}
+
+
+def bse_profile_handoff(h):
+    by = (_d * len(STAGES))()
+    _check(lib.bse_profile_handoff(h, by), "bse_profile_handoff")
+    return {s: by[i] for i, s in enumerate(STAGES)}
 
 
 def bse_probe_fp64_peak(stream=None):

@@ -36,9 +36,12 @@ int upload(T *&dst, const std::vector<T> &src) {
 
 struct StageTimer {
     bse_handle *h; int st;
-    StageTimer(bse_handle *h_, int st_, double flops, double bytes) : h(h_), st(st_) {
+    // bytes: algorithmic HBM bytes by SURVEY 8(d) (fields, coefficients on H, GEMM operands); handoff: bytes of the stick-plane
+    // intermediate Z, which exists only because the 3-D transform is split into two kernels (implementation traffic)
+    StageTimer(bse_handle *h_, int st_, double flops, double bytes, double handoff = 0.0) : h(h_), st(st_) {
         h->st_flops[st] += flops;
         h->st_bytes[st] += bytes;
+        h->st_handoff[st] += handoff;
         if (h->prof) cudaEventRecord(h->ev0, h->stream);
     }
     ~StageTimer() {
@@ -168,22 +171,22 @@ struct Model {
 
 int st_fwd_plane(bse_handle *h, const FftPlan &pl, const double *fields, const int2 *pairs, long long p0, int cnt) {
     const Model m(pl);
-    StageTimer t(h, BSE_ST_FWD_PLANE, cnt * m.plane_flops, cnt * (m.N8 + m.z));
+    StageTimer t(h, BSE_ST_FWD_PLANE, cnt * m.plane_flops, cnt * m.N8, cnt * m.z);
     return bse_launch_fwd_plane(pl, fields, pairs, p0, cnt, pl.N, h->Z, h->stream);
 }
 int st_fwd_stick(bse_handle *h, const FftPlan &pl, int cnt, double2 *X, const double *scale, const int *scatter = nullptr) {
     const Model m(pl);
-    StageTimer t(h, BSE_ST_FWD_STICK, cnt * m.stick_flops, cnt * (m.z + m.g));
+    StageTimer t(h, BSE_ST_FWD_STICK, cnt * m.stick_flops, cnt * m.g, cnt * m.z);
     return bse_launch_fwd_stick(pl, h->Z, cnt, X, scale, h->stream, scatter);
 }
 int st_inv_stick(bse_handle *h, const FftPlan &pl, const double2 *T, int cnt) {
     const Model m(pl);
-    StageTimer t(h, BSE_ST_INV_STICK, cnt * m.stick_flops, cnt * (m.z + m.g));
+    StageTimer t(h, BSE_ST_INV_STICK, cnt * m.stick_flops, cnt * m.g, cnt * m.z);
     return bse_launch_inv_stick(pl, T, cnt, h->Z, h->stream);
 }
 int st_inv_plane(bse_handle *h, const FftPlan &pl, int cnt, double *out) {
     const Model m(pl);
-    StageTimer t(h, BSE_ST_INV_PLANE, cnt * m.plane_flops, cnt * (m.N8 + m.z));
+    StageTimer t(h, BSE_ST_INV_PLANE, cnt * m.plane_flops, cnt * m.N8, cnt * m.z);
     return bse_launch_inv_plane(pl, h->Z, cnt, pl.N, out, h->stream);
 }
 // C[M][Nn] = alpha colscale[n] sum_k A[m][k] B[n][k]   (split-K DMMA)
@@ -271,14 +274,15 @@ int ensure_u_pw(bse_handle *h) {
         BSE_CUDA(cudaMalloc(&h->uG, bytes));
         BSE_CUDA(cudaMalloc(&h->uGw, bytes));
     }
-    h->uG_valid = true;
     int rc;
     for (long long v0 = 0; v0 < h->Nv; v0 += h->Pb) {
         const int cnt = (int)std::min<long long>(h->Pb, h->Nv - v0);
         if ((rc = st_fwd_plane(h, pl, h->u, nullptr, v0, cnt))) return rc;
         if ((rc = st_fwd_stick(h, pl, cnt, h->uG + v0 * pl.npw_h, pl.inv2n))) return rc;
     }
-    return bse_launch_weight_pw(h->uG, h->uGw, pl.npw_h, h->Nv, h->Omega, h->stream);
+    if ((rc = bse_launch_weight_pw(h->uG, h->uGw, pl.npw_h, h->Nv, h->Omega, h->stream))) return rc;
+    h->uG_valid = true;                       // only once every fill has been enqueued without error
+    return BSE_OK;
 }
 
 // Is every orbital band-limited to S?  Forms T_S u_v (forward transform, truncation to S, inverse transform) and requires
@@ -354,7 +358,7 @@ int p_c_rows_real(bse_handle *h, double *x, long long rows) {
         for (long long c0 = 0; c0 < mm; c0 += h->Pb) {
             const int cnt = (int)std::min<long long>(h->Pb, mm - c0);
             if ((rc = st_inv_stick(h, pl, h->accG + (r0 + c0) * npw_h, cnt))) return rc;
-            StageTimer t(h, BSE_ST_PC_UPDATE, cnt * m.plane_flops, cnt * (2.0 * m.N8 + m.z));
+            StageTimer t(h, BSE_ST_PC_UPDATE, cnt * m.plane_flops, cnt * 2.0 * m.N8, cnt * m.z);
             if ((rc = bse_launch_inv_plane(pl, h->Z, cnt, pl.N, x + (r0 + c0) * h->N, h->stream, true))) return rc;
         }
     }
@@ -403,12 +407,15 @@ int ensure_tau_store(bse_handle *h, bool real) {
 
 int fill_tau_store(bse_handle *h, bool real) {
     int rc;
+    cudaEventRecord(h->ev_fill0, h->stream);        // device time of the pair integrals alone (bse_last_tau_fill_ms)
     for (long long p0 = 0; p0 < h->P; p0 += h->Pb) {
         const int cnt = (int)std::min<long long>(h->Pb, h->P - p0);
         if (real) rc = run_pair_batch(h, p0, cnt, h->T, h->tau_r + p0 * h->N);
         else rc = run_pair_batch(h, p0, cnt, h->tau_g + p0 * h->fft.npw_h, nullptr);
         if (rc) return rc;
     }
+    cudaEventRecord(h->ev_fill1, h->stream);
+    h->fill_timed = true;
     return BSE_OK;
 }
 
@@ -488,7 +495,10 @@ int plan_row_batches(bse_handle *h, int rows_cap) {
 int plan_apply_memory(bse_handle *h, int B) {
     const bool pw = (h->flags & BSE_VEC_PW) != 0;
     const bool batched = (h->flags & BSE_TAU_MASK) != BSE_TAU_REAL;
-    if (h->plan_ok && h->plan_nadj == h->nadj && (!pw || h->Bg >= B || h->Bg_final)) return BSE_OK;
+    // the plan is kept only for the very adjacency it was made for (a rebuilt list with the same pair count but other
+    // pairs must not reuse the old batches / eslot) and while the group still holds B blocks
+    const bool same_list = !batched || (h->plan_adj_ptr_h == h->adj_ptr_h && h->plan_adj_h == h->adj_h);
+    if (h->plan_ok && same_list && (!pw || h->Bg >= B || h->Bg_final)) return BSE_OK;
     cudaFree(h->tau_batch); cudaFree(h->a_r); cudaFree(h->acc_r);
     h->tau_batch = h->a_r = h->acc_r = nullptr;
     h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
@@ -532,14 +542,11 @@ int plan_apply_memory(bse_handle *h, int B) {
         pacc = pacc_of(bg);
         rows_cap = std::min<long long>(h->Nv, std::max<long long>(1, (long long)(2.0 * pacc / avgdeg)));
     }
-    // test hooks: BSE_MAX_GROUP / BSE_MAX_BATCH cap B_g / the row batch so that small cases exercise several groups
-    // and several row batches (tests/test_gpu_parity.py); they never raise a limit
-    if (const char *e = std::getenv("BSE_MAX_GROUP")) {
-        const long long cap_g = std::atoll(e);
-        if (cap_g >= 1 && bg > cap_g) { bg = cap_g; }
-    }
-    if (const char *e = std::getenv("BSE_MAX_BATCH")) {
-        const long long cap_p = std::max<long long>(std::atoll(e), maxdeg);
+    // test knobs (bse_debug_set): cap B_g / the row batch so that small cases exercise several groups and several row
+    // batches (tests/test_gpu_parity.py); they never raise a limit
+    if (h->dbg_max_group >= 1 && bg > h->dbg_max_group) bg = h->dbg_max_group;
+    if (h->dbg_max_batch >= 1) {
+        const long long cap_p = std::max<long long>(h->dbg_max_batch, maxdeg);
         if (pacc > cap_p) {
             pacc = cap_p;
             if (pw && batched) rows_cap = std::min<long long>(h->Nv, std::max<long long>(1, (long long)(2.0 * pacc / avgdeg)));
@@ -556,7 +563,8 @@ int plan_apply_memory(bse_handle *h, int B) {
         if (rc) return rc;
     }
     h->plan_ok = true;
-    h->plan_nadj = h->nadj;
+    h->plan_adj_ptr_h = h->adj_ptr_h;
+    h->plan_adj_h = h->adj_h;
     return BSE_OK;
 }
 
@@ -609,12 +617,12 @@ int ensure_u_apply(bse_handle *h) {
         h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
         BSE_CUDA(cudaMalloc(&h->u_a, (size_t)h->Nv * pl.N * 8));
     }
-    h->u_a_valid = true;
     for (long long v0 = 0; v0 < h->Nv; v0 += h->Pb) {
         const int cnt = (int)std::min<long long>(h->Pb, h->Nv - v0);
         if ((rc = st_inv_stick(h, pl, h->uG + v0 * pl.npw_h, cnt))) return rc;
         if ((rc = st_inv_plane(h, pl, cnt, h->u_a + v0 * pl.N))) return rc;
     }
+    h->u_a_valid = true;
     return BSE_OK;
 }
 
@@ -660,9 +668,9 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
         const int r0 = bt.v0, rows = bt.v1 - bt.v0;               // rows rowlist[r0 .. r0 + rows)
         for (int c0 = 0; c0 < bt.nu; c0 += (int)h->Pb) {              // tau(G) -> tau(r) of the batch's pairs
             const int c = (int)std::min<long long>(h->Pb, bt.nu - c0);
-            { StageTimer t(h, BSE_ST_INV_STICK, uniq * c * m.stick_flops, uniq * c * (m.z + m.g));
+            { StageTimer t(h, BSE_ST_INV_STICK, uniq * c * m.stick_flops, uniq * c * m.g, uniq * c * m.z);
               if ((rc = bse_launch_inv_stick(pl, h->tau_g, c, h->Z, h->stream, h->batch_pairs, bt.u0 + c0))) return rc; }
-            { StageTimer t(h, BSE_ST_INV_PLANE, uniq * c * m.plane_flops, uniq * c * (m.N8 + m.z));
+            { StageTimer t(h, BSE_ST_INV_PLANE, uniq * c * m.plane_flops, uniq * c * m.N8, uniq * c * m.z);
               if ((rc = bse_launch_inv_plane(pl, h->Z, c, pl.N, h->tau_batch + (long long)c0 * pl.N, h->stream))) return rc; }
         }
         { StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)pl.N * (double)h->nadj * rows / h->Nv,
@@ -835,6 +843,8 @@ extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cel
     }
     cudaEventCreate(&h->ev0);
     cudaEventCreate(&h->ev1);
+    cudaEventCreate(&h->ev_fill0);
+    cudaEventCreate(&h->ev_fill1);
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) { bse_set_error("stream sync failed"); return fail(BSE_ECUDA); }
     *hout = h;
     return BSE_OK;
@@ -856,6 +866,8 @@ extern "C" int bse_destroy(bse_handle *h) {
     if (h->s_out) cudaStreamDestroy(h->s_out);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
+    if (h->ev_fill0) cudaEventDestroy(h->ev_fill0);
+    if (h->ev_fill1) cudaEventDestroy(h->ev_fill1);
     delete h;
     return BSE_OK;
 }
@@ -981,6 +993,10 @@ extern "C" int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B)
     // staging: the K1x plan's buffers when they exist (they took the free memory), else own workspace
     double *a_r = h->a_r, *dens = (h->tau_batch && h->Pacc >= h->Pb + 1) ? h->tau_batch : nullptr;
     if (!a_r || !dens) {
+        if ((rc = ensure_k1e_ws(h, (size_t)((a_r ? 0 : Nv) + (dens ? 0 : 1 + h->Pb)) * pl.N * 8))) return rc;
+        // ensure_k1e_ws may have dropped the K1x plan's buffers to make room: look at them again
+        if (a_r && !h->a_r) { a_r = nullptr; dens = nullptr; }
+        if (dens && !h->tau_batch) dens = nullptr;
         if ((rc = ensure_k1e_ws(h, (size_t)((a_r ? 0 : Nv) + (dens ? 0 : 1 + h->Pb)) * pl.N * 8))) return rc;
         double *ws = h->k1e_ws;
         if (!a_r) { a_r = ws; ws += Nv * pl.N; }
@@ -1144,6 +1160,29 @@ extern "C" int bse_get_tau(bse_handle *h, long long first, long long count, doub
     return BSE_OK;
 }
 
+// Debug / test knobs (they only ever lower a limit or pick between equivalent kernels; results do not change)
+extern "C" int bse_debug_set(bse_handle *h, const char *key, long long value) {
+    if (!h || !key) { bse_set_error("null pointer"); return BSE_EINVAL; }
+    const std::string k(key);
+    if (k == "max_group") { h->dbg_max_group = value; h->plan_ok = false; }
+    else if (k == "max_batch") { h->dbg_max_batch = value; h->plan_ok = false; }
+    else if (k == "compact_inv") { h->fft.compact_inv = h->ffta.compact_inv = (int)value; }
+    else { bse_set_error("bse_debug_set: unknown key " + k); return BSE_EINVAL; }
+    return BSE_OK;
+}
+
+// Device time of the most recent fill of the tau store (a2..a8(+a9) for all P pairs): inside bse_build_tau for BSE_TAU_REAL / PW,
+// inside bse_apply_k1x / bse_apply_k1 for BSE_TAU_STREAM.  Synchronises on the closing event.
+extern "C" int bse_last_tau_fill_ms(bse_handle *h, double *ms) {
+    if (!h || !ms) { bse_set_error("null pointer"); return BSE_EINVAL; }
+    if (!h->fill_timed) { bse_set_error("no tau fill yet"); return BSE_ESTATE; }
+    BSE_CUDA(cudaEventSynchronize(h->ev_fill1));
+    float f = 0.f;
+    BSE_CUDA(cudaEventElapsedTime(&f, h->ev_fill0, h->ev_fill1));
+    *ms = f;
+    return BSE_OK;
+}
+
 extern "C" int bse_profile_enable(bse_handle *h, int enable) {
     if (!h) return BSE_EINVAL;
     h->prof = enable != 0;
@@ -1151,7 +1190,7 @@ extern "C" int bse_profile_enable(bse_handle *h, int enable) {
 }
 extern "C" int bse_profile_reset(bse_handle *h) {
     if (!h) return BSE_EINVAL;
-    for (int i = 0; i < BSE_ST_COUNT; ++i) { h->st_ms[i] = 0; h->st_launch[i] = 0; h->st_flops[i] = 0; h->st_bytes[i] = 0; }
+    for (int i = 0; i < BSE_ST_COUNT; ++i) { h->st_ms[i] = 0; h->st_launch[i] = 0; h->st_flops[i] = 0; h->st_bytes[i] = 0; h->st_handoff[i] = 0; }
     return BSE_OK;
 }
 extern "C" int bse_profile_get(const bse_handle *h, double *ms, long long *launches) {
@@ -1168,5 +1207,10 @@ extern "C" int bse_profile_model(const bse_handle *h, double *flops, double *byt
         if (flops) flops[i] = h->st_flops[i];
         if (bytes) bytes[i] = h->st_bytes[i];
     }
+    return BSE_OK;
+}
+extern "C" int bse_profile_handoff(const bse_handle *h, double *bytes) {
+    if (!h || !bytes) return BSE_EINVAL;
+    for (int i = 0; i < BSE_ST_COUNT; ++i) bytes[i] = h->st_handoff[i];
     return BSE_OK;
 }

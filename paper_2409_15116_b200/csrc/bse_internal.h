@@ -19,6 +19,7 @@ struct FftPlan {
     int NS = 0;          // number of half sticks
     long long npw_h = 0;
     const void *ops = nullptr;    // bsefft::FftOps of this n
+    int compact_inv = -1;         // inverse plane kernel: -1 automatic, 0 never compact, k > 1 compact sized for k CTAs / SM
     // device tables
     double2 *tw = nullptr;        // [n]   exp(-2 pi i t / n)
     int *soff = nullptr;          // [n]   stick index of (t2 = m2 mod n, m3) is soff[t2] + m3
@@ -85,7 +86,10 @@ struct bse_handle {
     double *a_r = nullptr, *acc_r = nullptr;       // [Bg][Nv][N]
     int Bg = 0, rows_cap = 0;                      // acc_r holds rows_cap rows per block (row batches)
     bool Bg_final = false, plan_ok = false;
-    long long plan_nadj = -1;
+    std::vector<int> plan_adj_h, plan_adj_ptr_h;   // the adjacency the row batches were planned for (exact comparison)
+    // debug / test knobs (bse_debug_set; never read from the environment): caps that only ever lower a limit
+    long long dbg_max_group = 0, dbg_max_batch = 0;   // 0 = no cap
+    int dbg_compact_inv = -1;                         // -1 = automatic choice of the inverse plane kernel
     long long Pacc = 0;                            // capacity of tau_batch in directed entries                         // Bg is already the most that fits
     // K1e workspaces (grow-only): dens / vH [B][N] (REAL) or one block's a(r) [Nv][Na] + [1][Na] + product rows [Pb][Na] (PW)
     double *k1e_ws = nullptr;
@@ -110,8 +114,11 @@ struct bse_handle {
     bool prof = false;
     double st_ms[BSE_ST_COUNT] = {0};
     long long st_launch[BSE_ST_COUNT] = {0};
-    double st_flops[BSE_ST_COUNT] = {0}, st_bytes[BSE_ST_COUNT] = {0};   // algorithmic work of the launches so far
+    double st_flops[BSE_ST_COUNT] = {0}, st_bytes[BSE_ST_COUNT] = {0};   // algorithmic work of the launches so far (SURVEY 8(d))
+    double st_handoff[BSE_ST_COUNT] = {0};                               // + bytes of the Z hand-off between plane and stick pass
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    cudaEvent_t ev_fill0 = nullptr, ev_fill1 = nullptr;   // around the last fill of the tau store
+    bool fill_timed = false;
 };
 
 void bse_set_error(const std::string &msg);
@@ -128,8 +135,9 @@ int bse_cuda_fail(cudaError_t e, const char *what);
 int bse_fft_select(FftPlan &pl);     // sets R1, R2, ops for pl.n; BSE_EUNSUPPORTED if there is no kernel for n
 // fields: [.][N]; pairs == nullptr: plain transform of field p0+p.  scale: [npw_h] table applied in the stick pass.
 // fwd_stick: scatter != nullptr (device array): field p is written to X + scatter[p] * npw_h instead of X + p * npw_h.
+// np > 0: the fields hold np planes each (one slab, N = np n^2 is then the field stride) instead of n
 int bse_launch_fwd_plane(const FftPlan &pl, const double *fields, const int2 *pairs, long long p0, int count,
-                         long long N, double2 *Z, cudaStream_t s);
+                         long long N, double2 *Z, cudaStream_t s, int np = 0);
 int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2 *X, const double *scale,
                          cudaStream_t s, const int *scatter = nullptr);
 // gather != nullptr: field p is read from T + gather[g0 + p] * npw_h (pair indices of a row batch)
@@ -137,7 +145,13 @@ int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2
                          const int *gather = nullptr, int g0 = 0);
 // subtract: out <- out - transform instead of out <- transform (P_c update of the REAL layout)
 int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long long N, double *out, cudaStream_t s,
-                         bool subtract = false);
+                         bool subtract = false, int np = 0);
+// slab forms of the stick passes (fft_kernels.cuh): the planes i1 = slab + R1 k2, k2 < R2, only.  Zs[count][R2][NS].
+// forward: field p goes to row (p / rc) * row_ld + row0 + p % rc of X; accumulate: X += (slabs 1 .. R1-1) instead of X =
+int bse_launch_inv_stick_slab(const FftPlan &pl, const double2 *T, int count, double2 *Zs, cudaStream_t s, int slab,
+                              const int *gather = nullptr, int g0 = 0);
+int bse_launch_fwd_stick_slab(const FftPlan &pl, const double2 *Zs, int count, double2 *X, const double *scale, cudaStream_t s,
+                              int slab, bool accumulate, int rc, long long row_ld, long long row0);
 
 // gemm_dmma.cu
 enum { EPI_PARTIAL = 0, EPI_TAU = 1, EPI_SUB = 2, EPI_STORE = 3 };

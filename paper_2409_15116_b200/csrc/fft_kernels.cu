@@ -32,22 +32,34 @@ int bse_fft_select(FftPlan &pl) {
     return BSE_OK;
 }
 
-static PlanDev to_dev(const FftPlan &pl) {
+static PlanDev to_dev(const FftPlan &pl, int np = 0) {
     PlanDev d;
     d.R = pl.R; d.W = pl.W; d.NS = pl.NS;
+    d.np = np > 0 ? np : pl.n;
     d.tw = pl.tw; d.soff = pl.soff; d.wmax = pl.wmax; d.wmin = pl.wmin; d.hmapT = pl.hmapT;
     return d;
 }
 
 int bse_launch_fwd_plane(const FftPlan &pl, const double *fields, const int2 *pairs, long long p0, int count,
-                         long long N, double2 *Z, cudaStream_t s) {
+                         long long N, double2 *Z, cudaStream_t s, int np) {
     if (count <= 0) return BSE_OK;
-    return ((const FftOps *)pl.ops)->fwd_plane(to_dev(pl), fields, pairs, p0, count, N, Z, s);
+    return ((const FftOps *)pl.ops)->fwd_plane(to_dev(pl, np), fields, pairs, p0, count, N, Z, s);
 }
 int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long long N, double *out, cudaStream_t s,
-                         bool subtract) {
+                         bool subtract, int np) {
     if (count <= 0) return BSE_OK;
-    return ((const FftOps *)pl.ops)->inv_plane(to_dev(pl), Z, count, N, out, s, subtract ? 1 : 0);
+    return ((const FftOps *)pl.ops)->inv_plane(to_dev(pl, np), Z, count, N, out, s, subtract ? 1 : 0, pl.compact_inv);
+}
+int bse_launch_inv_stick_slab(const FftPlan &pl, const double2 *T, int count, double2 *Zs, cudaStream_t s, int slab,
+                              const int *gather, int g0) {
+    if (count <= 0) return BSE_OK;
+    return ((const FftOps *)pl.ops)->inv_stick_slab(to_dev(pl), T, count, pl.npw_h, Zs, s, gather, g0, slab);
+}
+int bse_launch_fwd_stick_slab(const FftPlan &pl, const double2 *Zs, int count, double2 *X, const double *scale, cudaStream_t s,
+                              int slab, bool accumulate, int rc, long long row_ld, long long row0) {
+    if (count <= 0) return BSE_OK;
+    return ((const FftOps *)pl.ops)->fwd_stick_slab(to_dev(pl), Zs, count, X, pl.npw_h, scale, s, slab, accumulate ? 1 : 0, rc,
+                                                    row_ld, row0);
 }
 int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2 *X, const double *scale,
                          cudaStream_t s, const int *scatter) {

@@ -199,15 +199,11 @@ __global__ void splitk_reduce_kernel(const double *__restrict__ part, int splits
 constexpr int SMEM_DOT = STAGES * (A_TILE + B_TILE_K) * 8;
 constexpr int SMEM_NN = STAGES * (A_TILE + B_TILE_N) * 8;
 
+// Dynamic shared-memory opt-in of one kernel instantiation.  cudaFuncSetAttribute is thread-safe and idempotent, so it is
+// simply issued before every launch (a few hundred ns on the host) instead of remembering pointers in a shared table.
 template <typename KernelT>
 int prep(KernelT k, int smem) {
-    // all instantiations share one function-pointer type, so remember the pointers already prepared
-    static const void *done[16];
-    static int ndone = 0;
-    for (int i = 0; i < ndone; ++i)
-        if (done[i] == (const void *)k) return BSE_OK;
     BSE_CUDA(cudaFuncSetAttribute((const void *)k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    if (ndone < 16) done[ndone++] = (const void *)k;
     return BSE_OK;
 }
 

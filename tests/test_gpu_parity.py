@@ -26,7 +26,7 @@ def rel(a, b):
 class Gpu:
     """Device-resident inputs + handle for one workload."""
 
-    def __init__(self, w, flags=0):
+    def __init__(self, w, flags=0, knobs=None):
         bse = _bse()
         self.bse, self.w = bse, w
         dev = torch.device("cuda:0")
@@ -34,6 +34,8 @@ class Gpu:
         phi = np.ascontiguousarray(w.phi).view(np.float64)          # interleaved (re, im)
         self.phi = torch.from_numpy(phi).to(dev)
         self.h = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, self.u, w.phi.shape[0], self.phi, w.lam, w.eta, flags)
+        for key, value in (knobs or {}).items():           # test knobs of the handle (include/bse.h: bse_debug_set)
+            bse.bse_debug_set(self.h, key, value)
 
     def build(self):
         self.bse.bse_build_tau(self.h)
@@ -64,11 +66,11 @@ class Gpu:
         self.bse.bse_destroy(self.h)
 
 
-def _check_full(w, flags=0, check_g=True):
+def _check_full(w, flags=0, check_g=True, knobs=None):
     tab = orc.Tables(w.n, w.L, w.ecut)
     pairs_ref, O = orc.screen_pairs(w.u, w.eta)
     assert orc.screen_margin(O, w.eta) > 1e-9, "workload violates the screen guard band (S10)"
-    g = Gpu(w, flags)
+    g = Gpu(w, flags, knobs)
     try:
         assert np.array_equal(g.bse.bse_gvectors(g.h), w.mill)
         pairs = g.build()
@@ -95,12 +97,12 @@ def _check_full(w, flags=0, check_g=True):
         g.close()
 
 
-def _check_pw(w, flags=0):
+def _check_pw(w, flags=0, knobs=None):
     """PW layout (a12): a, out on the half sphere H; reference = oracle apply_k1x_pw (O8 'K1x PW')."""
     bse = _bse()
     tab = orc.Tables(w.n, w.L, w.ecut)
     pairs_ref, _ = orc.screen_pairs(w.u, w.eta)
-    g = Gpu(w, flags | bse.BSE_VEC_PW)
+    g = Gpu(w, flags | bse.BSE_VEC_PW, knobs)
     try:
         pairs = g.build()
         assert np.array_equal(pairs, pairs_ref)
@@ -135,20 +137,17 @@ def test_pw_layout_all_tau_modes():
     _check_pw(wl.make(2, Nv=12, Npdep=40, B=2), bse.BSE_TAU_PW)
 
 
-def test_several_groups_and_row_batches(monkeypatch):
+def test_several_groups_and_row_batches():
     """Small case forced through the large-config machinery: trial blocks in groups of 2 (B = 5: ragged last group) and
     row batches of at most 7 pairs (several batches, pairs shared between batches re-inverted)."""
     bse = _bse()
-    monkeypatch.setenv("BSE_MAX_GROUP", "2")
-    monkeypatch.setenv("BSE_MAX_BATCH", "7")
+    knobs = {"max_group": 2, "max_batch": 7}
     cfg = wl.Config("grp", 10.0, 24, 9, 20, 8.0, 1.2, 0.8, 3.0, 0.02, 5, "random", seed=77)
     w = wl.make(cfg=cfg)
-    o1 = _check_pw(w, bse.BSE_TAU_PW)
-    o2 = _check_pw(w, bse.BSE_TAU_STREAM)
+    o1 = _check_pw(w, bse.BSE_TAU_PW, knobs)
+    o2 = _check_pw(w, bse.BSE_TAU_STREAM, knobs)
     assert rel(o2, o1) < 1e-12
-    _check_full(w, bse.BSE_TAU_PW, check_g=False)
-    monkeypatch.delenv("BSE_MAX_GROUP")
-    monkeypatch.delenv("BSE_MAX_BATCH")
+    _check_full(w, bse.BSE_TAU_PW, check_g=False, knobs=knobs)
     o3 = _check_pw(w, bse.BSE_TAU_PW)
     assert rel(o3, o1) < 1e-12
 
@@ -386,7 +385,7 @@ def test_rotate_between_representations(Nv):
 
 
 @pytest.mark.parametrize("tau", ["real", "pw", "stream"])
-def test_combined_two_body_call(tau, monkeypatch):
+def test_combined_two_body_call(tau):
     """bse_apply_k1 = ce * K1e + cd * K1x with one P_c (eq. 1), against the oracle's two terms, both layouts, every tau mode;
     the PW case is also forced through several block groups and row batches."""
     bse = _bse()
@@ -414,10 +413,7 @@ def test_combined_two_body_call(tau, monkeypatch):
     wt = np.full(tab.npw_h, 2.0)
     wt[0] = 1.0
     for forced in (False, True):
-        if forced:
-            monkeypatch.setenv("BSE_MAX_GROUP", "2")
-            monkeypatch.setenv("BSE_MAX_BATCH", "7")
-        g = Gpu(w, flag | bse.BSE_VEC_PW)
+        g = Gpu(w, flag | bse.BSE_VEC_PW, {"max_group": 2, "max_batch": 7} if forced else None)
         try:
             g.build()
             a_d = torch.from_numpy(np.ascontiguousarray(w.a_pw).view(np.float64)).to("cuda:0")
@@ -431,7 +427,7 @@ def test_combined_two_body_call(tau, monkeypatch):
             g.close()
 
 
-def test_block_count_grows_and_stream_real_batches(monkeypatch):
+def test_block_count_grows_and_stream_real_batches():
     """One handle, PW layout: B = 1 first, then B = 3 (the apply plan is re-made for the larger group) - same rows both
     times.  Then the REAL layout with BSE_TAU_STREAM forced through several row batches."""
     bse = _bse()
@@ -459,18 +455,17 @@ def test_block_count_grows_and_stream_real_batches(monkeypatch):
         assert rel(g.tau_g(2, 3), tg_ref) <= TOL
     finally:
         g.close()
-    monkeypatch.setenv("BSE_MAX_BATCH", "5")
-    _check_full(w, bse.BSE_TAU_STREAM, check_g=True)
+    _check_full(w, bse.BSE_TAU_STREAM, check_g=True, knobs={"max_batch": 5})
 
 
-def test_compact_inverse_plane_kernel_small_grids(monkeypatch):
+def test_compact_inverse_plane_kernel_small_grids():
     """The compact inverse plane kernel (used by default only at n = 120, 144) forced on small grids: radices 4x6, 5x4, 5x6."""
-    monkeypatch.setenv("BSE_COMPACT_INV", "2")
+    knobs = {"compact_inv": 2}
     for n, L, ecut, Nv, Npdep, B in ((24, 10.0, 8.0, 8, 16, 2), (20, 12.0, 4.0, 6, 9, 1), (30, 14.0, 5.0, 4, 16, 2)):
         cfg = wl.Config("cmp", L, n, Nv, Npdep, ecut, 1.3, 0.8, 3.0, 0.0, B, "random", seed=300 + n)
         w = wl.make(cfg=cfg)
-        _check_full(w)
-        _check_pw(w, _bse().BSE_TAU_PW)
+        _check_full(w, knobs=knobs)
+        _check_pw(w, _bse().BSE_TAU_PW, knobs)
 
 
 def test_real_layout_with_orbitals_that_are_not_band_limited():
@@ -486,3 +481,67 @@ def test_real_layout_with_orbitals_that_are_not_band_limited():
     w.u = np.ascontiguousarray(((V / np.sqrt(ev)) @ V.T) @ u)                                    # orthonormal again
     _check_full(w, bse.BSE_TAU_REAL, check_g=True)
     _check_full(w, bse.BSE_TAU_PW, check_g=False)
+
+
+def test_rebuilt_list_with_the_same_pair_count_gets_a_new_plan():
+    """new orbitals whose surviving-pair list has the SAME length but other pairs (the old orbitals, permuted)
+    must not reuse the row batches / slots planned for the old list.  PW layout, tau on H, row batches forced small."""
+    bse = _bse()
+    cfg = wl.Config("perm", 10.0, 24, 10, 20, 8.0, 1.2, 0.8, 3.0, 0.05, 2, "random", seed=91)
+    w = wl.make(cfg=cfg)
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    phi = np.ascontiguousarray(w.phi).view(np.float64)
+    wt = np.full(tab.npw_h, 2.0)
+    wt[0] = 1.0
+    rng = np.random.default_rng(4)
+    h = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, np.ascontiguousarray(w.u), w.phi.shape[0], phi, w.lam, w.eta,
+                       bse.BSE_PTR_HOST | bse.BSE_TAU_PW | bse.BSE_VEC_PW)
+    try:
+        bse.bse_debug_set(h, "max_batch", 6)
+        lists = []
+        for trial in range(3):
+            perm = np.arange(w.Nv) if trial == 0 else rng.permutation(w.Nv)
+            u = np.ascontiguousarray(w.u[perm])
+            a_pw = np.ascontiguousarray(w.a_pw[:, perm])
+            bse.bse_set_inputs_host(h, u, None)
+            bse.bse_build_tau(h)
+            pairs = bse.bse_get_pairs(h)
+            pairs_ref, _ = orc.screen_pairs(u, w.eta)
+            assert np.array_equal(pairs, pairs_ref)
+            lists.append(pairs)
+            a = np.ascontiguousarray(a_pw).view(np.float64)
+            out = np.empty_like(a)
+            bse.bse_apply_k1x_host(h, a, out, a_pw.shape[0])
+            tau_ref = orc.build_tau(tab, u, w.phi, w.lam, pairs_ref, want="r")
+            ref = orc.apply_k1x_pw(tab, u, pairs_ref, tau_ref, a_pw)
+            got = out.view(np.complex128).reshape(ref.shape)
+            err = np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum())
+            assert err <= TOL, (trial, err)
+        assert len(lists[0]) == len(lists[1]) == len(lists[2]) < w.Nv * (w.Nv + 1) // 2
+        assert not np.array_equal(lists[0], lists[1])          # same P, other pairs: the case the old plan check missed
+    finally:
+        bse.bse_destroy(h)
+
+
+@pytest.mark.parametrize("n", [16, 32, 36, 40, 60, 80, 100, 128])
+def test_every_supported_grid_edge(n):
+    """the grid edges no other test touches (each has its own Geo<R1,R2> instantiation), as the problem grid in
+    the REAL layout and, tau on H, in the PW layout (which runs on whatever apply grid n_a >= 3R+1 the library picks)."""
+    bse = _bse()
+    R = max(2, n // 5)
+    L = 10.0
+    ecut = 0.5 * (2.0 * np.pi / L) ** 2 * (R * R + 0.5)
+    cfg = wl.Config(f"n{n}", L, n, 3, 5, ecut, 1.6, 0.8, 3.0, 0.0, 1, "random", seed=400 + n)
+    w = wl.make(cfg=cfg)
+    _check_full(w, check_g=True)
+    _check_pw(w, bse.BSE_TAU_PW)
+
+
+def test_compact_inverse_kernel_subtract_epilogue():
+    """the SUB epilogue of the compact inverse plane kernel (P_c update of the REAL layout, taken from N_v >= 48
+    with band-limited orbitals) forced on a small grid."""
+    cfg = wl.Config("sub", 12.0, 24, 48, 24, 5.5, 1.3, 0.8, 3.0, 0.1, 2, "random", seed=95)
+    w = wl.make(cfg=cfg)
+    o1 = _check_full(w, check_g=False, knobs={"compact_inv": 2})
+    o0 = _check_full(w, check_g=False, knobs={"compact_inv": 0})
+    assert rel(o1, o0) < 1e-12
