@@ -325,12 +325,13 @@ def main():
         out_host = torch.empty_like(a_host).pin_memory()
         u_d, phi_d, a_d = u_host.to(dev), phi_host.to(dev), a_host.to(dev)
     n_pdep = phi_d.shape[0]
+    Nv = w.Nv
     t_gen = time.perf_counter() - t_gen0
     out_d = torch.empty_like(a_d)
     flags = {"real": bse.BSE_TAU_REAL, "pw": bse.BSE_TAU_PW, "stream": bse.BSE_TAU_STREAM}[args.tau]
     flags |= bse.BSE_VEC_PW if args.vec == "pw" else bse.BSE_VEC_REAL
     stream = torch.cuda.current_stream().cuda_stream
-    h = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u_d, n_pdep, phi_d, w.lam, w.eta, flags, stream)
+    h = bse.bse_create([w.n] * 3, w.cell, w.ecut, Nv, u_d, n_pdep, phi_d, w.lam, w.eta, flags, stream)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
     def step(timed):
@@ -466,7 +467,7 @@ def main():
 
     # ---- end to end through the C ABI with host (pinned) buffers ----
     def run_e2e(flags_e, a_h, out_h, reps):
-        hh = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u_host, n_pdep, phi_host, w.lam, w.eta,
+        hh = bse.bse_create([w.n] * 3, w.cell, w.ecut, Nv, u_host, n_pdep, phi_host, w.lam, w.eta,
                             flags_e | bse.BSE_PTR_HOST, stream)
         eb, ea, ef = [], [], []
         for i in range(1 + reps):
@@ -518,19 +519,19 @@ def main():
         if large:
             if u_host is not None:
                 phi_np = phi_host.numpy().view(np.complex128)[..., 0]
-                info = oracle_sample(lambda v: u_host[v].numpy(), w.n, w.L, w.ecut, w.Nv, phi_np, w.lam, pairs_host,
+                info = oracle_sample(lambda v: u_host[v].numpy(), w.n, w.L, w.ecut, Nv, phi_np, w.lam, pairs_host,
                                      n_pairs=2, n_rows=1, n_cols=24)
             else:                                         # --no-e2e: the inputs are still on the device
                 phi_np = phi_d.cpu().numpy().view(np.complex128)[..., 0]
-                info = oracle_sample(lambda v: u_d[v].cpu().numpy(), w.n, w.L, w.ecut, w.Nv, phi_np, w.lam, pairs_host,
+                info = oracle_sample(lambda v: u_d[v].cpu().numpy(), w.n, w.L, w.ecut, Nv, phi_np, w.lam, pairs_host,
                                      n_pairs=2, n_rows=1, n_cols=24)
         else:
-            info = oracle_sample(lambda v: w.u[v], w.n, w.L, w.ecut, w.Nv, w.phi, w.lam, pairs_host,
-                                 n_pairs=40, n_rows=8, n_cols=w.Nv, seconds_cap=15.0)
+            info = oracle_sample(lambda v: w.u[v], w.n, w.L, w.ecut, Nv, w.phi, w.lam, pairs_host,
+                                 n_pairs=40, n_rows=8, n_cols=Nv, seconds_cap=15.0)
         if info:
             cpu = {"value": info["pairs_per_s"], "unit": "pairs/s", "cores": info["cores"], "kind": "oracle",
                    "sample": f"{info['sampled_entries']} entries of the eq.16 overlap matrix in long double ({info['per_entry_s']:.4f} s "
-                             f"each, extrapolated to Nv^2 = {w.Nv * w.Nv}: {info['screen_s']:.0f} s) + tau for {info['sampled_pairs']} "
+                             f"each, extrapolated to Nv^2 = {Nv * Nv}: {info['screen_s']:.0f} s) + tau for {info['sampled_pairs']} "
                              f"of {info['P']} surviving pairs ({info['per_pair_s']:.3f} s/pair, extrapolated to all pairs); the pairs "
                              f"are drawn from the list this run produced"}
 
@@ -538,7 +539,7 @@ def main():
         "metric": METRIC, "value": world * P / (t_pairs_ms * 1e-3), "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": tb_ms + ta_ms, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_string(args.config, w.n, w.Nv, n_pdep, npw_h, w.eta, P, B),
+        "config": {"workload": workload_string(args.config, w.n, Nv, n_pdep, npw_h, w.eta, P, B),
                    "tau_storage": args.tau, "vec_layout": args.vec, "parallelism": "replicas" if world > 1 else "1gpu",
                    "l2": "512 MB buffer written between timed steps (L2 flush); inputs also exceed L2",
                    "fallback": fallback},

@@ -95,6 +95,20 @@ int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, double ce, 
  * U: DEVICE [Nv][Nv] row-major real orthogonal (Gamma point); x, y: DEVICE, layout per BSE_VEC_* flag; y must not alias x. */
 int bse_rotate(bse_handle *h, const double *U, int transpose, const double *x, double *y, int B);
 
+/* JADE localisation of the occupied orbitals (eq. 12-15): the U that bse_rotate applies and
+ * that makes the screen of eq. 16 effective.  Needs no handle.
+ *   psi     DEVICE [Nv][N] real orthonormal orbitals on the n^3 grid (cubic cell of edge cell[0], even n)
+ *   U       DEVICE [Nv][Nv] row-major, written: psi~_v = sum_v' U[v][v'] psi_v' (eq. 12) minimises the spread of eq. 14
+ *   psi_loc DEVICE [Nv][N] or NULL: U psi
+ *   tol, max_sweeps  sweeps of concurrent Givens rotations (round-robin rounds of disjoint pairs; every angle of a round from
+ *           the six matrices A^(n) = <psi|cos,sin(2 pi x/L)|psi> as they stand) until the largest |sin theta| of a sweep < tol
+ *   init_eig != 0: start from the eigenvectors of A^(1) sorted by ascending eigenvalue (the paper's choice), else the identity
+ *   sweeps  HOST, may be NULL: sweeps done      spread HOST [2], may be NULL: sigma^2 of eq. 14 before and after
+ * Work runs on an internal stream ordered after `stream`; `stream` is made to wait for the results; the call synchronises.
+ * Readings J1-J4 (angle formula, schedule, stopping, orientation): DESIGN.md section 2. */
+int bse_jade(const int grid[3], const double cell[9], int Nv, const double *psi, double *U, double *psi_loc,
+             double tol, int max_sweeps, int init_eig, int *sweeps, double *spread, void *stream);
+
 /* Same with HOST pointers: copies a to the device, applies, copies out back, synchronises (the end-to-end
  * call bench.py times as `e2e`).  With BSE_TAU_REAL the blocks are pipelined: block b+1 is copied in and block b-1
  * copied out (two copy streams) while block b is applied.  Pinned host memory is needed for the overlap. */
@@ -122,7 +136,9 @@ int bse_get_tau(bse_handle *h, long long first, long long count, double *dst, un
  * equivalent kernels, never change a result:  "max_group" caps the number of trial blocks processed together in the PW
  * layout, "max_batch" caps the pairs of one row batch (so that small cases exercise the multi-group / multi-batch paths of
  * the large configurations; 0 = no cap);  "compact_inv" = k forces the compact inverse plane kernel sized for k CTAs per SM
- * (0 = never, -1 = automatic).  BSE_EINVAL for an unknown key. */
+ * (0 = never, -1 = automatic);  "slab_rows" = k caps the rows per chunk of the plane-slab apply (PW layout with tau on H; -1 = never
+ * take that path, 0 = no cap); setting "max_group" or "max_batch" also keeps the apply on the group / row-batch path.
+ * BSE_EINVAL for an unknown key. */
 int bse_debug_set(bse_handle *h, const char *key, long long value);
 /* Per-stage device time (CUDA events on the library's stream).  enable != 0 switches recording on (adds a
  * host sync per call).  Stage indices: BSE_ST_*; ms and launches are arrays of BSE_ST_COUNT, accumulated since

@@ -36,6 +36,7 @@ _sig = {
     "bse_rotate": [_vp, _vp, _i, _vp, _vp, _i],
     "bse_apply_k1": [_vp, _vp, _vp, _i, _d, _d],
     "bse_set_inputs_host": [_vp, _vp, _vp],
+    "bse_jade": [C.POINTER(_i), C.POINTER(_d), _i, _vp, _vp, _vp, _d, _i, _i, C.POINTER(_i), C.POINTER(_d), _vp],
     "bse_destroy": [_vp],
     "bse_npw_half": [_vp, C.POINTER(_ll)],
     "bse_gvectors": [_vp, _vp],
@@ -112,6 +113,17 @@ def bse_apply_k1(h, a, out, B, ce=1.0, cd=-1.0):
 
 def bse_rotate(h, U, x, y, B, transpose=False):
     _check(lib.bse_rotate(h, _ptr(U), 1 if transpose else 0, _ptr(x), _ptr(y), int(B)), "bse_rotate")
+
+
+def bse_jade(grid, cell, Nv, psi, U, psi_loc=None, tol=1e-14, max_sweeps=60, init_eig=True, stream=None):
+    """Returns (sweeps done, sigma^2 before, sigma^2 after); U (and psi_loc) are written on the device."""
+    g = (_i * 3)(*[int(v) for v in grid])
+    c = (_d * 9)(*[float(v) for v in np.asarray(cell, dtype=np.float64).ravel()])
+    sw = _i()
+    sp = (_d * 2)()
+    _check(lib.bse_jade(g, c, int(Nv), _ptr(psi), _ptr(U), _ptr(psi_loc), float(tol), int(max_sweeps), 1 if init_eig else 0,
+                        C.byref(sw), sp, _ptr(stream)), "bse_jade")
+    return sw.value, sp[0], sp[1]
 
 
 def bse_apply_k1x_host(h, a_host, out_host, B):

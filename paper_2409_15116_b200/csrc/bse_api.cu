@@ -492,9 +492,10 @@ int plan_row_batches(bse_handle *h, int rows_cap) {
 //   acc_r[Bg][rows_cap][N] PW layout: accumulated rows of the current row batch (all Nv rows with BSE_TAU_REAL)
 // A larger row batch re-reads a fewer times and lets rows that share neighbours hit L2, a larger group inverts tau fewer
 // times: 60 % of the free memory goes to the group, the rest to the batch.
-int plan_apply_memory(bse_handle *h, int B) {
+int plan_apply_memory(bse_handle *h, int B, bool allow_slab = true) {
     const bool pw = (h->flags & BSE_VEC_PW) != 0;
     const bool batched = (h->flags & BSE_TAU_MASK) != BSE_TAU_REAL;
+    if (h->plan_ok && h->plan_allow_slab != allow_slab) h->plan_ok = false;
     // the plan is kept only for the very adjacency it was made for (a rebuilt list with the same pair count but other
     // pairs must not reuse the old batches / eslot) and while the group still holds B blocks
     const bool same_list = !batched || (h->plan_adj_ptr_h == h->adj_ptr_h && h->plan_adj_h == h->adj_h);
@@ -502,8 +503,41 @@ int plan_apply_memory(bse_handle *h, int B) {
     cudaFree(h->tau_batch); cudaFree(h->a_r); cudaFree(h->acc_r);
     h->tau_batch = h->a_r = h->acc_r = nullptr;
     h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
+    h->slab_mode = false; h->slab_rc = 0; h->plan_allow_slab = allow_slab;
     size_t free_b = 0, total_b = 0;
     cudaMemGetInfo(&free_b, &total_b);
+    // Plane-slab streaming (PW layout, tau on H): the whole apply runs on one slab of R2 planes at a time, with a(r) of ALL B
+    // blocks and tau(r) of ALL pairs resident for that slab, so every field is inverse-transformed exactly once per call (no
+    // trial-block groups, no pair shared between two row batches).  Taken whenever it fits.
+    if (pw && batched && allow_slab && h->dbg_max_group < 1 && h->dbg_max_batch < 1 && h->dbg_slab_rows >= 0) {
+        const FftPlan &pl = *h->ap;
+        const double SN8 = 8.0 * (double)pl.R2 * pl.n * pl.n;
+        const double avail_s = 0.92 * (double)free_b - 512.0 * 1048576.0;
+        const double fixed = ((double)B * h->Nv + (double)h->P) * SN8;
+        const long long pz = (long long)(((double)h->Pb * h->n * h->fft.NS) / ((double)pl.R2 * pl.NS));
+        long long rc = (long long)((avail_s - fixed) / ((double)B * SN8));
+        rc = std::min<long long>(rc, std::min<long long>(pz / B, 65535 / B));
+        rc = std::min<long long>(rc, std::min<long long>(h->Nv, 256));
+        if (h->dbg_slab_rows >= 1) rc = std::min<long long>(rc, h->dbg_slab_rows);
+        if (rc >= std::min<long long>(h->Nv, 8) || (h->dbg_slab_rows >= 1 && rc >= 1)) {
+            BSE_CUDA(cudaMalloc(&h->a_r, (size_t)((double)B * h->Nv * SN8)));
+            h->a_r_elems = (size_t)((double)B * h->Nv * SN8 / 8.0);
+            BSE_CUDA(cudaMalloc(&h->tau_batch, (size_t)std::max<double>((double)h->P * SN8, 8.0)));
+            BSE_CUDA(cudaMalloc(&h->acc_r, (size_t)((double)B * rc * SN8)));
+            if (!h->rowid) {
+                std::vector<int> ids((size_t)h->Nv);
+                for (int v = 0; v < h->Nv; ++v) ids[v] = v;
+                BSE_CUDA(cudaMalloc(&h->rowid, (size_t)h->Nv * 4));
+                BSE_CUDA(cudaMemcpy(h->rowid, ids.data(), (size_t)h->Nv * 4, cudaMemcpyHostToDevice));
+            }
+            h->slab_mode = true; h->slab_rc = (int)rc; h->slab_pz = pz;
+            h->Bg = B; h->Bg_final = false;
+            h->plan_ok = true;
+            h->plan_adj_ptr_h = h->adj_ptr_h;
+            h->plan_adj_h = h->adj_h;
+            return BSE_OK;
+        }
+    }
     const double N8 = 8.0 * (double)h->ap->N;      // staging lives on the apply grid
     const double avail = 0.92 * (double)free_b - 512.0 * 1048576.0;   // leave the caller some room
     const double avgdeg = std::max(1.0, (double)h->nadj / h->Nv);
@@ -555,6 +589,7 @@ int plan_apply_memory(bse_handle *h, int B) {
     if (pacc) BSE_CUDA(cudaMalloc(&h->tau_batch, (size_t)pacc * h->ap->N * 8));
     if (bg) {
         BSE_CUDA(cudaMalloc(&h->a_r, (size_t)bg * h->Nv * h->ap->N * 8));
+        h->a_r_elems = (size_t)bg * h->Nv * h->ap->N;
         BSE_CUDA(cudaMalloc(&h->acc_r, (size_t)bg * rows_cap * h->ap->N * 8));
     }
     h->Bg = (int)bg; h->Bg_final = bg < B; h->Pacc = pacc; h->rows_cap = (int)rows_cap;
@@ -701,11 +736,53 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
     return BSE_OK;
 }
 
+// PW layout, plane-slab streaming (a9 + a10 + a12 on one slab of planes at a time; see plan_apply_memory and the slab stick
+// kernels of fft_kernels.cuh).  For slab s = { i1 = s + R1 k2 }:  a(G) -> a(r) on the slab for all B blocks, tau(G) -> tau(r)
+// on the slab for all pairs, then chunks of rows: accumulate (eq. 5), forward plane pass, forward slab stick pass that
+// accumulates the slab's share of acc(G) into out.  P_c follows on the finished coefficients.
+int apply_pw_slab(bse_handle *h, const double2 *a, double2 *out, int B) {
+    const FftPlan &pl = *h->ap;
+    const Model m(pl);
+    const int S = pl.R1, M = pl.R2;
+    const long long SN = (long long)M * pl.n * pl.n, npw_h = pl.npw_h, Nv = h->Nv;
+    const double share = (double)M / pl.n;               // one slab's share of a whole-field pass
+    int rc;
+    auto to_slab = [&](const double2 *src, long long fields, double *dst, int s) -> int {
+        for (long long f0 = 0; f0 < fields; f0 += h->slab_pz) {
+            const int cnt = (int)std::min<long long>(h->slab_pz, fields - f0);
+            { StageTimer t(h, BSE_ST_INV_STICK, cnt * m.stick_flops * share, cnt * m.g * share, cnt * m.z * share);
+              if (int r = bse_launch_inv_stick_slab(pl, src + f0 * npw_h, cnt, h->Z, h->stream, s)) return r; }
+            { StageTimer t(h, BSE_ST_INV_PLANE, cnt * m.plane_flops * share, cnt * m.N8 * share, cnt * m.z * share);
+              if (int r = bse_launch_inv_plane(pl, h->Z, cnt, SN, dst + f0 * SN, h->stream, false, M)) return r; }
+        }
+        return BSE_OK;
+    };
+    for (int s = 0; s < S; ++s) {
+        if ((rc = to_slab(a, (long long)B * Nv, h->a_r, s))) return rc;
+        if ((rc = to_slab(h->tau_g, h->P, h->tau_batch, s))) return rc;
+        for (long long v0 = 0; v0 < Nv; v0 += h->slab_rc) {
+            const int rows = (int)std::min<long long>(h->slab_rc, Nv - v0);
+            const double directed = (double)(h->adj_ptr_h[v0 + rows] - h->adj_ptr_h[v0]);
+            { StageTimer t(h, BSE_ST_ACCUM, 2.0 * B * (double)SN * directed,
+                           8.0 * SN * ((double)h->P * rows / Nv + (double)B * rows + (v0 == 0 ? (double)B * Nv : 0.0)));
+              if ((rc = bse_launch_accumulate_rows(h, SN, h->tau_batch, nullptr, h->rowid + v0, rows, h->a_r, h->acc_r, rows, true,
+                                                   B))) return rc; }
+            const int cnt = B * rows;
+            { StageTimer t(h, BSE_ST_FWD_PLANE, cnt * m.plane_flops * share, cnt * m.N8 * share, cnt * m.z * share);
+              if ((rc = bse_launch_fwd_plane(pl, h->acc_r, nullptr, 0, cnt, SN, h->Z, h->stream, M))) return rc; }
+            { StageTimer t(h, BSE_ST_FWD_STICK, cnt * m.stick_flops * share, cnt * m.g * share, cnt * m.z * share);
+              if ((rc = bse_launch_fwd_stick_slab(pl, h->Z, cnt, out, pl.inv2n, h->stream, s, s > 0, rows, Nv, v0))) return rc; }
+        }
+    }
+    return p_c_rows(h, (double *)out, (long long)B * Nv, 2 * npw_h, (const double *)h->uGw, (const double *)h->uG, 1.0);
+}
+
 // PW layout (a12): a, out = [B][Nv][npw_h] complex on H
 int apply_pw(bse_handle *h, const double2 *a, double2 *out, int B) {
     const FftPlan &pl = *h->ap;
     int rc;
     if ((rc = ensure_u_pw(h))) return rc;
+    if (h->slab_mode && !h->mix_on) return apply_pw_slab(h, a, out, B);
     const long long Nv = h->Nv, npw_h = pl.npw_h;
     for (int b0 = 0; b0 < B; b0 += h->Bg) {
         const int nb = std::min(h->Bg, B - b0);
@@ -860,7 +937,7 @@ extern "C" int bse_destroy(bse_handle *h) {
     cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);
     cudaFree(h->part); cudaFree(h->Sov); cudaFree(h->tau_batch); cudaFree(h->a_dev); cudaFree(h->out_dev);
     cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->a_r); cudaFree(h->acc_r);
-    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist); cudaFree(h->k1e_ws); cudaFree(h->u_a); cudaFree(h->Ut); cudaFree(h->accG);
+    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist); cudaFree(h->rowid); cudaFree(h->k1e_ws); cudaFree(h->u_a); cudaFree(h->Ut); cudaFree(h->accG);
     for (cudaEvent_t e : h->ev_pipe) cudaEventDestroy(e);
     if (h->s_in) cudaStreamDestroy(h->s_in);
     if (h->s_out) cudaStreamDestroy(h->s_out);
@@ -991,11 +1068,12 @@ extern "C" int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B)
     if ((rc = ensure_u_apply(h))) return rc;
     const double *ua = h->u_a ? h->u_a : h->u;
     // staging: the K1x plan's buffers when they exist (they took the free memory), else own workspace
-    double *a_r = h->a_r, *dens = (h->tau_batch && h->Pacc >= h->Pb + 1) ? h->tau_batch : nullptr;
+    double *a_r = (h->a_r && h->a_r_elems >= (size_t)Nv * pl.N) ? h->a_r : nullptr;
+    double *dens = (h->tau_batch && h->Pacc >= h->Pb + 1) ? h->tau_batch : nullptr;
     if (!a_r || !dens) {
         if ((rc = ensure_k1e_ws(h, (size_t)((a_r ? 0 : Nv) + (dens ? 0 : 1 + h->Pb)) * pl.N * 8))) return rc;
         // ensure_k1e_ws may have dropped the K1x plan's buffers to make room: look at them again
-        if (a_r && !h->a_r) { a_r = nullptr; dens = nullptr; }
+        if (a_r && !h->a_r) a_r = nullptr;
         if (dens && !h->tau_batch) dens = nullptr;
         if ((rc = ensure_k1e_ws(h, (size_t)((a_r ? 0 : Nv) + (dens ? 0 : 1 + h->Pb)) * pl.N * 8))) return rc;
         double *ws = h->k1e_ws;
@@ -1046,7 +1124,7 @@ extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, 
         if ((rc = ensure_tau_store(h, false))) return rc;
         if ((rc = fill_tau_store(h, false))) return rc;
     }
-    if ((rc = plan_apply_memory(h, B))) return rc;
+    if ((rc = plan_apply_memory(h, B, false))) return rc;    // the combined call keeps the group / row-batch path
     h->mix_ce = ce; h->mix_cd = cd; h->mix_B = B;
     h->mix_u = fly ? nullptr : ((pw && h->u_a) ? h->u_a : h->u);
     if (pw) {
@@ -1167,6 +1245,7 @@ extern "C" int bse_debug_set(bse_handle *h, const char *key, long long value) {
     if (k == "max_group") { h->dbg_max_group = value; h->plan_ok = false; }
     else if (k == "max_batch") { h->dbg_max_batch = value; h->plan_ok = false; }
     else if (k == "compact_inv") { h->fft.compact_inv = h->ffta.compact_inv = (int)value; }
+    else if (k == "slab_rows") { h->dbg_slab_rows = value; h->plan_ok = false; }
     else { bse_set_error("bse_debug_set: unknown key " + k); return BSE_EINVAL; }
     return BSE_OK;
 }

@@ -88,7 +88,15 @@ struct bse_handle {
     bool Bg_final = false, plan_ok = false;
     std::vector<int> plan_adj_h, plan_adj_ptr_h;   // the adjacency the row batches were planned for (exact comparison)
     // debug / test knobs (bse_debug_set; never read from the environment): caps that only ever lower a limit
-    long long dbg_max_group = 0, dbg_max_batch = 0;   // 0 = no cap
+    long long dbg_max_group = 0, dbg_max_batch = 0;   // 0 = no cap; either one set keeps the apply on the group / row-batch path
+    long long dbg_slab_rows = 0;                      // cap of the rows per chunk of the plane-slab apply; -1 = never use it
+    // plane-slab streaming of the PW-layout apply: a_r = [B][Nv][SN], tau_batch = [P][SN],
+    // acc_r = [B][slab_rc][SN], SN = R2 n_a^2 points of the slab { i1 = s + R1 k2 }
+    bool slab_mode = false, plan_allow_slab = true;
+    int slab_rc = 0;                                  // rows per chunk
+    size_t a_r_elems = 0;                             // capacity of a_r in doubles
+    long long slab_pz = 0;                            // slab fields that fit the stick-plane buffer Z
+    int *rowid = nullptr;                             // device [Nv]: rows in the order the chunks take them
     int dbg_compact_inv = -1;                         // -1 = automatic choice of the inverse plane kernel
     long long Pacc = 0;                            // capacity of tau_batch in directed entries                         // Bg is already the most that fits
     // K1e workspaces (grow-only): dens / vH [B][N] (REAL) or one block's a(r) [Nv][Na] + [1][Na] + product rows [Pb][Na] (PW)
@@ -158,7 +166,7 @@ enum { EPI_PARTIAL = 0, EPI_TAU = 1, EPI_SUB = 2, EPI_STORE = 3 };
 // C[M][N] (+)= A[M][K] * B[N][K]^T, split-K partials into `part` then reduced: C = alpha * colscale[n] * sum
 int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb, int M, int N, long long K,
                  bool squareA, bool squareB, double *part, size_t part_bytes, double *C, long long ldc,
-                 double alpha, const double *colscale, cudaStream_t s);
+                 double alpha, const double *colscale, cudaStream_t s, bool accumulate = false);   // accumulate: C += instead of C =
 // NN form: acc = A[M][K] * B[K][N];  EPI_TAU: C = colscale2[n>>1] * (Xin + acc);  EPI_SUB: C = C - acc;  EPI_STORE: C = acc
 int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, int M, long long N, int K,
                 int epi, const double *Xin, const double *colscale2, double *C, long long ldc, cudaStream_t s);

@@ -184,7 +184,7 @@ dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restri
 // C[m][n] = alpha * colscale[n] * sum_z part[z][m][n], fixed order (deterministic)
 __global__ void splitk_reduce_kernel(const double *__restrict__ part, int splits, long long MN, int N,
                                      double *__restrict__ C, long long ldc, double alpha,
-                                     const double *__restrict__ colscale) {
+                                     const double *__restrict__ colscale, int accumulate) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= MN) return;
     double s = 0.0;
@@ -193,7 +193,7 @@ __global__ void splitk_reduce_kernel(const double *__restrict__ part, int splits
     const long long m = i / N;
     const int n = (int)(i - m * N);
     if (colscale) s *= colscale[n];
-    C[m * ldc + n] = s;
+    C[m * ldc + n] = accumulate ? C[m * ldc + n] + s : s;
 }
 
 constexpr int SMEM_DOT = STAGES * (A_TILE + B_TILE_K) * 8;
@@ -211,7 +211,7 @@ int prep(KernelT k, int smem) {
 
 int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb, int M, int N, long long K,
                  bool squareA, bool squareB, double *part, size_t part_bytes, double *C, long long ldc,
-                 double alpha, const double *colscale, cudaStream_t s) {
+                 double alpha, const double *colscale, cudaStream_t s, bool accumulate) {
     if (M <= 0 || N <= 0) return BSE_OK;
     const int tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
     const long long ksteps = (K + BK - 1) / BK;
@@ -249,7 +249,8 @@ int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb,
     }
     BSE_CUDA(cudaGetLastError());
     const long long MN = (long long)M * N;
-    splitk_reduce_kernel<<<(unsigned)((MN + 255) / 256), 256, 0, s>>>(part, (int)splits, MN, N, C, ldc, alpha, colscale);
+    splitk_reduce_kernel<<<(unsigned)((MN + 255) / 256), 256, 0, s>>>(part, (int)splits, MN, N, C, ldc, alpha, colscale,
+                                                                       accumulate ? 1 : 0);
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }

@@ -171,7 +171,8 @@ accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict
     for (int e = ea; e < eb; ++e) {
         const int w = adj[e].x;
         // tau is read once per use: streaming load, so that it does not push the re-used a tiles out of L2
-        const double2 t = __ldcs(reinterpret_cast<const double2 *>(tau_dir + (long long)eslot[e] * N + r));
+        const long long slot = eslot ? eslot[e] : adj[e].y;      // no slot table: the buffer holds tau of every pair, by pair index
+        const double2 t = __ldcs(reinterpret_cast<const double2 *>(tau_dir + slot * N + r));
 #pragma unroll
         for (int b = 0; b < BB; ++b) {
             const double2 x = *reinterpret_cast<const double2 *>(a + ((long long)(b0 + b) * Nv + w) * N + r);

@@ -1,15 +1,23 @@
 """GPU parity at the FULL size of BASELINE.json configs 3, 4 and 5, on sampled outputs the oracle can compute one by one.
 
 The oracle cannot run these configurations in full (its long-double screen alone is N_v^2 N = 4e12 operations at cfg 4-5, one
-pair integral takes ~10 s), so each test checks, against oracle values computed one at a time on the same inputs:
-  * the surviving-pair list restricted to sampled rows v (every w, both orders) - bit-exact, with the S10 guard band asserted
-    on those rows - and the GPU's O rows to 1e-12;
-  * tau_vw(r) for every pair of one complete row v* (the row with the fewest neighbours, >= 3) - 1e-10 relative L2 each;
-  * the K1x output row out[b, v*] for sampled blocks b in the layout the config uses (PW on H for cfg 4-5) - 1e-10;
+pair integral takes ~10 s), so each test checks, against oracle values computed one at a time on the same inputs
+(SURVEY 8(d) / BASELINE.md section 3 "Coverage": >= 4 complete rows and their K1x outputs):
+  * the surviving-pair list restricted to >= 8 sampled rows v (every w, both orders) - bit-exact, with the S10 guard band
+    asserted on those rows - and the GPU's O rows to 1e-12;
+  * tau_vw(r) for EVERY pair of 4 complete rows: the row with the most neighbours (cfg 5: a line-defect centre), the row
+    with the fewest (>= 3), a row of the first row chunk and a row of the last one (cfg 5: index >= 1000, the seeded line of
+    displaced centres) - 1e-10 relative L2 each;
+  * the K1x output rows out[b, v] of those 4 rows: every block b for the smallest row, the first and the last block for the
+    others, in the layout the config uses (PW on H for cfg 4-5) - 1e-10;
   * (cfg 3, 4) one K1e output row (eq. 4) in the PW layout - 1e-10.
+The oracle functions are called as they stand; the harness only spreads independent calls (one pair integral, one
+inverse transform, one projected row, one block of overlap columns) over forked worker processes.
 Inputs come from workloads.make_device (seeded, built on the GPU with torch: input preparation only).
 Launch configuration = the one bench.py uses for that config (tau storage / vector layout per SURVEY.md 8(d) item 7).
 """
+import multiprocessing as mp
+import os
 import time
 
 import numpy as np
@@ -23,6 +31,55 @@ from paper_2409_15116_b200 import workloads as wl         # noqa: E402
 
 TOL = 1e-10
 
+# ---- worker side: plain calls of oracle functions on data the parent put in _G before forking (never touches CUDA) ----
+_G = {}
+
+
+def _limit_threads():
+    try:
+        import threadpoolctl
+        threadpoolctl.threadpool_limits(1)
+    except Exception:
+        pass
+
+
+def _w_tau(vx):
+    v, x = vx
+    return orc.tau_r(_G["tab"], _G["U"][v], _G["U"][x], _G["phiS"], _G["lam"])
+
+
+def _w_to_r(bw):
+    return _G["tab"].to_r(_G["tab"].expand_H_to_S(_G["A"][bw]))
+
+
+def _w_pc_pw(acc):
+    tab = _G["tab"]
+    return orc.S_to_H(tab, orc.p_c_pw(tab, _G["uS"], tab.to_G(acc)))
+
+
+def _w_pc_real(acc):
+    return orc.p_c_real(_G["tab"], _G["U"], acc)
+
+
+def _w_overlap_cols(chunk):
+    """O[rows, chunk] by the oracle's overlap_rows on the orbital subset rows + chunk (O_vw depends on v and w only)."""
+    rows = _G["rows"]
+    sub = list(rows) + [c for c in chunk if c not in rows]
+    U = _G["U"]
+    O = orc.overlap_rows(lambda i: U[sub[i]], len(sub), list(range(len(rows))))
+    pos = {x: i for i, x in enumerate(sub)}
+    return chunk, O[:, [pos[c] for c in chunk]]
+
+
+def _pmap(fn, items, procs):
+    """fn over items in forked workers (the parent's arrays are shared copy-on-write)."""
+    items = list(items)
+    if not items:
+        return []
+    procs = max(1, min(procs, len(items)))
+    with mp.get_context("fork").Pool(procs, initializer=_limit_threads) as pool:
+        return pool.map(fn, items, chunksize=1)
+
 
 def rel(a, b):
     return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / np.linalg.norm(np.asarray(b)))
@@ -34,14 +91,19 @@ def _need_memory(gb):
         pytest.skip(f"needs {gb} GB of free device memory, {free / 1e9:.0f} GB available")
 
 
-def _k1e_row_check(bse, h, w, u_pw_host, row):
+def _pw_err(got, ref, npw_h):
+    wt = np.full(npw_h, 2.0)
+    wt[0] = 1.0
+    return float(np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum()))
+
+
+def _k1e_row_check(bse, h, w, tab, row, a_pw0):
     """K1e (eq. 4) at full size in the PW layout, block 0, one output row against the oracle.  The oracle's PW form needs
     a_v(r) of every orbital by its own FFT (hours at this size), so it is evaluated through its REAL form on
     a(r) = inverse transform of the input coefficients (input preparation, torch) and gathered to H, which pin P16 shows is
     the same thing."""
     Nv, N = w.Nv, w.N
-    tab = orc.Tables(w.n, w.L, w.ecut)
-    a0 = torch.view_as_real(w.a_pw[0:1]).contiguous()
+    a0 = torch.view_as_real(a_pw0[None]).contiguous()
     out0 = torch.empty_like(a0)
     bse.bse_apply_k1e(h, a0, out0, 1)
     torch.cuda.synchronize()
@@ -49,22 +111,21 @@ def _k1e_row_check(bse, h, w, u_pw_host, row):
     tabs = _scatter_tables(w)
     n_r = np.zeros(N)
     for v0 in range(0, Nv, 16):
-        ar = _to_real(w, w.a_pw[0, v0:v0 + 16], tabs)
-        n_r += np.einsum("vr,vr->r", w.u[v0:v0 + 16].cpu().numpy(), ar.cpu().numpy())      # sum_v u_v a_v, in numpy
+        ar = _to_real(w, a_pw0[v0:v0 + 16], tabs)
+        n_r += np.einsum("vr,vr->r", _G["U"][v0:v0 + 16], ar.cpu().numpy())      # sum_v u_v a_v, in numpy
     vH = orc.hartree_r(tab, n_r)
-    uS = tab.expand_H_to_S(u_pw_host)
-    ref = orc.S_to_H(tab, orc.p_c_pw(tab, uS, tab.to_G(2.0 * w.u[row].cpu().numpy() * vH)))
-    wt = np.full(tab.npw_h, 2.0)
-    wt[0] = 1.0
-    e = float(np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum()))
+    ref = orc.S_to_H(tab, orc.p_c_pw(tab, _G["uS"], tab.to_G(2.0 * _G["U"][row] * vH)))
+    e = _pw_err(got, ref, tab.npw_h)
     assert e <= TOL, e
     return e
 
 
-def _sampled_full_check(cfg_id, tau_flag, vec_pw, screen_rows, blocks, need_gb, k1e_row=None):
+def _sampled_full_check(cfg_id, tau_flag, vec_pw, need_gb, k1e_row=None, procs_tau=8, procs_fft=12):
     from paper_2409_15116_b200 import bse
     _need_memory(need_gb)
     t0 = time.time()
+    ncpu = os.cpu_count() or 4
+    procs_tau, procs_fft = min(procs_tau, ncpu), min(procs_fft, ncpu)
     w = wl.make_device(cfg_id, "cuda:0")
     u_pw_host = w.u_pw.cpu().numpy()
     w.u_pw = None                                           # not an input of the library: free its device copy
@@ -86,13 +147,44 @@ def _sampled_full_check(cfg_id, tau_flag, vec_pw, screen_rows, blocks, need_gb, 
             nbr[v].append(x)
             if x != v:
                 nbr[x].append(v)
+        deg = np.array([len(x) for x in nbr])
         print(f"\ncfg{cfg_id}: generated in {time.time() - t0:.0f} s, P = {P} of {Nv * (Nv + 1) // 2} "
-              f"({100.0 * (P - Nv) / (Nv * (Nv - 1) // 2):.2f} % of off-diagonal pairs kept)")
+              f"({100.0 * (P - Nv) / (Nv * (Nv - 1) // 2):.2f} % of off-diagonal pairs kept), degree {deg.min()}..{deg.max()}")
 
-        # ---- a1: screen on sampled rows, oracle rows computed one (v, w) at a time in long double
-        def get_u(v):
-            return w.u[v].cpu().numpy()
-        Or = orc.overlap_rows(get_u, Nv, screen_rows)
+        # ---- the sample: 4 complete rows + 4 more rows for the list
+        v_max = int(np.argmax(deg))
+        if cfg_id == 5:                                     # the line-defect centres are the last 24 orbitals
+            v_max = 1000 + int(np.argmax(deg[1000:]))
+        cand = [v for v in range(Nv) if deg[v] >= 3]
+        v_min = min(cand, key=lambda v: (deg[v], v))
+        rows4 = []
+        for v in (v_max, v_min, 1, Nv - 1, 2, Nv - 2, 3):
+            if v not in rows4 and len(rows4) < 4:
+                rows4.append(v)
+        rng = np.random.default_rng(1000 + cfg_id)
+        screen_rows = list(rows4)
+        for v in rng.permutation(Nv).tolist():
+            if len(screen_rows) >= 8:
+                break
+            if v not in screen_rows:
+                screen_rows.append(v)
+
+        # ---- host copies the workers read (set before any fork)
+        U = w.u.cpu().numpy()
+        tab = orc.Tables(w.n, w.L, w.ecut)
+        phi_host = w.phi.cpu().numpy()
+        _G.clear()
+        _G.update(tab=tab, U=U, lam=w.lam, rows=screen_rows, phiS=tab.expand_H_to_S(phi_host),
+                  uS=tab.expand_H_to_S(u_pw_host))
+        del phi_host
+        assert rel(_G["uS"][v_min], tab.to_G(U[v_min])) < 1e-12          # the generator's coefficients = the oracle's own transform
+
+        # ---- a1: screen on the sampled rows, oracle rows in long double, columns spread over workers
+        t1 = time.time()
+        chunks = [list(range(c0, min(c0 + 16, Nv))) for c0 in range(0, Nv, 16)]
+        Or = np.empty((len(screen_rows), Nv))
+        for chunk, blockO in _pmap(_w_overlap_cols, chunks, procs_fft):
+            Or[:, chunk] = blockO
         O_gpu = bse.bse_get_overlap(h, Nv)
         for i, v in enumerate(screen_rows):
             off = np.arange(Nv) != v
@@ -100,21 +192,23 @@ def _sampled_full_check(cfg_id, tau_flag, vec_pw, screen_rows, blocks, need_gb, 
             ref = sorted(x for x in range(Nv) if x == v or Or[i, x] >= w.eta)
             assert sorted(nbr[v]) == ref, f"pair list differs from the oracle on row {v}"
             assert np.abs(O_gpu[v] - Or[i]).max() < 1e-12
+        print(f"cfg{cfg_id}: pair list bit-exact on rows {screen_rows} ({time.time() - t1:.0f} s)")
 
+        a_pw = w.a_pw
         if k1e_row is not None:
-            e1 = _k1e_row_check(bse, h, w, u_pw_host, k1e_row)
+            e1 = _k1e_row_check(bse, h, w, tab, k1e_row, a_pw[0])
             print(f"cfg{cfg_id}: K1e row {k1e_row}, block 0: error {e1:.2e}")
             torch.cuda.empty_cache()
 
         # ---- apply on the GPU
         if vec_pw:
-            a_d = torch.view_as_real(w.a_pw).contiguous()
+            a_d = torch.view_as_real(a_pw).contiguous()
         else:
             a_d = torch.empty((B, Nv, N), dtype=torch.float64, device="cuda:0")
             tabs = _scatter_tables(w)
             for b in range(B):
                 for v0 in range(0, Nv, 16):
-                    a_d[b, v0:v0 + 16] = _to_real(w, w.a_pw[b, v0:v0 + 16], tabs)
+                    a_d[b, v0:v0 + 16] = _to_real(w, a_pw[b, v0:v0 + 16], tabs)
         out = torch.empty_like(a_d)
         torch.cuda.empty_cache()
         try:
@@ -125,43 +219,50 @@ def _sampled_full_check(cfg_id, tau_flag, vec_pw, screen_rows, blocks, need_gb, 
             raise
         torch.cuda.synchronize()
 
-        # ---- one complete row v*: tau of each of its pairs, then the K1x output row for sampled blocks
-        cand = [v for v in range(Nv) if len(nbr[v]) >= 3]
-        vs = min(cand, key=lambda v: (len(nbr[v]), v))
-        tab = orc.Tables(w.n, w.L, w.ecut)
-        phiS = tab.expand_H_to_S(w.phi.cpu().numpy())
-        u_vs = get_u(vs)
-        acc = {b: np.zeros(N) for b in blocks}
+        # ---- tau of every pair of the 4 complete rows
+        t2 = time.time()
+        keys = sorted({(min(v, x), max(v, x)) for v in rows4 for x in nbr[v]})
+        tau_ref = dict(zip(keys, _pmap(_w_tau, keys, procs_tau)))
         dst = torch.empty((1, N), dtype=torch.float64, device="cuda:0")
         worst = 0.0
-        for x in sorted(nbr[vs]):
-            t_ref = orc.tau_r(tab, u_vs, get_u(x), phiS, w.lam)
-            bse.bse_get_tau(h, index[(min(vs, x), max(vs, x))], 1, dst, bse.BSE_TAU_REAL)
+        for key in keys:
+            bse.bse_get_tau(h, index[key], 1, dst, bse.BSE_TAU_REAL)
             torch.cuda.synchronize()
-            e = rel(dst[0].cpu().numpy(), t_ref)
+            e = rel(dst[0].cpu().numpy(), tau_ref[key])
             worst = max(worst, e)
-            assert e <= TOL, (vs, x, e)
-            for b in blocks:
-                acc[b] += t_ref * tab.to_r(tab.expand_H_to_S(w.a_pw[b, x].cpu().numpy()))
-        uS = tab.expand_H_to_S(u_pw_host)      # the generator's coefficients of the same orbitals ...
-        assert rel(uS[vs], tab.to_G(u_vs)) < 1e-12          # ... which are what the oracle's own transform gives
-        errs = []
-        for b in blocks:
+            assert e <= TOL, (key, e)
+        print(f"cfg{cfg_id}: tau of all {len(keys)} pairs of rows {rows4} (degrees {[int(deg[v]) for v in rows4]}): "
+              f"worst error {worst:.2e} ({time.time() - t2:.0f} s)")
+
+        # ---- their K1x output rows: every block for the smallest row, first and last block for the others
+        t3 = time.time()
+        blocks = {v: (list(range(B)) if v == v_min else sorted({0, B - 1})) for v in rows4}
+        need = sorted({(b, x) for v in rows4 for b in blocks[v] for x in nbr[v]})
+        _G["A"] = {bw: a_pw[bw[0], bw[1]].cpu().numpy() for bw in need}
+        a_r = dict(zip(need, _pmap(_w_to_r, need, procs_fft)))
+        jobs, accs = [], []
+        for v in rows4:
+            for b in blocks[v]:
+                acc = np.zeros(N)
+                for x in nbr[v]:
+                    acc += tau_ref[(min(v, x), max(v, x))] * a_r[(b, x)]
+                jobs.append((v, b))
+                accs.append(acc)
+        del a_r
+        refs = _pmap(_w_pc_pw if vec_pw else _w_pc_real, accs, procs_tau)
+        errs = {}
+        for (v, b), ref in zip(jobs, refs):
             if vec_pw:
-                ref = orc.S_to_H(tab, orc.p_c_pw(tab, uS, tab.to_G(acc[b])))
-                got = torch.view_as_complex(out[b, vs]).cpu().numpy()
-                wt = np.full(npw_h, 2.0)
-                wt[0] = 1.0
-                e = float(np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum()))
+                e = _pw_err(torch.view_as_complex(out[b, v]).cpu().numpy(), ref, npw_h)
             else:
-                ref = orc.p_c_real(tab, w.u.cpu().numpy(), acc[b])
-                e = rel(out[b, vs].cpu().numpy(), ref)
-            errs.append(e)
-            assert e <= TOL, (b, e)
-        print(f"cfg{cfg_id}: row v* = {vs} with {len(nbr[vs])} neighbours; worst tau error {worst:.2e}; "
-              f"K1x row errors {['%.2e' % e for e in errs]}; total {time.time() - t0:.0f} s")
+                e = rel(out[b, v].cpu().numpy(), ref)
+            errs[(v, b)] = e
+            assert e <= TOL, (v, b, e)
+        print(f"cfg{cfg_id}: {len(jobs)} K1x output rows (rows {rows4}; all {B} blocks for row {v_min}): worst error "
+              f"{max(errs.values()):.2e} ({time.time() - t3:.0f} s); total {time.time() - t0:.0f} s")
     finally:
         bse.bse_destroy(h)
+        _G.clear()
         del w
         torch.cuda.empty_cache()
 
@@ -186,19 +287,19 @@ def _to_real(w, cH, tabs):
 
 def test_cfg3_full_size_real_layout():
     from paper_2409_15116_b200 import bse
-    _sampled_full_check(3, bse.BSE_TAU_PW, False, screen_rows=[3, 101, 255], blocks=[0, 7], need_gb=60)
+    _sampled_full_check(3, bse.BSE_TAU_PW, False, need_gb=60)
 
 
 def test_cfg3_full_size_pw_layout():
     from paper_2409_15116_b200 import bse
-    _sampled_full_check(3, bse.BSE_TAU_PW, True, screen_rows=[17], blocks=[5], need_gb=40, k1e_row=200)
+    _sampled_full_check(3, bse.BSE_TAU_PW, True, need_gb=40, k1e_row=200)
 
 
 def test_cfg4_full_size():
     from paper_2409_15116_b200 import bse
-    _sampled_full_check(4, bse.BSE_TAU_PW, True, screen_rows=[777], blocks=[7], need_gb=120, k1e_row=513)
+    _sampled_full_check(4, bse.BSE_TAU_PW, True, need_gb=120, k1e_row=513)
 
 
 def test_cfg5_full_size_streamed():
     from paper_2409_15116_b200 import bse
-    _sampled_full_check(5, bse.BSE_TAU_STREAM, True, screen_rows=[1010], blocks=[15], need_gb=150)
+    _sampled_full_check(5, bse.BSE_TAU_STREAM, True, need_gb=150, procs_tau=6)

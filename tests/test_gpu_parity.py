@@ -66,7 +66,7 @@ class Gpu:
         self.bse.bse_destroy(self.h)
 
 
-def _check_full(w, flags=0, check_g=True, knobs=None):
+def _check_full(w, flags=0, check_g=True, knobs=None, tau_ref=None):
     tab = orc.Tables(w.n, w.L, w.ecut)
     pairs_ref, O = orc.screen_pairs(w.u, w.eta)
     assert orc.screen_margin(O, w.eta) > 1e-9, "workload violates the screen guard band (S10)"
@@ -77,7 +77,8 @@ def _check_full(w, flags=0, check_g=True, knobs=None):
         assert pairs.dtype == np.int32 and np.array_equal(pairs, pairs_ref)          # bit-exact list
         O_gpu = g.bse.bse_get_overlap(g.h, w.Nv)
         assert np.abs(O_gpu - O).max() < 1e-12
-        tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs_ref, want="r")
+        if tau_ref is None:
+            tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs_ref, want="r")
         tau = g.tau_r(0, len(pairs))
         assert rel(tau, tau_ref) <= TOL
         worst = max(rel(tau[p], tau_ref[p]) for p in range(len(pairs)))
@@ -180,44 +181,28 @@ def test_cfg2_reduced_full_check():
         _check_full(w, flags, check_g=(flags == 0))
 
 
-def _sampled_check(w, n_pairs, rows, flags=0):
-    """Full-size config: bit-exact list; tau on sampled pairs; K1x on sampled rows v (all blocks)."""
-    tab = orc.Tables(w.n, w.L, w.ecut)
-    pairs_ref, O = orc.screen_pairs(w.u, w.eta)
-    assert orc.screen_margin(O, w.eta) > 1e-9
-    g = Gpu(w, flags)
-    try:
-        pairs = g.build()
-        assert np.array_equal(pairs, pairs_ref)
-        P = len(pairs)
-        rng = np.random.default_rng(5)
-        sample = sorted(set(rng.choice(P, size=min(n_pairs, P), replace=False).tolist()) | {0, P - 1})
-        phiS = tab.expand_H_to_S(w.phi)
-        for p in sample:
-            v, x = pairs[p]
-            ref = orc.tau_r(tab, w.u[v], w.u[x], phiS, w.lam)
-            assert rel(g.tau_r(p, 1)[0], ref) <= TOL
-        a = w.a_real()
-        out = g.apply(a)
-        index = {(int(v), int(x)): p for p, (v, x) in enumerate(pairs)}
-        for v in rows:
-            acc = np.zeros((a.shape[0], tab.N))
-            for x in range(w.Nv):
-                key = (min(v, x), max(v, x))
-                if key in index:
-                    t = orc.tau_r(tab, w.u[key[0]], w.u[key[1]], phiS, w.lam)
-                    acc += t[None, :] * a[:, x, :]
-            ref = np.array([orc.p_c_real(tab, w.u, acc[b]) for b in range(a.shape[0])])
-            assert rel(out[:, v, :], ref) <= TOL
-        return P
-    finally:
-        g.close()
+_W2 = {}
 
 
-def test_cfg2_full_size_sampled():
+def _w_tau_pair(vx):
+    return orc.tau_r(_W2["tab"], _W2["u"][vx[0]], _W2["u"][vx[1]], _W2["phiS"], _W2["lam"])
+
+
+def test_cfg2_full_size_in_full():
+    """BASELINE config 2 at full size IN FULL: the whole list, all 234 tau, all 64 x 4 output rows.  The oracle's pair integrals
+    (independent calls of orc.tau_r, as it stands) are spread over forked worker processes by the harness."""
+    import multiprocessing as mp
+    import os
     w = wl.make(2)
-    P = _sampled_check(w, n_pairs=6, rows=[0, 37])
-    assert 64 <= P < 2080
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    pairs_ref, _ = orc.screen_pairs(w.u, w.eta)
+    assert 64 <= len(pairs_ref) < 2080
+    _W2.update(tab=tab, u=w.u, phiS=tab.expand_H_to_S(w.phi), lam=w.lam)
+    with mp.get_context("fork").Pool(min(12, os.cpu_count() or 4)) as pool:
+        tau_ref = np.array(pool.map(_w_tau_pair, [(int(v), int(x)) for v, x in pairs_ref], chunksize=4))
+    _W2.clear()
+    _check_full(w, 0, check_g=False, tau_ref=tau_ref)
+    _check_full(w, _bse().BSE_TAU_PW, check_g=False, tau_ref=tau_ref)
 
 
 def test_error_paths():
@@ -545,3 +530,19 @@ def test_compact_inverse_kernel_subtract_epilogue():
     o1 = _check_full(w, check_g=False, knobs={"compact_inv": 2})
     o0 = _check_full(w, check_g=False, knobs={"compact_inv": 0})
     assert rel(o1, o0) < 1e-12
+
+
+def test_plane_slab_apply_matches_the_group_path():
+    """PW layout with tau on H: the plane-slab streaming apply (default: one slab of planes at a time, all blocks and all
+    pairs resident, slab stick passes) against the oracle, with ragged row chunks, and against the group / row-batch path
+    it replaces (knob slab_rows = -1).  Grids 24 = 4 x 6 (apply grid 20 = 5 x 4 or 24), 30 = 5 x 6 and 12 = 3 x 4."""
+    bse = _bse()
+    for cfg in (wl.Config("slab", 10.0, 24, 9, 20, 8.0, 1.2, 0.8, 3.0, 0.02, 5, "random", seed=77),
+                wl.Config("slab", 14.0, 30, 7, 16, 5.0, 1.3, 0.8, 3.0, 0.0, 3, "random", seed=311),
+                wl.Config("slab", 9.0, 12, 5, 7, 3.0, 1.3, 0.8, 3.0, 0.05, 2, "random", seed=112)):
+        w = wl.make(cfg=cfg)
+        for tau in (bse.BSE_TAU_PW, bse.BSE_TAU_STREAM):
+            o_def = _check_pw(w, tau)
+            o_rag = _check_pw(w, tau, {"slab_rows": 4})
+            o_old = _check_pw(w, tau, {"slab_rows": -1})
+            assert rel(o_rag, o_def) < 1e-13 and rel(o_old, o_def) < 1e-12
