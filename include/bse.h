@@ -109,6 +109,26 @@ int bse_rotate(bse_handle *h, const double *U, int transpose, const double *x, d
 int bse_jade(const int grid[3], const double cell[9], int Nv, const double *psi, double *U, double *psi_loc,
              double tol, int max_sweeps, int init_eig, int *sweeps, double *spread, void *stream);
 
+/* Row-sharded operation (PAPER.md:156 and Fig. 2: "we distributed the N_occ orbitals across band groups, using a
+ * block distribution scheme"): this handle owns the output rows [v0, v1) of every trial block.  Call before bse_build_tau, which
+ * then keeps tau only for the pairs (v, v') that touch an owned row (a pair that straddles two owners is built by both);
+ * bse_apply_k1x takes the FULL trial blocks a [B][Nv][Npw_h] (after the all-gather of PAPER.md:156) and writes the owned rows
+ * only, out [B][v1 - v0][Npw_h].  u (replicated) and P_c are unchanged.  Needs BSE_VEC_PW with BSE_TAU_PW / BSE_TAU_STREAM
+ * (BSE_EUNSUPPORTED otherwise); (0, Nv) restores the unsharded behaviour.  bse_num_pairs / bse_get_pairs still describe the whole
+ * list.  paper_2409_15116_b200/sharded.py drives one such handle per rank with torch.distributed. */
+int bse_set_rows(bse_handle *h, int v0, int v1);
+
+/* K1e on a row-sharded trial block (eq. 4 sums over all occupied states inside the integral; "communications
+ * between band groups are required only when a summation over occupied states is carried out").  PW layout only.
+ *   bse_k1e_hartree_partial: vG[b](G) = v_c(G) sum_{v in [v0,v1)} [u_v a_bv](G) on H, from the rows this rank holds
+ *       a_rows DEVICE [B][v1-v0][Npw_h] complex;  vG DEVICE [B][Npw_h] complex (written)
+ *   the caller sums vG over the ranks (an all-reduce of B * Npw_h coefficients), then
+ *   bse_k1e_from_hartree:    out_rows[b, v-v0] = P_c [ 2 u_v v_H[b] ], v_H[b] the potential with coefficients vG[b]
+ *       out_rows DEVICE [B][v1-v0][Npw_h] complex (written)
+ * With (v0, v1) = (0, Nv) the two calls together are bse_apply_k1e. */
+int bse_k1e_hartree_partial(bse_handle *h, const double *a_rows, int v0, int v1, int B, double *vG);
+int bse_k1e_from_hartree(bse_handle *h, const double *vG, int v0, int v1, int B, double *out_rows);
+
 /* Same with HOST pointers: copies a to the device, applies, copies out back, synchronises (the end-to-end
  * call bench.py times as `e2e`).  With BSE_TAU_REAL the blocks are pipelined: block b+1 is copied in and block b-1
  * copied out (two copy streams) while block b is applied.  Pinned host memory is needed for the overlap. */
@@ -137,7 +157,7 @@ int bse_get_tau(bse_handle *h, long long first, long long count, double *dst, un
  * layout, "max_batch" caps the pairs of one row batch (so that small cases exercise the multi-group / multi-batch paths of
  * the large configurations; 0 = no cap);  "compact_inv" = k forces the compact inverse plane kernel sized for k CTAs per SM
  * (0 = never, -1 = automatic);  "slab_rows" = k caps the rows per chunk of the plane-slab apply (PW layout with tau on H; -1 = never
- * take that path, 0 = no cap); setting "max_group" or "max_batch" also keeps the apply on the group / row-batch path.
+ * take that path, 0 = no cap), "slab_planes" = k the planes per slab; setting "max_group" or "max_batch" also keeps the apply on the group / row-batch path.
  * BSE_EINVAL for an unknown key. */
 int bse_debug_set(bse_handle *h, const char *key, long long value);
 /* Per-stage device time (CUDA events on the library's stream).  enable != 0 switches recording on (adds a

@@ -45,6 +45,9 @@ _sig = {
     "bse_get_overlap": [_vp, _vp],
     "bse_get_tau": [_vp, _ll, _ll, _vp, _u],
     "bse_debug_set": [_vp, C.c_char_p, _ll],
+    "bse_set_rows": [_vp, _i, _i],
+    "bse_k1e_hartree_partial": [_vp, _vp, _i, _i, _i, _vp],
+    "bse_k1e_from_hartree": [_vp, _vp, _i, _i, _i, _vp],
     "bse_last_tau_fill_ms": [_vp, C.POINTER(_d)],
     "bse_profile_enable": [_vp, _i],
     "bse_profile_reset": [_vp],
@@ -170,6 +173,18 @@ def bse_get_overlap(h, Nv):
 
 def bse_get_tau(h, first, count, dst, layout=BSE_TAU_REAL):
     _check(lib.bse_get_tau(h, int(first), int(count), _ptr(dst), int(layout)), "bse_get_tau")
+
+
+def bse_set_rows(h, v0, v1):
+    _check(lib.bse_set_rows(h, int(v0), int(v1)), "bse_set_rows")
+
+
+def bse_k1e_hartree_partial(h, a_rows, v0, v1, B, vG):
+    _check(lib.bse_k1e_hartree_partial(h, _ptr(a_rows), int(v0), int(v1), int(B), _ptr(vG)), "bse_k1e_hartree_partial")
+
+
+def bse_k1e_from_hartree(h, vG, v0, v1, B, out_rows):
+    _check(lib.bse_k1e_from_hartree(h, _ptr(vG), int(v0), int(v1), int(B), _ptr(out_rows)), "bse_k1e_from_hartree")
 
 
 def bse_debug_set(h, key, value):

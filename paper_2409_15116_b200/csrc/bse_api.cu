@@ -215,11 +215,11 @@ int st_accumulate(bse_handle *h, const double *tau, long long p0, long long cnt,
 }
 
 // tau for pairs [p0, p0+cnt): a2..a8 into dstG ([cnt][npw_h] complex), then a9 into dstR ([cnt][N]) if given
-int run_pair_batch(bse_handle *h, long long p0, int cnt, double2 *dstG, double *dstR) {
+int run_pair_batch(bse_handle *h, const int2 *plist, long long p0, int cnt, double2 *dstG, double *dstR) {
     const FftPlan &pl = h->fft;
     const long long K2 = 2 * pl.npw_h;
     int rc;
-    if ((rc = st_fwd_plane(h, pl, h->u, h->pairs, p0, cnt))) return rc;
+    if ((rc = st_fwd_plane(h, pl, h->u, plist, p0, cnt))) return rc;
     if ((rc = st_fwd_stick(h, pl, cnt, h->X, pl.vc12n))) return rc;
     if ((rc = st_gemm_dot(h, BSE_ST_PROJECT, (const double *)h->X, K2, h->phi, K2, cnt, h->Npdep, K2, false, h->Dm,
                           ldD(h), 1.0, h->f2))) return rc;
@@ -385,7 +385,7 @@ int alloc_batch_ws(bse_handle *h, long long pb) {
 // tau store of the REAL / PW modes (grow-only); BSE_TAU_STREAM uses the PW store as a transient that is refilled inside
 // every apply call (tau(G) is 16 N / N_pw_h ~ 16x smaller than tau(r), which stays streamed in batches)
 int ensure_tau_store(bse_handle *h, bool real) {
-    const size_t need = real ? (size_t)h->P * h->N * 8 : (size_t)h->P * h->fft.npw_h * 16;
+    const size_t need = real ? (size_t)h->Pa * h->N * 8 : (size_t)h->Pa * h->fft.npw_h * 16;
     if (need <= h->tau_bytes && (real ? h->tau_r != nullptr : h->tau_g != nullptr)) return BSE_OK;
     cudaFree(h->tau_r); h->tau_r = nullptr;
     cudaFree(h->tau_g); h->tau_g = nullptr;
@@ -408,10 +408,11 @@ int ensure_tau_store(bse_handle *h, bool real) {
 int fill_tau_store(bse_handle *h, bool real) {
     int rc;
     cudaEventRecord(h->ev_fill0, h->stream);        // device time of the pair integrals alone (bse_last_tau_fill_ms)
-    for (long long p0 = 0; p0 < h->P; p0 += h->Pb) {
-        const int cnt = (int)std::min<long long>(h->Pb, h->P - p0);
-        if (real) rc = run_pair_batch(h, p0, cnt, h->T, h->tau_r + p0 * h->N);
-        else rc = run_pair_batch(h, p0, cnt, h->tau_g + p0 * h->fft.npw_h, nullptr);
+    const int2 *plist = h->rows_set ? h->pairs_act : h->pairs;       // row-sharded: only the pairs that touch an owned row
+    for (long long p0 = 0; p0 < h->Pa; p0 += h->Pb) {
+        const int cnt = (int)std::min<long long>(h->Pb, h->Pa - p0);
+        if (real) rc = run_pair_batch(h, plist, p0, cnt, h->T, h->tau_r + p0 * h->N);
+        else rc = run_pair_batch(h, plist, p0, cnt, h->tau_g + p0 * h->fft.npw_h, nullptr);
         if (rc) return rc;
     }
     cudaEventRecord(h->ev_fill1, h->stream);
@@ -511,18 +512,32 @@ int plan_apply_memory(bse_handle *h, int B, bool allow_slab = true) {
     // trial-block groups, no pair shared between two row batches).  Taken whenever it fits.
     if (pw && batched && allow_slab && h->dbg_max_group < 1 && h->dbg_max_batch < 1 && h->dbg_slab_rows >= 0) {
         const FftPlan &pl = *h->ap;
-        const double SN8 = 8.0 * (double)pl.R2 * pl.n * pl.n;
         const double avail_s = 0.92 * (double)free_b - 512.0 * 1048576.0;
-        const double fixed = ((double)B * h->Nv + (double)h->P) * SN8;
-        const long long pz = (long long)(((double)h->Pb * h->n * h->fft.NS) / ((double)pl.R2 * pl.NS));
-        long long rc = (long long)((avail_s - fixed) / ((double)B * SN8));
-        rc = std::min<long long>(rc, std::min<long long>(pz / B, 65535 / B));
-        rc = std::min<long long>(rc, std::min<long long>(h->Nv, 256));
-        if (h->dbg_slab_rows >= 1) rc = std::min<long long>(rc, h->dbg_slab_rows);
-        if (rc >= std::min<long long>(h->Nv, 8) || (h->dbg_slab_rows >= 1 && rc >= 1)) {
+        // the slab split n_a = S * M (any factorisation with M <= 32, fft_kernels.cuh): the fewest slabs whose working set fits,
+        // because every slab sweeps all coefficient arrays once.  dbg_slab_planes caps M (tests: several slabs on small grids).
+        long long rc = 0, pz = 0;
+        int Ssel = 0, Msel = 0;
+        double SN8 = 0.0;
+        for (int M = std::min(pl.n, 32); M >= 1; --M) {
+            if (pl.n % M || pl.n / M > 16) continue;           // the slab stick kernels keep <= 16 folded terms per thread
+            if (h->dbg_slab_planes >= 1 && M > h->dbg_slab_planes) continue;
+            SN8 = 8.0 * (double)M * pl.n * pl.n;
+            const double fixed = ((double)B * h->Nv + (double)h->Pa) * SN8;
+            pz = (long long)(((double)h->Pb * h->n * h->fft.NS) / ((double)M * pl.NS));
+            rc = (long long)((avail_s - fixed) / ((double)B * SN8));
+            rc = std::min<long long>(rc, std::min<long long>(pz / B, 65535 / B));
+            rc = std::min<long long>(rc, std::min<long long>(h->Nv, 256));
+            if (h->dbg_slab_rows >= 1) rc = std::min<long long>(rc, h->dbg_slab_rows);
+            if (rc >= std::min<long long>(h->Nv, 32) || (h->dbg_slab_rows >= 1 && rc >= 1) || (M == 1 && rc >= 1)) {
+                Ssel = pl.n / M; Msel = M;
+                break;
+            }
+            rc = 0;
+        }
+        if (Msel >= 1 && rc >= 1) {
             BSE_CUDA(cudaMalloc(&h->a_r, (size_t)((double)B * h->Nv * SN8)));
             h->a_r_elems = (size_t)((double)B * h->Nv * SN8 / 8.0);
-            BSE_CUDA(cudaMalloc(&h->tau_batch, (size_t)std::max<double>((double)h->P * SN8, 8.0)));
+            BSE_CUDA(cudaMalloc(&h->tau_batch, (size_t)std::max<double>((double)h->Pa * SN8, 8.0)));
             BSE_CUDA(cudaMalloc(&h->acc_r, (size_t)((double)B * rc * SN8)));
             if (!h->rowid) {
                 std::vector<int> ids((size_t)h->Nv);
@@ -530,7 +545,7 @@ int plan_apply_memory(bse_handle *h, int B, bool allow_slab = true) {
                 BSE_CUDA(cudaMalloc(&h->rowid, (size_t)h->Nv * 4));
                 BSE_CUDA(cudaMemcpy(h->rowid, ids.data(), (size_t)h->Nv * 4, cudaMemcpyHostToDevice));
             }
-            h->slab_mode = true; h->slab_rc = (int)rc; h->slab_pz = pz;
+            h->slab_mode = true; h->slab_rc = (int)rc; h->slab_pz = pz; h->slab_S = Ssel; h->slab_M = Msel;
             h->Bg = B; h->Bg_final = false;
             h->plan_ok = true;
             h->plan_adj_ptr_h = h->adj_ptr_h;
@@ -743,15 +758,16 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
 int apply_pw_slab(bse_handle *h, const double2 *a, double2 *out, int B) {
     const FftPlan &pl = *h->ap;
     const Model m(pl);
-    const int S = pl.R1, M = pl.R2;
+    const int S = h->slab_S, M = h->slab_M;
     const long long SN = (long long)M * pl.n * pl.n, npw_h = pl.npw_h, Nv = h->Nv;
     const double share = (double)M / pl.n;               // one slab's share of a whole-field pass
+    const long long nloc = h->row1 - h->row0;            // out holds the owned rows only: [B][nloc][npw_h]
     int rc;
     auto to_slab = [&](const double2 *src, long long fields, double *dst, int s) -> int {
         for (long long f0 = 0; f0 < fields; f0 += h->slab_pz) {
             const int cnt = (int)std::min<long long>(h->slab_pz, fields - f0);
             { StageTimer t(h, BSE_ST_INV_STICK, cnt * m.stick_flops * share, cnt * m.g * share, cnt * m.z * share);
-              if (int r = bse_launch_inv_stick_slab(pl, src + f0 * npw_h, cnt, h->Z, h->stream, s)) return r; }
+              if (int r = bse_launch_inv_stick_slab(pl, S, M, src + f0 * npw_h, cnt, h->Z, h->stream, s)) return r; }
             { StageTimer t(h, BSE_ST_INV_PLANE, cnt * m.plane_flops * share, cnt * m.N8 * share, cnt * m.z * share);
               if (int r = bse_launch_inv_plane(pl, h->Z, cnt, SN, dst + f0 * SN, h->stream, false, M)) return r; }
         }
@@ -759,22 +775,22 @@ int apply_pw_slab(bse_handle *h, const double2 *a, double2 *out, int B) {
     };
     for (int s = 0; s < S; ++s) {
         if ((rc = to_slab(a, (long long)B * Nv, h->a_r, s))) return rc;
-        if ((rc = to_slab(h->tau_g, h->P, h->tau_batch, s))) return rc;
-        for (long long v0 = 0; v0 < Nv; v0 += h->slab_rc) {
-            const int rows = (int)std::min<long long>(h->slab_rc, Nv - v0);
+        if ((rc = to_slab(h->tau_g, h->Pa, h->tau_batch, s))) return rc;
+        for (long long v0 = h->row0; v0 < h->row1; v0 += h->slab_rc) {       // the owned rows (all of them unless bse_set_rows)
+            const int rows = (int)std::min<long long>(h->slab_rc, h->row1 - v0);
             const double directed = (double)(h->adj_ptr_h[v0 + rows] - h->adj_ptr_h[v0]);
             { StageTimer t(h, BSE_ST_ACCUM, 2.0 * B * (double)SN * directed,
-                           8.0 * SN * ((double)h->P * rows / Nv + (double)B * rows + (v0 == 0 ? (double)B * Nv : 0.0)));
-              if ((rc = bse_launch_accumulate_rows(h, SN, h->tau_batch, nullptr, h->rowid + v0, rows, h->a_r, h->acc_r, rows, true,
-                                                   B))) return rc; }
+                           8.0 * SN * ((double)h->Pa * rows / nloc + (double)B * rows + (v0 == h->row0 ? (double)B * Nv : 0.0)));
+              if ((rc = bse_launch_accumulate_rows(h, SN, h->tau_batch, h->eslot_act, h->rowid + v0, rows, h->a_r, h->acc_r, rows,
+                                                   true, B))) return rc; }
             const int cnt = B * rows;
             { StageTimer t(h, BSE_ST_FWD_PLANE, cnt * m.plane_flops * share, cnt * m.N8 * share, cnt * m.z * share);
               if ((rc = bse_launch_fwd_plane(pl, h->acc_r, nullptr, 0, cnt, SN, h->Z, h->stream, M))) return rc; }
             { StageTimer t(h, BSE_ST_FWD_STICK, cnt * m.stick_flops * share, cnt * m.g * share, cnt * m.z * share);
-              if ((rc = bse_launch_fwd_stick_slab(pl, h->Z, cnt, out, pl.inv2n, h->stream, s, s > 0, rows, Nv, v0))) return rc; }
+              if ((rc = bse_launch_fwd_stick_slab(pl, S, M, h->Z, cnt, out, pl.inv2n, h->stream, s, s > 0, rows, nloc, v0 - h->row0))) return rc; }
         }
     }
-    return p_c_rows(h, (double *)out, (long long)B * Nv, 2 * npw_h, (const double *)h->uGw, (const double *)h->uG, 1.0);
+    return p_c_rows(h, (double *)out, (long long)B * nloc, 2 * npw_h, (const double *)h->uGw, (const double *)h->uG, 1.0);
 }
 
 // PW layout (a12): a, out = [B][Nv][npw_h] complex on H
@@ -783,6 +799,7 @@ int apply_pw(bse_handle *h, const double2 *a, double2 *out, int B) {
     int rc;
     if ((rc = ensure_u_pw(h))) return rc;
     if (h->slab_mode && !h->mix_on) return apply_pw_slab(h, a, out, B);
+    if (h->rows_set) { bse_set_error("row-sharded apply needs the plane-slab path (PW layout, tau on H, enough memory)"); return BSE_EUNSUPPORTED; }
     const long long Nv = h->Nv, npw_h = pl.npw_h;
     for (int b0 = 0; b0 < B; b0 += h->Bg) {
         const int nb = std::min(h->Bg, B - b0);
@@ -855,6 +872,7 @@ extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cel
     h->N = (long long)h->n * h->n * h->n;
     h->L = L; h->Omega = L * L * L; h->dV = h->Omega / (double)h->N;
     h->ecut = ecut; h->eta = eta; h->Nv = Nv; h->Npdep = Npdep; h->flags = flags;
+    h->row0 = 0; h->row1 = Nv;
     h->stream = (cudaStream_t)stream;
     h->msq_max = (int)std::floor(2.0 * ecut * (L / (2.0 * M_PI)) * (L / (2.0 * M_PI)) * (1.0 + 1e-12));
     const int R = (int)std::floor(std::sqrt((double)h->msq_max) + 1e-9);
@@ -937,7 +955,7 @@ extern "C" int bse_destroy(bse_handle *h) {
     cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);
     cudaFree(h->part); cudaFree(h->Sov); cudaFree(h->tau_batch); cudaFree(h->a_dev); cudaFree(h->out_dev);
     cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->a_r); cudaFree(h->acc_r);
-    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist); cudaFree(h->rowid); cudaFree(h->k1e_ws); cudaFree(h->u_a); cudaFree(h->Ut); cudaFree(h->accG);
+    cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist); cudaFree(h->rowid); cudaFree(h->pairs_act); cudaFree(h->eslot_act); cudaFree(h->k1e_ws); cudaFree(h->u_a); cudaFree(h->Ut); cudaFree(h->accG);
     for (cudaEvent_t e : h->ev_pipe) cudaEventDestroy(e);
     if (h->s_in) cudaStreamDestroy(h->s_in);
     if (h->s_out) cudaStreamDestroy(h->s_out);
@@ -946,6 +964,23 @@ extern "C" int bse_destroy(bse_handle *h) {
     if (h->ev_fill0) cudaEventDestroy(h->ev_fill0);
     if (h->ev_fill1) cudaEventDestroy(h->ev_fill1);
     delete h;
+    return BSE_OK;
+}
+
+// Row-sharded operation (Fig. 2: the N_occ orbitals of A_s block-distributed over band groups):
+// this handle owns the output rows [v0, v1).  bse_build_tau then keeps tau only for the pairs that touch an owned row, and
+// bse_apply_k1x takes the FULL (all-gathered) trial blocks a [B][Nv][.] and writes the owned rows out [B][v1 - v0][.].
+extern "C" int bse_set_rows(bse_handle *h, int v0, int v1) {
+    if (!h) { bse_set_error("null handle"); return BSE_EINVAL; }
+    if (v0 < 0 || v1 > h->Nv || v0 >= v1) { bse_set_error("bse_set_rows: need 0 <= v0 < v1 <= Nv"); return BSE_EINVAL; }
+    if (!(h->flags & BSE_VEC_PW) || (h->flags & BSE_TAU_MASK) == BSE_TAU_REAL) {
+        bse_set_error("bse_set_rows needs BSE_VEC_PW with BSE_TAU_PW or BSE_TAU_STREAM");
+        return BSE_EUNSUPPORTED;
+    }
+    h->row0 = v0; h->row1 = v1;
+    h->rows_set = !(v0 == 0 && v1 == h->Nv);
+    h->built = false;
+    h->plan_ok = false;
     return BSE_OK;
 }
 
@@ -1103,6 +1138,66 @@ extern "C" int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B)
     return p_c_rows(h, (double *)out, (long long)B * Nv, 2 * npw_h, (const double *)h->uGw, (const double *)h->uG, 1.0);
 }
 
+// ---- K1e split for the row-sharded operation.  eq. 4 sums over ALL occupied states inside the integral:
+// each rank forms the Hartree potential of its own rows' share of the transition density, the shares are summed over the ranks
+// (an all-reduce of B * N_pw_h coefficients - "communications between band groups are required only when a summation over
+// occupied states is carried out"), and every rank finishes its own rows.  PW layout only.
+//   vG[b](G) = v_c(G) * sum_{v in [v0, v1)} [u_v a_bv](G)  on H        a_rows: [B][v1 - v0][npw_h] (the owned rows of each block)
+extern "C" int bse_k1e_hartree_partial(bse_handle *h, const double *a_rows, int v0, int v1, int B, double *vG) {
+    if (!h || !a_rows || !vG || B <= 0 || v0 < 0 || v1 > h->Nv || v0 >= v1) { bse_set_error("bad argument"); return BSE_EINVAL; }
+    if (!(h->flags & BSE_VEC_PW)) { bse_set_error("bse_k1e_hartree_partial needs BSE_VEC_PW"); return BSE_EUNSUPPORTED; }
+    const FftPlan &pl = *h->ap;
+    const long long npw_h = pl.npw_h, nloc = v1 - v0;
+    const double N8 = 8.0 * (double)pl.N;
+    int rc;
+    if ((rc = ensure_u_pw(h))) return rc;
+    if ((rc = ensure_u_apply(h))) return rc;
+    const double *ua = h->u_a ? h->u_a : h->u;
+    if ((rc = ensure_k1e_ws(h, (size_t)(h->Pb + 1) * pl.N * 8))) return rc;
+    double *dens = h->k1e_ws, *chunk = h->k1e_ws + pl.N;
+    const double2 *ag = (const double2 *)a_rows;
+    for (int b = 0; b < B; ++b) {
+        for (long long c0 = 0; c0 < nloc; c0 += h->Pb) {
+            const int cnt = (int)std::min<long long>(h->Pb, nloc - c0);
+            if ((rc = st_inv_stick(h, pl, ag + ((long long)b * nloc + c0) * npw_h, cnt))) return rc;
+            if ((rc = st_inv_plane(h, pl, cnt, chunk))) return rc;
+            StageTimer t(h, BSE_ST_K1E_DENSITY, 2.0 * cnt * (double)pl.N, N8 * (2.0 * cnt + 1));
+            if ((rc = bse_launch_k1e_density(ua + (v0 + c0) * pl.N, chunk, dens, cnt, pl.N, 1, h->stream, 0, cnt, c0 > 0))) return rc;
+        }
+        if ((rc = st_fwd_plane(h, pl, dens, nullptr, 0, 1))) return rc;
+        if ((rc = st_fwd_stick(h, pl, 1, (double2 *)vG + (long long)b * npw_h, pl.vcn))) return rc;
+    }
+    return BSE_OK;
+}
+
+//   out_rows[b, v - v0] = P_c [ 2 u_v v_H[b] ] truncated to S,  v_H[b](r) = sum_{G in S} vG[b](G) e^{iG.r}   (vG summed over the ranks)
+extern "C" int bse_k1e_from_hartree(bse_handle *h, const double *vG, int v0, int v1, int B, double *out_rows) {
+    if (!h || !vG || !out_rows || B <= 0 || v0 < 0 || v1 > h->Nv || v0 >= v1) { bse_set_error("bad argument"); return BSE_EINVAL; }
+    if (!(h->flags & BSE_VEC_PW)) { bse_set_error("bse_k1e_from_hartree needs BSE_VEC_PW"); return BSE_EUNSUPPORTED; }
+    const FftPlan &pl = *h->ap;
+    const long long npw_h = pl.npw_h, nloc = v1 - v0;
+    const double N8 = 8.0 * (double)pl.N;
+    int rc;
+    if ((rc = ensure_u_pw(h))) return rc;
+    if ((rc = ensure_u_apply(h))) return rc;
+    const double *ua = h->u_a ? h->u_a : h->u;
+    if ((rc = ensure_k1e_ws(h, (size_t)(h->Pb + 1) * pl.N * 8))) return rc;
+    double *vH = h->k1e_ws, *prod = h->k1e_ws + pl.N;
+    double2 *og = (double2 *)out_rows;
+    for (int b = 0; b < B; ++b) {
+        if ((rc = st_inv_stick(h, pl, (const double2 *)vG + (long long)b * npw_h, 1))) return rc;
+        if ((rc = st_inv_plane(h, pl, 1, vH))) return rc;
+        for (long long c0 = 0; c0 < nloc; c0 += h->Pb) {
+            const int cnt = (int)std::min<long long>(h->Pb, nloc - c0);
+            { StageTimer t(h, BSE_ST_K1E_PRODUCT, 2.0 * cnt * (double)pl.N, N8 * (2.0 * cnt + 1));
+              if ((rc = bse_launch_k1e_product(ua, vH, prod, (int)(v0 + c0), cnt, h->Pb, pl.N, 1, h->stream))) return rc; }
+            if ((rc = st_fwd_plane(h, pl, prod, nullptr, 0, cnt))) return rc;
+            if ((rc = st_fwd_stick(h, pl, cnt, og + ((long long)b * nloc + c0) * npw_h, pl.inv2n))) return rc;
+        }
+    }
+    return p_c_rows(h, out_rows, (long long)B * nloc, 2 * npw_h, (const double *)h->uGw, (const double *)h->uG, 1.0);
+}
+
 // Two-body kernel in one call (eq. 1: K1e and K1d enter with one P_c): out = P_c( ce * 2 u_v v_H + cd * sum_v' tau_vv' a_v' )
 extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, double ce, double cd) {
     if (!h || !a || !out || B <= 0) { bse_set_error("null pointer or B <= 0"); return BSE_EINVAL; }
@@ -1124,6 +1219,7 @@ extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, 
         if ((rc = ensure_tau_store(h, false))) return rc;
         if ((rc = fill_tau_store(h, false))) return rc;
     }
+    if (h->rows_set) { bse_set_error("bse_apply_k1 is not available on a row-sharded handle"); return BSE_EUNSUPPORTED; }
     if ((rc = plan_apply_memory(h, B, false))) return rc;    // the combined call keeps the group / row-batch path
     h->mix_ce = ce; h->mix_cd = cd; h->mix_B = B;
     h->mix_u = fly ? nullptr : ((pw && h->u_a) ? h->u_a : h->u);
@@ -1218,11 +1314,11 @@ extern "C" int bse_get_tau(bse_handle *h, long long first, long long count, doub
     if (first + count > h->P) { bse_set_error("pair range out of bounds"); return BSE_EINVAL; }
     const unsigned mode = h->flags & BSE_TAU_MASK;
     const long long npw_h = h->fft.npw_h;
-    if (layout == BSE_TAU_REAL && mode == BSE_TAU_REAL) {
+    if (layout == BSE_TAU_REAL && mode == BSE_TAU_REAL && !h->rows_set) {
         BSE_CUDA(cudaMemcpyAsync(dst, h->tau_r + first * h->N, (size_t)count * h->N * 8, cudaMemcpyDeviceToDevice, h->stream));
         return BSE_OK;
     }
-    if (layout == BSE_TAU_PW && mode == BSE_TAU_PW) {
+    if (layout == BSE_TAU_PW && mode == BSE_TAU_PW && !h->rows_set) {
         BSE_CUDA(cudaMemcpyAsync(dst, h->tau_g + first * npw_h, (size_t)count * npw_h * 16, cudaMemcpyDeviceToDevice, h->stream));
         return BSE_OK;
     }
@@ -1231,8 +1327,8 @@ extern "C" int bse_get_tau(bse_handle *h, long long first, long long count, doub
     int rc;
     for (long long p0 = first; p0 < first + count; p0 += h->Pb) {
         const int cnt = (int)std::min<long long>(h->Pb, first + count - p0);
-        if (layout == BSE_TAU_PW) rc = run_pair_batch(h, p0, cnt, (double2 *)dst + (p0 - first) * npw_h, nullptr);
-        else rc = run_pair_batch(h, p0, cnt, h->T, dst + (p0 - first) * h->N);
+        if (layout == BSE_TAU_PW) rc = run_pair_batch(h, h->pairs, p0, cnt, (double2 *)dst + (p0 - first) * npw_h, nullptr);
+        else rc = run_pair_batch(h, h->pairs, p0, cnt, h->T, dst + (p0 - first) * h->N);
         if (rc) return rc;
     }
     return BSE_OK;
@@ -1246,6 +1342,7 @@ extern "C" int bse_debug_set(bse_handle *h, const char *key, long long value) {
     else if (k == "max_batch") { h->dbg_max_batch = value; h->plan_ok = false; }
     else if (k == "compact_inv") { h->fft.compact_inv = h->ffta.compact_inv = (int)value; }
     else if (k == "slab_rows") { h->dbg_slab_rows = value; h->plan_ok = false; }
+    else if (k == "slab_planes") { h->dbg_slab_planes = value; h->plan_ok = false; }
     else { bse_set_error("bse_debug_set: unknown key " + k); return BSE_EINVAL; }
     return BSE_OK;
 }

@@ -66,6 +66,13 @@ struct bse_handle {
     double uniq_share = 1.0;         // P / (sum of nu): share of the inverted fields that is algorithmic work
     std::vector<int> adj_ptr_h;      // host copy of adj_ptr (row batches of the batched tau modes)
     bool built = false;
+    // row-sharded operation (bse_set_rows): this handle owns the output rows [row0, row1); the tau store then
+    // holds only the Pa pairs that touch one of them (pairs_act, ascending pair index; eslot_act[e] = slot of directed entry e)
+    int row0 = 0, row1 = 0;                // row1 = Nv when unrestricted
+    bool rows_set = false;
+    long long Pa = 0;                      // pairs in the tau store (= P when unrestricted)
+    int2 *pairs_act = nullptr;             // device [Pa] (restricted only; else the store follows `pairs`)
+    int *eslot_act = nullptr;              // device [nadj] (restricted only)
     // tau store
     double *tau_r = nullptr;         // [P][N]
     double2 *tau_g = nullptr;        // [P][npw_h]
@@ -89,11 +96,13 @@ struct bse_handle {
     std::vector<int> plan_adj_h, plan_adj_ptr_h;   // the adjacency the row batches were planned for (exact comparison)
     // debug / test knobs (bse_debug_set; never read from the environment): caps that only ever lower a limit
     long long dbg_max_group = 0, dbg_max_batch = 0;   // 0 = no cap; either one set keeps the apply on the group / row-batch path
+    long long dbg_slab_planes = 0;                    // cap of the planes per slab (0 = no cap)
     long long dbg_slab_rows = 0;                      // cap of the rows per chunk of the plane-slab apply; -1 = never use it
     // plane-slab streaming of the PW-layout apply: a_r = [B][Nv][SN], tau_batch = [P][SN],
     // acc_r = [B][slab_rc][SN], SN = R2 n_a^2 points of the slab { i1 = s + R1 k2 }
     bool slab_mode = false, plan_allow_slab = true;
     int slab_rc = 0;                                  // rows per chunk
+    int slab_S = 0, slab_M = 0;                       // the slab split n_a = S * M chosen by the plan (fewest slabs that fit)
     size_t a_r_elems = 0;                             // capacity of a_r in doubles
     long long slab_pz = 0;                            // slab fields that fit the stick-plane buffer Z
     int *rowid = nullptr;                             // device [Nv]: rows in the order the chunks take them
@@ -154,12 +163,12 @@ int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2
 // subtract: out <- out - transform instead of out <- transform (P_c update of the REAL layout)
 int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long long N, double *out, cudaStream_t s,
                          bool subtract = false, int np = 0);
-// slab forms of the stick passes (fft_kernels.cuh): the planes i1 = slab + R1 k2, k2 < R2, only.  Zs[count][R2][NS].
+// slab forms of the stick passes (fft_kernels.cuh): the planes i1 = slab + S k, k < M, only (n = S M, M <= 32).  Zs[count][M][NS].
 // forward: field p goes to row (p / rc) * row_ld + row0 + p % rc of X; accumulate: X += (slabs 1 .. R1-1) instead of X =
-int bse_launch_inv_stick_slab(const FftPlan &pl, const double2 *T, int count, double2 *Zs, cudaStream_t s, int slab,
+int bse_launch_inv_stick_slab(const FftPlan &pl, int S, int M, const double2 *T, int count, double2 *Zs, cudaStream_t s, int slab,
                               const int *gather = nullptr, int g0 = 0);
-int bse_launch_fwd_stick_slab(const FftPlan &pl, const double2 *Zs, int count, double2 *X, const double *scale, cudaStream_t s,
-                              int slab, bool accumulate, int rc, long long row_ld, long long row0);
+int bse_launch_fwd_stick_slab(const FftPlan &pl, int S, int M, const double2 *Zs, int count, double2 *X, const double *scale,
+                              cudaStream_t s, int slab, bool accumulate, int rc, long long row_ld, long long row0);
 
 // gemm_dmma.cu
 enum { EPI_PARTIAL = 0, EPI_TAU = 1, EPI_SUB = 2, EPI_STORE = 3 };

@@ -1,6 +1,9 @@
 // Size dispatch of the two-pass FFT kernels (fft_kernels.cuh).  Each supported grid edge n = R1 * R2 is instantiated in
 // one of the fft_sizes_*.cu translation units (compiled in parallel); this file holds the table and the launch wrappers.
+#include <algorithm>
+
 #include "fft_kernels.cuh"
+#include "fft_slab.cuh"
 
 namespace bsefft {
 FftOps ops_12(); FftOps ops_16(); FftOps ops_20(); FftOps ops_24(); FftOps ops_30(); FftOps ops_32(); FftOps ops_36();
@@ -50,16 +53,51 @@ int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long lo
     if (count <= 0) return BSE_OK;
     return ((const FftOps *)pl.ops)->inv_plane(to_dev(pl, np), Z, count, N, out, s, subtract ? 1 : 0, pl.compact_inv);
 }
-int bse_launch_inv_stick_slab(const FftPlan &pl, const double2 *T, int count, double2 *Zs, cudaStream_t s, int slab,
+// slab stick passes: any factorisation n = S * M with M <= 32 (fft_slab.cuh); M = A * B with A the largest divisor <= sqrt(M)
+static int slab_split(int M) {
+    int A = 1;
+    for (int a = 1; a * a <= M; ++a)
+        if (M % a == 0) A = a;
+    return A;
+}
+// the fields of a launch are spread over the CTAs of a stick group so that the grid holds ~8 CTAs per SM
+static int slab_per_cta(int groups, int count) {
+    const int want = std::max(1, (148 * 8 + groups - 1) / groups);      // field chunks per stick group
+    return std::max(1, (count + want - 1) / want);
+}
+int bse_launch_inv_stick_slab(const FftPlan &pl, int S, int M, const double2 *T, int count, double2 *Zs, cudaStream_t s, int slab,
                               const int *gather, int g0) {
     if (count <= 0) return BSE_OK;
-    return ((const FftOps *)pl.ops)->inv_stick_slab(to_dev(pl), T, count, pl.npw_h, Zs, s, gather, g0, slab);
+    if (S * M != pl.n || M > 32 || M < 1 || S > 16) { bse_set_error("slab stick pass: bad factorisation"); return BSE_EINVAL; }
+    const PlanDev P = to_dev(pl);
+    const int TS = bsefft::SLAB_TS, A = slab_split(M), groups = (pl.NS + TS - 1) / TS;
+    const int smem = 2 * M * (TS + 1) * 16;
+    const int per = slab_per_cta(groups, count);
+    const dim3 grid(groups, (count + per - 1) / per);
+    const bool small = TS * M <= 512;
+#define BSE_SLAB_PICK(name) \
+    (small ? (S <= 4 ? bsefft::name<4, 512> : (S <= 8 ? bsefft::name<8, 512> : (S <= 12 ? bsefft::name<12, 512> : bsefft::name<16, 512>))) \
+           : (S <= 4 ? bsefft::name<4, 1024> : (S <= 8 ? bsefft::name<8, 1024> : (S <= 12 ? bsefft::name<12, 1024> : bsefft::name<16, 1024>))))
+    auto kern = BSE_SLAB_PICK(inv_stick_slab_kernel);
+    kern<<<grid, TS * M, smem, s>>>(P, pl.n, S, M, A, T, pl.npw_h, Zs, gather, g0, slab, count, per);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
 }
-int bse_launch_fwd_stick_slab(const FftPlan &pl, const double2 *Zs, int count, double2 *X, const double *scale, cudaStream_t s,
-                              int slab, bool accumulate, int rc, long long row_ld, long long row0) {
+int bse_launch_fwd_stick_slab(const FftPlan &pl, int S, int M, const double2 *Zs, int count, double2 *X, const double *scale,
+                              cudaStream_t s, int slab, bool accumulate, int rc_rows, long long row_ld, long long row0) {
     if (count <= 0) return BSE_OK;
-    return ((const FftOps *)pl.ops)->fwd_stick_slab(to_dev(pl), Zs, count, X, pl.npw_h, scale, s, slab, accumulate ? 1 : 0, rc,
-                                                    row_ld, row0);
+    if (S * M != pl.n || M > 32 || M < 1 || S > 16) { bse_set_error("slab stick pass: bad factorisation"); return BSE_EINVAL; }
+    const PlanDev P = to_dev(pl);
+    const int TS = bsefft::SLAB_TS, A = slab_split(M), groups = (pl.NS + TS - 1) / TS;
+    const int smem = 2 * M * (TS + 1) * 16;
+    const int per = 1;          // one field per CTA: the read-modify-writes of many short CTAs overlap better than a walk
+    const dim3 grid(groups, (count + per - 1) / per);
+    const bool small = TS * M <= 512;
+    auto kern = BSE_SLAB_PICK(fwd_stick_slab_kernel);
+    kern<<<grid, TS * M, smem, s>>>(P, pl.n, S, M, A, Zs, X, pl.npw_h, scale, slab, accumulate ? 1 : 0, rc_rows, row_ld, row0,
+                                    count, per);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
 }
 int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2 *X, const double *scale,
                          cudaStream_t s, const int *scatter) {

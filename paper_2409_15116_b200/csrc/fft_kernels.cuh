@@ -495,95 +495,6 @@ inv_stick_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, doub
 
 
 // ---------------------------------------------------------------------------------------------------------
-// SLAB stick passes (plane-slab streaming of the PW-layout apply).  A product tau(r) a(r) is local in
-// r, so the apply may run on one subset of the i1 planes at a time; with the slab s = { i1 = s + R1 k2 : k2 < R2 } the 1-D
-// transform along i1 splits exactly (one decimation step of the same n = R1 R2 factorisation):
-//   inverse:  x[s + R1 k2] = sum_{j < R2} e^{+2 pi i k2 j / R2}  y_s[j],    y_s[j] = sum_{q < R1} X[j + q R2] e^{+2 pi i s (j + q R2) / n}
-//   forward:  X[t1] = sum_s e^{-2 pi i s t1 / n}  Y_s[t1 mod R2],          Y_s[j] = sum_{k2 < R2} x[s + R1 k2] e^{-2 pi i k2 j / R2}
-// so every slab costs one fold over the (at most 2R+1) non-zero coefficients of a stick plus one R2-point transform, all slabs
-// together one full transform plus R1 sweeps over the coefficients on H, and the forward pass ACCUMULATES its slab's
-// contribution into X (slab 0 stores).  One thread = one stick of one field; Zs[p][k2][NS].
-template <int R1, int R2>
-__global__ void __launch_bounds__(128)
-inv_stick_slab_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, double2 *__restrict__ Zs,
-                      const int *__restrict__ gather, int g0, int slab) {
-    using G = Geo<R1, R2>;
-    constexpr int n = G::n;
-    const int NS = P.NS, R = P.R;
-    const int sidx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (sidx >= NS) return;
-    const long long p = blockIdx.y;
-    const double2 *tg = T + (gather ? (long long)gather[g0 + p] : p) * npw_h;
-    double2 y[R2];
-#pragma unroll
-    for (int j = 0; j < R2; ++j) y[j] = make_double2(0.0, 0.0);
-    int ti = 0;                                   // (slab * t1) mod n
-#pragma unroll
-    for (int q = 0; q < R1; ++q) {
-#pragma unroll
-        for (int j = 0; j < R2; ++j) {
-            const int t1 = j + q * R2;            // compile-time after unrolling
-            if (t1 <= R || t1 >= n - R) {         // |m1| <= R: everything else is outside the sphere
-                const int code = P.hmapT[t1 * NS + sidx];
-                if (code != -1) {
-                    double2 v;
-                    if (code >= 0) v = tg[code];
-                    else { v = tg[-2 - code]; v.y = -v.y; }
-                    const double2 w = P.tw[ti];   // e^{-2 pi i slab t1 / n}: the inverse pass needs its conjugate
-                    y[j].x += v.x * w.x + v.y * w.y;
-                    y[j].y += v.y * w.x - v.x * w.y;
-                }
-            }
-            ti += slab;
-            if (ti >= n) ti -= n;
-        }
-    }
-    Dft<R2, +1>::run(y);
-    double2 *z = Zs + p * R2 * (long long)NS + sidx;
-#pragma unroll
-    for (int k2 = 0; k2 < R2; ++k2) z[(long long)k2 * NS] = y[k2];
-}
-
-// field p of the launch goes to row  (p / rc) * row_ld + row0 + (p % rc)  of X (the rows of a chunk, block after block)
-template <int R1, int R2>
-__global__ void __launch_bounds__(128)
-fwd_stick_slab_kernel(PlanDev P, const double2 *__restrict__ Zs, double2 *__restrict__ X, long long npw_h,
-                      const double *__restrict__ scale, int slab, int accumulate, int rc, long long row_ld, long long row0) {
-    using G = Geo<R1, R2>;
-    constexpr int n = G::n;
-    const int NS = P.NS, R = P.R;
-    const int sidx = blockIdx.x * blockDim.x + threadIdx.x;
-    if (sidx >= NS) return;
-    const long long p = blockIdx.y;
-    const double2 *z = Zs + p * R2 * (long long)NS + sidx;
-    double2 y[R2];
-#pragma unroll
-    for (int k2 = 0; k2 < R2; ++k2) y[k2] = z[(long long)k2 * NS];
-    Dft<R2, -1>::run(y);
-    double2 *xo = X + ((p / rc) * row_ld + row0 + (p % rc)) * npw_h;
-    int ti = 0;
-#pragma unroll
-    for (int q = 0; q < R1; ++q) {
-#pragma unroll
-        for (int j = 0; j < R2; ++j) {
-            const int t1 = j + q * R2;
-            if (t1 <= R || t1 >= n - R) {
-                const int hh = P.hmapT[t1 * NS + sidx];
-                if (hh >= 0) {
-                    const double2 w = P.tw[ti];   // e^{-2 pi i slab t1 / n}
-                    const double sc = scale[hh];
-                    double2 v = make_double2((y[j].x * w.x - y[j].y * w.y) * sc, (y[j].x * w.y + y[j].y * w.x) * sc);
-                    if (accumulate) { const double2 o = xo[hh]; v.x += o.x; v.y += o.y; }
-                    xo[hh] = v;
-                }
-            }
-            ti += slab;
-            if (ti >= n) ti -= n;
-        }
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------
 // host launchers for one factorisation; collected in a table by fft_kernels.cu
 struct FftOps {
     int n, R1, R2, plane_smem;
@@ -591,9 +502,6 @@ struct FftOps {
     int (*inv_plane)(const PlanDev &, const double2 *, int, long long, double *, cudaStream_t, int, int);
     int (*fwd_stick)(const PlanDev &, const double2 *, int, double2 *, long long, const double *, cudaStream_t, const int *);
     int (*inv_stick)(const PlanDev &, const double2 *, int, long long, double2 *, cudaStream_t, const int *, int);
-    int (*inv_stick_slab)(const PlanDev &, const double2 *, int, long long, double2 *, cudaStream_t, const int *, int, int);
-    int (*fwd_stick_slab)(const PlanDev &, const double2 *, int, double2 *, long long, const double *, cudaStream_t, int, int,
-                          int, long long, long long);
 };
 
 inline int plane_threads(int tasks) {
@@ -685,29 +593,8 @@ struct Launch {
         BSE_CUDA(cudaGetLastError());
         return BSE_OK;
     }
-    static int inv_stick_slab(const PlanDev &P, const double2 *T, int count, long long npw_h, double2 *Zs, cudaStream_t s,
-                              const int *gather, int g0, int slab) {
-        for (int c0 = 0; c0 < count; c0 += 65535) {
-            const int c = count - c0 < 65535 ? count - c0 : 65535;
-            inv_stick_slab_kernel<R1, R2><<<dim3((P.NS + 127) / 128, c), 128, 0, s>>>(
-                P, gather ? T : T + (long long)c0 * npw_h, npw_h, Zs + (long long)c0 * R2 * P.NS, gather, g0 + c0, slab);
-        }
-        BSE_CUDA(cudaGetLastError());
-        return BSE_OK;
-    }
-    static int fwd_stick_slab(const PlanDev &P, const double2 *Zs, int count, double2 *X, long long npw_h, const double *scale,
-                              cudaStream_t s, int slab, int accumulate, int rc, long long row_ld, long long row0) {
-        if (count > 65535 * 1) {                  // fields are addressed through (p / rc, p % rc): one launch only
-            bse_set_error("fwd_stick_slab: more than 65535 fields in one launch");
-            return BSE_EINVAL;
-        }
-        fwd_stick_slab_kernel<R1, R2><<<dim3((P.NS + 127) / 128, count), 128, 0, s>>>(P, Zs, X, npw_h, scale, slab, accumulate,
-                                                                                     rc, row_ld, row0);
-        BSE_CUDA(cudaGetLastError());
-        return BSE_OK;
-    }
     static FftOps ops() {
-        return FftOps{G::n, R1, R2, G::plane_smem, fwd_plane, inv_plane, fwd_stick, inv_stick, inv_stick_slab, fwd_stick_slab};
+        return FftOps{G::n, R1, R2, G::plane_smem, fwd_plane, inv_plane, fwd_stick, inv_stick};
     }
 };
 

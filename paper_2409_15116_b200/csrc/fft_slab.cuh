@@ -1,0 +1,178 @@
+// Slab forms of the stick passes (included by fft_kernels.cu only: the kernels are not templates).
+#pragma once
+#include "fft_kernels.cuh"
+
+namespace bsefft {
+
+// ---------------------------------------------------------------------------------------------------------
+// SLAB stick passes (plane-slab streaming of the PW-layout apply).  A product tau(r) a(r) is local in
+// r, so the apply may run on one subset of the i1 planes at a time; for ANY factorisation n = S M the slab
+// s = { i1 = s + S k : k < M } splits the 1-D transform along i1 exactly (one decimation step):
+//   inverse:  x[s + S k] = sum_{j < M} e^{+2 pi i k j / M}  y_s[j],    y_s[j] = sum_{q < S} X[j + q M] e^{+2 pi i s (j + q M) / n}
+//   forward:  X[t1] = sum_s e^{-2 pi i s t1 / n}  Y_s[t1 mod M],      Y_s[j] = sum_{k < M} x[s + S k] e^{-2 pi i k j / M}
+// so every slab costs one fold over the (at most 2R+1) non-zero coefficients of a stick plus one M-point transform, all
+// slabs together S sweeps over the coefficients on H, and the forward pass ACCUMULATES its slab's contribution into X (slab 0
+// stores).  The host picks the smallest S whose slab fits the free memory (fewest sweeps).  Zs[p][k][NS].
+// CTA = TS sticks of one field, TS * M threads (M <= 32): thread (j, stick) folds residue class j (<= S stick-coalesced
+// gathers, four in flight at a time).  The M-point transform runs out of shared memory as two passes of the split
+// M = A B (A + B terms per thread instead of M), input index j = j1 B + j2, output index k = k1 + A k2:
+//   z[k1][j2] = w_M^{k1 j2} sum_{j1 < A} y[j1 B + j2] w_A^{k1 j1},      x[k1 + A k2] = sum_{j2 < B} z[k1][j2] w_B^{k2 j2}
+// with every root taken from the table tw[t] = e^{-2 pi i t / n} (A | M | n), conjugated for the inverse.
+// dynamic smem: C[M][TS + 1] | D[M][TS + 1]
+constexpr int SLAB_TS = 32;
+
+// v * w (SIGN < 0, forward) or v * conj(w) (SIGN > 0, inverse)
+template <int SIGN>
+__device__ __forceinline__ double2 cmul_s(double2 v, double2 w) {
+    return SIGN < 0 ? make_double2(v.x * w.x - v.y * w.y, v.x * w.y + v.y * w.x)
+                    : make_double2(v.x * w.x + v.y * w.y, v.y * w.x - v.x * w.y);
+}
+
+// M-point transform of the TS sticks held in C[j][stick]; thread t (< M) of lane sl returns the value of index
+// k = k1 + A k2, k1 = t / B, k2 = t % B.  D is the second buffer; contains one __syncthreads (every thread must call) and
+// expects C complete (a barrier) on entry.
+template <int SIGN>
+__device__ __forceinline__ double2 slab_dft(const double2 *C, double2 *D, const double2 *__restrict__ tw, int n, int M, int A,
+                                            int B, int t, int sl, int &k_out) {
+    constexpr int LDT = SLAB_TS + 1;
+    const int k1 = t / B, r2 = t - k1 * B;                      // pass 1: (k1, j2 = r2); pass 2: (k1, k2 = r2)
+    double2 z = make_double2(0.0, 0.0);
+    {
+        int wi = 0;                                             // (k1 j1 mod A) * (n / A)
+        const int wstep = k1 * (n / A);
+        const double2 *c = C + r2 * LDT + sl;
+        for (int j1 = 0; j1 < A; ++j1) {
+            const double2 p = cmul_s<SIGN>(c[j1 * B * LDT], tw[wi]);
+            z.x += p.x;
+            z.y += p.y;
+            wi += wstep;
+            if (wi >= n) wi -= n;
+        }
+        z = cmul_s<SIGN>(z, tw[k1 * r2 * (n / M)]);             // w_M^{k1 j2}, k1 j2 < M
+    }
+    D[t * LDT + sl] = z;                                        // D[k1 B + j2]
+    __syncthreads();
+    double2 x = make_double2(0.0, 0.0);
+    {
+        int wi = 0;                                             // (k2 j2 mod B) * (n / B)
+        const int wstep = r2 * (n / B);
+        const double2 *d = D + k1 * B * LDT + sl;
+        for (int j2 = 0; j2 < B; ++j2) {
+            const double2 p = cmul_s<SIGN>(d[j2 * LDT], tw[wi]);
+            x.x += p.x;
+            x.y += p.y;
+            wi += wstep;
+            if (wi >= n) wi -= n;
+        }
+    }
+    k_out = k1 + A * r2;
+    return x;
+}
+
+// Both kernels: grid = (stick groups, field chunks).  A CTA keeps ITS sticks and walks over the fields of its chunk, so the
+// index map of a stick (which coefficient of H each of its <= S folded terms is) is read once into registers and every field
+// costs one round of independent, stick-coalesced gathers (no index load in front of them).  S <= 16.
+// NQ = S rounded up to a multiple of 4 (template: the index registers are a compile-time array); MAXT = 512 or 1024 bounds the
+// CTA (32 M threads), so that slabs of <= 16 planes get 128 registers per thread.
+template <int NQ, int MAXT>
+__global__ void __launch_bounds__(MAXT)
+inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__restrict__ T, long long npw_h,
+                      double2 *__restrict__ Zs, const int *__restrict__ gather, int g0, int slab, int count, int per_cta) {
+    constexpr int TS = SLAB_TS, LDT = TS + 1;
+    extern __shared__ __align__(16) unsigned char smem[];
+    double2 *C = reinterpret_cast<double2 *>(smem);
+    double2 *D = C + M * LDT;
+    const double2 *__restrict__ tw = P.tw;                      // small table, read through L1
+    const int NS = P.NS, R = P.R;
+    const int sl = threadIdx.x % TS, j = threadIdx.x / TS;      // lanes run over sticks: coalesced gathers
+    const int sidx = blockIdx.x * TS + sl;
+    int code[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        const int t1 = j + q * M;
+        code[q] = (q < S && sidx < NS && (t1 <= R || t1 >= n - R)) ? P.hmapT[(long long)t1 * NS + sidx] : -1;   // |m1| <= R
+    }
+    const int ti0 = (slab * j) % n, tstep = (slab * M) % n;     // (slab * t1) mod n for t1 = j + q M
+    const int p_end = min(count, (int)(blockIdx.y + 1) * per_cta);
+    for (int p = blockIdx.y * per_cta; p < p_end; ++p) {
+        const double2 *tg = T + (gather ? (long long)gather[g0 + p] : (long long)p) * npw_h;
+        double2 y = make_double2(0.0, 0.0);
+        int ti = ti0;
+#pragma unroll
+        for (int q0 = 0; q0 < NQ; q0 += 4) {
+            double2 v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int c = code[q0 + u];
+                v[u] = make_double2(0.0, 0.0);
+                if (c >= 0) v[u] = tg[c];
+                else if (c <= -2) { v[u] = tg[-2 - c]; v[u].y = -v[u].y; }
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const double2 pr = cmul_s<+1>(v[u], tw[ti]);    // times e^{+2 pi i slab t1 / n}
+                y.x += pr.x;
+                y.y += pr.y;
+                ti += tstep;
+                if (ti >= n) ti -= n;
+            }
+        }
+        __syncthreads();                                        // the previous field's transform has left C and D
+        C[j * LDT + sl] = y;
+        __syncthreads();
+        int k;
+        const double2 x = slab_dft<+1>(C, D, tw, n, M, A, M / A, j, sl, k);
+        if (sidx < NS) Zs[((long long)p * M + k) * NS + sidx] = x;
+    }
+}
+
+// field p of the launch goes to row  (p / rc) * row_ld + row0 + (p % rc)  of X (the rows of a chunk, block after block)
+template <int NQ, int MAXT>
+__global__ void __launch_bounds__(MAXT)
+fwd_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__restrict__ Zs, double2 *__restrict__ X,
+                      long long npw_h, const double *__restrict__ scale, int slab, int accumulate, int rc, long long row_ld,
+                      long long row0, int count, int per_cta) {
+    constexpr int TS = SLAB_TS, LDT = TS + 1;
+    extern __shared__ __align__(16) unsigned char smem[];
+    double2 *C = reinterpret_cast<double2 *>(smem);
+    double2 *D = C + M * LDT;
+    const double2 *__restrict__ tw = P.tw;
+    const int NS = P.NS, R = P.R;
+    const int sl = threadIdx.x % TS, t = threadIdx.x / TS;
+    const int sidx = blockIdx.x * TS + sl;
+    // this thread's output residue j = k1 + A k2 (what slab_dft returns for thread t) and its targets on H, with their scale
+    const int Bf = M / A, j = t / Bf + A * (t % Bf);
+    int hh[NQ];
+#pragma unroll
+    for (int q = 0; q < NQ; ++q) {
+        const int t1 = j + q * M;
+        hh[q] = (q < S && sidx < NS && (t1 <= R || t1 >= n - R)) ? P.hmapT[(long long)t1 * NS + sidx] : -1;
+    }
+    const int ti0 = (slab * j) % n, tstep = (slab * M) % n;
+    const int p_end = min(count, (int)(blockIdx.y + 1) * per_cta);
+    for (int p = blockIdx.y * per_cta; p < p_end; ++p) {
+        const double2 zin = sidx < NS ? Zs[((long long)p * M + t) * NS + sidx] : make_double2(0.0, 0.0);   // plane k = t of the slab
+        double2 *xo = X + ((p / rc) * row_ld + row0 + (p % rc)) * npw_h;
+        __syncthreads();
+        C[t * LDT + sl] = zin;
+        __syncthreads();
+        int jj;                                                 // Y[j] = sum_k x[k] e^{-2 pi i k j / M}
+        const double2 y = slab_dft<-1>(C, D, tw, n, M, A, Bf, t, sl, jj);
+        int ti = ti0;
+        // one read-modify-write after the other (measured: a batch of reads followed by a batch of writes is slower)
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) {
+            if (hh[q] >= 0) {
+                const double2 pr = cmul_s<-1>(y, tw[ti]);       // times e^{-2 pi i slab t1 / n}
+                const double sc = scale[hh[q]];
+                double2 v = make_double2(pr.x * sc, pr.y * sc);
+                if (accumulate) { const double2 o = xo[hh[q]]; v.x += o.x; v.y += o.y; }
+                xo[hh[q]] = v;
+            }
+            ti += tstep;
+            if (ti >= n) ti -= n;
+        }
+    }
+}
+
+}  // namespace bsefft

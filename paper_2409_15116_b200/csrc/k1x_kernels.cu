@@ -1,6 +1,8 @@
 // Pair screen decision + pair list (eq. 16) and the K1x accumulation (eq. 5):
 //   keep (v<=w) iff v == w or M_vw / sqrt(M_vv M_ww) >= eta;   list in lexicographic order
 //   acc[b,v,r] = sum_{w : (v,w) or (w,v) kept} tau_{vw}(r) a[b,w,r]
+#include <algorithm>
+
 #include "bse_internal.h"
 
 namespace {
@@ -314,6 +316,31 @@ int bse_launch_pairlist(bse_handle *h) {
         h->adj_h.resize((size_t)nadj * 2);
         BSE_CUDA(cudaMemcpyAsync(h->adj_h.data(), h->adj, (size_t)nadj * 8, cudaMemcpyDeviceToHost, h->stream));
         BSE_CUDA(cudaStreamSynchronize(h->stream));
+    }
+    h->Pa = P;
+    cudaFree(h->pairs_act); cudaFree(h->eslot_act);
+    h->pairs_act = nullptr; h->eslot_act = nullptr;
+    if (h->rows_set) {
+        // the pairs that touch a row of [row0, row1), in ascending pair index; slot of every directed entry of those rows
+        std::vector<int2> pairs_h((size_t)std::max(P, 1));
+        BSE_CUDA(cudaMemcpyAsync(pairs_h.data(), h->pairs, (size_t)P * 8, cudaMemcpyDeviceToHost, h->stream));
+        BSE_CUDA(cudaStreamSynchronize(h->stream));
+        std::vector<int> slot((size_t)std::max(P, 1), -1), eslot((size_t)std::max(nadj, 1), -1);
+        std::vector<int2> act;
+        for (int p = 0; p < P; ++p) {
+            const int2 vw = pairs_h[p];
+            if ((vw.x >= h->row0 && vw.x < h->row1) || (vw.y >= h->row0 && vw.y < h->row1)) {
+                slot[p] = (int)act.size();
+                act.push_back(vw);
+            }
+        }
+        for (int v = h->row0; v < h->row1; ++v)
+            for (int e = h->adj_ptr_h[v]; e < h->adj_ptr_h[v + 1]; ++e) eslot[e] = slot[h->adj_h[2 * (size_t)e + 1]];
+        h->Pa = (long long)act.size();
+        BSE_CUDA(cudaMalloc(&h->pairs_act, std::max<size_t>(act.size(), 1) * 8));
+        BSE_CUDA(cudaMalloc(&h->eslot_act, std::max<size_t>(eslot.size(), 1) * 4));
+        BSE_CUDA(cudaMemcpy(h->pairs_act, act.data(), act.size() * 8, cudaMemcpyHostToDevice));
+        BSE_CUDA(cudaMemcpy(h->eslot_act, eslot.data(), eslot.size() * 4, cudaMemcpyHostToDevice));
     }
     return BSE_OK;
 }

@@ -535,14 +535,121 @@ def test_compact_inverse_kernel_subtract_epilogue():
 def test_plane_slab_apply_matches_the_group_path():
     """PW layout with tau on H: the plane-slab streaming apply (default: one slab of planes at a time, all blocks and all
     pairs resident, slab stick passes) against the oracle, with ragged row chunks, and against the group / row-batch path
-    it replaces (knob slab_rows = -1).  Grids 24 = 4 x 6 (apply grid 20 = 5 x 4 or 24), 30 = 5 x 6 and 12 = 3 x 4."""
+    it replaces (knob slab_rows = -1).  Apply grids 20 / 24, 30 and 12, split into slabs of 6, 5, 4, 3 or 2 planes."""
     bse = _bse()
     for cfg in (wl.Config("slab", 10.0, 24, 9, 20, 8.0, 1.2, 0.8, 3.0, 0.02, 5, "random", seed=77),
                 wl.Config("slab", 14.0, 30, 7, 16, 5.0, 1.3, 0.8, 3.0, 0.0, 3, "random", seed=311),
                 wl.Config("slab", 9.0, 12, 5, 7, 3.0, 1.3, 0.8, 3.0, 0.05, 2, "random", seed=112)):
         w = wl.make(cfg=cfg)
         for tau in (bse.BSE_TAU_PW, bse.BSE_TAU_STREAM):
-            o_def = _check_pw(w, tau)
-            o_rag = _check_pw(w, tau, {"slab_rows": 4})
+            o_def = _check_pw(w, tau)                                           # small grid: one slab holds every plane
+            o_rag = _check_pw(w, tau, {"slab_rows": 4, "slab_planes": 6})      # several slabs, ragged row chunks
+            o_thin = _check_pw(w, tau, {"slab_planes": 2})
             o_old = _check_pw(w, tau, {"slab_rows": -1})
-            assert rel(o_rag, o_def) < 1e-13 and rel(o_old, o_def) < 1e-12
+            assert rel(o_rag, o_def) < 1e-12 and rel(o_thin, o_def) < 1e-12 and rel(o_old, o_def) < 1e-12
+
+
+def test_row_sharded_handles_reproduce_the_full_apply():
+    """SURVEY 8(f) #3 on one GPU: handles that own the row blocks [0, 4), [4, 7), [7, 9) (one after the other, nothing waits on
+    anything) build tau only for the pairs that touch their rows and together reproduce the unsharded K1x output; the pieces
+    are also compared with the oracle through the full result."""
+    bse = _bse()
+    cfg = wl.Config("shard", 10.0, 24, 9, 20, 8.0, 1.2, 0.8, 3.0, 0.02, 3, "random", seed=77)
+    w = wl.make(cfg=cfg)
+    for tau in (bse.BSE_TAU_PW, bse.BSE_TAU_STREAM):
+        full = _check_pw(w, tau)                                              # [B][Nv][npw_h], checked against the oracle
+        B, Nv, npw_h = full.shape
+        a_d = torch.from_numpy(np.ascontiguousarray(w.a_pw).view(np.float64)).to("cuda:0")
+        pieces = []
+        for v0, v1 in ((0, 4), (4, 7), (7, 9)):
+            g = Gpu(w, tau | bse.BSE_VEC_PW, {"slab_planes": 6})
+            try:
+                bse.bse_set_rows(g.h, v0, v1)
+                g.build()
+                out = torch.empty((B, v1 - v0, npw_h, 2), dtype=torch.float64, device="cuda:0")
+                bse.bse_apply_k1x(g.h, a_d, out, B)
+                torch.cuda.synchronize()
+                pieces.append(out.cpu().numpy().view(np.complex128)[..., 0])
+            finally:
+                g.close()
+        got = np.concatenate(pieces, axis=1)
+        assert rel(got, full) < 1e-13
+    g = Gpu(w, 0)
+    try:
+        with pytest.raises(bse.BseError) as e:
+            bse.bse_set_rows(g.h, 0, 4)                                       # REAL layout: not supported
+        assert e.value.code == bse.BSE_EUNSUPPORTED
+    finally:
+        g.close()
+
+
+def test_k1e_split_over_row_blocks():
+    """SURVEY 8(f) #3, K1e part: the Hartree shares of row blocks (bse_k1e_hartree_partial) summed - the all-reduce a
+    multi-GPU run does - then bse_k1e_from_hartree on every block reproduce bse_apply_k1e and the oracle."""
+    bse = _bse()
+    cfg = wl.Config("k1es", 10.0, 24, 9, 20, 8.0, 1.2, 0.8, 3.0, 0.02, 3, "random", seed=78)
+    w = wl.make(cfg=cfg)
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    ref = orc.apply_k1e_pw(tab, w.u, w.a_pw)
+    B, Nv, npw_h = ref.shape
+    g = Gpu(w, bse.BSE_TAU_PW | bse.BSE_VEC_PW)
+    try:
+        blocks = ((0, 4), (4, 7), (7, 9))
+        a_d = torch.from_numpy(np.ascontiguousarray(w.a_pw).view(np.float64)).to("cuda:0").reshape(B, Nv, npw_h, 2)
+        vG = torch.zeros((B, npw_h, 2), dtype=torch.float64, device="cuda:0")
+        for v0, v1 in blocks:
+            share = torch.empty_like(vG)
+            bse.bse_k1e_hartree_partial(g.h, a_d[:, v0:v1].contiguous(), v0, v1, B, share)
+            vG += share                                                       # what the all-reduce does
+        pieces = []
+        for v0, v1 in blocks:
+            out = torch.empty((B, v1 - v0, npw_h, 2), dtype=torch.float64, device="cuda:0")
+            bse.bse_k1e_from_hartree(g.h, vG, v0, v1, B, out)
+            torch.cuda.synchronize()
+            pieces.append(out.cpu().numpy().view(np.complex128)[..., 0])
+        got = np.concatenate(pieces, axis=1)
+        wt = np.full(tab.npw_h, 2.0)
+        wt[0] = 1.0
+        err = np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum())
+        assert err <= TOL, err
+    finally:
+        g.close()
+
+
+def test_sharded_driver_single_rank():
+    """paper_2409_15116_b200/sharded.py end to end on one rank (world size 1, no collective to wait on): K1e and K1d rows
+    against the oracle."""
+    bse = _bse()
+    from paper_2409_15116_b200 import sharded
+
+    class _NoDist:
+        @staticmethod
+        def is_initialized():
+            return False
+
+    cfg = wl.Config("shd", 10.0, 24, 8, 16, 8.0, 1.2, 0.8, 3.0, 0.02, 2, "random", seed=83)
+    w = wl.make(cfg=cfg)
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    pairs, _ = orc.screen_pairs(w.u, w.eta)
+    tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs, want="r")
+    ref_x = orc.apply_k1x_pw(tab, w.u, pairs, tau_ref, w.a_pw)
+    ref_e = orc.apply_k1e_pw(tab, w.u, w.a_pw)
+    dev = torch.device("cuda:0")
+    u_d = torch.from_numpy(w.u).to(dev)
+    phi_d = torch.from_numpy(np.ascontiguousarray(w.phi).view(np.float64)).to(dev)
+    sh = sharded.ShardedBSE([w.n] * 3, w.cell, w.ecut, w.Nv, u_d, w.phi.shape[0], phi_d, w.lam, w.eta, bse.BSE_TAU_PW, 0, 1,
+                            _NoDist, dev)
+    try:
+        sh.build()
+        B, Nv, npw_h = ref_x.shape
+        a_d = torch.from_numpy(np.ascontiguousarray(w.a_pw).view(np.float64)).to(dev).reshape(B, Nv, npw_h, 2)
+        out_e, out_x = torch.empty_like(a_d), torch.empty_like(a_d)
+        sh.apply(a_d, out_e, out_x)
+        torch.cuda.synchronize()
+        wt = np.full(tab.npw_h, 2.0)
+        wt[0] = 1.0
+        for got_d, ref in ((out_e, ref_e), (out_x, ref_x)):
+            got = got_d.cpu().numpy().view(np.complex128)[..., 0]
+            assert np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum()) <= TOL
+    finally:
+        sh.close()
