@@ -493,10 +493,10 @@ int plan_row_batches(bse_handle *h, int rows_cap) {
 //   acc_r[Bg][rows_cap][N] PW layout: accumulated rows of the current row batch (all Nv rows with BSE_TAU_REAL)
 // A larger row batch re-reads a fewer times and lets rows that share neighbours hit L2, a larger group inverts tau fewer
 // times: 60 % of the free memory goes to the group, the rest to the batch.
-int plan_apply_memory(bse_handle *h, int B, bool allow_slab = true) {
+int plan_apply_memory(bse_handle *h, int B, bool allow_slab = true, bool mix = false) {
     const bool pw = (h->flags & BSE_VEC_PW) != 0;
     const bool batched = (h->flags & BSE_TAU_MASK) != BSE_TAU_REAL;
-    if (h->plan_ok && h->plan_allow_slab != allow_slab) h->plan_ok = false;
+    if (h->plan_ok && (h->plan_allow_slab != allow_slab || (mix && !h->plan_mix))) h->plan_ok = false;
     // the plan is kept only for the very adjacency it was made for (a rebuilt list with the same pair count but other
     // pairs must not reuse the old batches / eslot) and while the group still holds B blocks
     const bool same_list = !batched || (h->plan_adj_ptr_h == h->adj_ptr_h && h->plan_adj_h == h->adj_h);
@@ -504,7 +504,7 @@ int plan_apply_memory(bse_handle *h, int B, bool allow_slab = true) {
     cudaFree(h->tau_batch); cudaFree(h->a_r); cudaFree(h->acc_r);
     h->tau_batch = h->a_r = h->acc_r = nullptr;
     h->Bg = 0; h->Pacc = 0; h->rows_cap = 0; h->plan_ok = false;
-    h->slab_mode = false; h->slab_rc = 0; h->plan_allow_slab = allow_slab;
+    h->slab_mode = false; h->slab_rc = 0; h->plan_allow_slab = allow_slab; h->plan_mix = mix;
     size_t free_b = 0, total_b = 0;
     cudaMemGetInfo(&free_b, &total_b);
     // Plane-slab streaming (PW layout, tau on H): the whole apply runs on one slab of R2 planes at a time, with a(r) of ALL B
@@ -522,7 +522,8 @@ int plan_apply_memory(bse_handle *h, int B, bool allow_slab = true) {
             if (pl.n % M || pl.n / M > 16) continue;           // the slab stick kernels keep <= 16 folded terms per thread
             if (h->dbg_slab_planes >= 1 && M > h->dbg_slab_planes) continue;
             SN8 = 8.0 * (double)M * pl.n * pl.n;
-            const double fixed = ((double)B * h->Nv + (double)h->Pa) * SN8;
+            // a(r) of all blocks + tau(r) of all (owned) pairs; the combined call also keeps u and v_H of the slab (k1e_ws)
+            const double fixed = ((double)B * h->Nv + (double)h->Pa + (mix ? (double)h->Nv + 2.0 * B : 0.0)) * SN8;
             pz = (long long)(((double)h->Pb * h->n * h->fft.NS) / ((double)M * pl.NS));
             rc = (long long)((avail_s - fixed) / ((double)B * SN8));
             rc = std::min<long long>(rc, std::min<long long>(pz / B, 65535 / B));
@@ -773,9 +774,30 @@ int apply_pw_slab(bse_handle *h, const double2 *a, double2 *out, int B) {
         }
         return BSE_OK;
     };
+    // combined call (eq. 1, bse_apply_k1): k1e_ws = u_slab [Nv][SN] | vH_slab [B][SN] | vG [B][npw_h].  A first sweep over the
+    // slabs forms the transition density n_b = sum_v u_v a_bv slab by slab and accumulates v_c n_b(G) into vG (eq. 4); the main
+    // sweep then adds 2 ce u_v v_H[b] to the accumulated rows before their forward transform, so P_c is applied once.
+    double *u_slab = h->k1e_ws, *vH_slab = h->k1e_ws ? h->k1e_ws + Nv * SN : nullptr;
+    double2 *vG = h->k1e_ws ? (double2 *)(vH_slab + (long long)B * SN) : nullptr;
+    if (h->mix_on) {
+        for (int s = 0; s < S; ++s) {
+            if ((rc = to_slab(a, (long long)B * Nv, h->a_r, s))) return rc;
+            if ((rc = to_slab(h->uG, Nv, u_slab, s))) return rc;
+            { StageTimer t(h, BSE_ST_K1E_DENSITY, 2.0 * B * Nv * (double)SN, 8.0 * SN * (double)(B * Nv + Nv + B));
+              if ((rc = bse_launch_k1e_density(u_slab, h->a_r, vH_slab, h->Nv, SN, B, h->stream))) return rc; }
+            { StageTimer t(h, BSE_ST_FWD_PLANE, B * m.plane_flops * share, B * m.N8 * share, B * m.z * share);
+              if ((rc = bse_launch_fwd_plane(pl, vH_slab, nullptr, 0, B, SN, h->Z, h->stream, M))) return rc; }
+            { StageTimer t(h, BSE_ST_FWD_STICK, B * m.stick_flops * share, B * m.g * share, B * m.z * share);
+              if ((rc = bse_launch_fwd_stick_slab(pl, S, M, h->Z, B, vG, pl.vcn, h->stream, s, s > 0, B, 0, 0))) return rc; }
+        }
+    }
     for (int s = 0; s < S; ++s) {
         if ((rc = to_slab(a, (long long)B * Nv, h->a_r, s))) return rc;
         if ((rc = to_slab(h->tau_g, h->Pa, h->tau_batch, s))) return rc;
+        if (h->mix_on) {
+            if ((rc = to_slab(h->uG, Nv, u_slab, s))) return rc;
+            if ((rc = to_slab(vG, B, vH_slab, s))) return rc;
+        }
         for (long long v0 = h->row0; v0 < h->row1; v0 += h->slab_rc) {       // the owned rows (all of them unless bse_set_rows)
             const int rows = (int)std::min<long long>(h->slab_rc, h->row1 - v0);
             const double directed = (double)(h->adj_ptr_h[v0 + rows] - h->adj_ptr_h[v0]);
@@ -783,6 +805,11 @@ int apply_pw_slab(bse_handle *h, const double2 *a, double2 *out, int B) {
                            8.0 * SN * ((double)h->Pa * rows / nloc + (double)B * rows + (v0 == h->row0 ? (double)B * Nv : 0.0)));
               if ((rc = bse_launch_accumulate_rows(h, SN, h->tau_batch, h->eslot_act, h->rowid + v0, rows, h->a_r, h->acc_r, rows,
                                                    true, B))) return rc; }
+            if (h->mix_on) {
+                StageTimer t(h, BSE_ST_K1E_PRODUCT, 3.0 * B * rows * (double)SN, 8.0 * SN * (2.0 * B * rows + rows + B));
+                if ((rc = bse_launch_k1_mix(u_slab, vH_slab, h->acc_r, h->rowid + v0, rows, rows, true, SN, B, h->mix_ce, h->mix_cd,
+                                            h->stream))) return rc;
+            }
             const int cnt = B * rows;
             { StageTimer t(h, BSE_ST_FWD_PLANE, cnt * m.plane_flops * share, cnt * m.N8 * share, cnt * m.z * share);
               if ((rc = bse_launch_fwd_plane(pl, h->acc_r, nullptr, 0, cnt, SN, h->Z, h->stream, M))) return rc; }
@@ -798,7 +825,7 @@ int apply_pw(bse_handle *h, const double2 *a, double2 *out, int B) {
     const FftPlan &pl = *h->ap;
     int rc;
     if ((rc = ensure_u_pw(h))) return rc;
-    if (h->slab_mode && !h->mix_on) return apply_pw_slab(h, a, out, B);
+    if (h->slab_mode) return apply_pw_slab(h, a, out, B);
     if (h->rows_set) { bse_set_error("row-sharded apply needs the plane-slab path (PW layout, tau on H, enough memory)"); return BSE_EUNSUPPORTED; }
     const long long Nv = h->Nv, npw_h = pl.npw_h;
     for (int b0 = 0; b0 < B; b0 += h->Bg) {
@@ -1205,7 +1232,39 @@ extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, 
     if (a == out) { bse_set_error("out must not alias a"); return BSE_EINVAL; }
     int rc;
     const bool pw = (h->flags & BSE_VEC_PW) != 0;
-    const bool fly = pw && h->ap != &h->fft && (h->flags & BSE_TAU_MASK) != BSE_TAU_REAL;   // u on the apply grid is made on
+    const bool batched = (h->flags & BSE_TAU_MASK) != BSE_TAU_REAL;
+    if (h->rows_set) { bse_set_error("bse_apply_k1 is not available on a row-sharded handle"); return BSE_EUNSUPPORTED; }
+    if (pw && batched) {
+        // plane-slab path (the one bse_apply_k1x takes) with room kept for u and v_H of one slab
+        if ((rc = ensure_u_pw(h))) return rc;
+        if ((h->flags & BSE_TAU_MASK) == BSE_TAU_STREAM) {
+            if ((rc = ensure_tau_store(h, false))) return rc;
+            if ((rc = fill_tau_store(h, false))) return rc;
+        }
+        if (h->u_a) {                                           // a copy left by bse_apply_k1e: give its memory to the plan
+            BSE_CUDA(cudaStreamSynchronize(h->stream));
+            cudaFree(h->u_a);
+            h->u_a = nullptr; h->u_a_valid = false;
+            h->plan_ok = false;
+        }
+        if (!(h->plan_ok && h->slab_mode && h->plan_mix)) {      // the K1e scratch of another call would eat the slab's room
+            BSE_CUDA(cudaStreamSynchronize(h->stream));
+            cudaFree(h->k1e_ws);
+            h->k1e_ws = nullptr; h->k1e_bytes = 0;
+        }
+        if ((rc = plan_apply_memory(h, B, true, true))) return rc;
+        if (h->slab_mode) {
+            const size_t SN = (size_t)h->slab_M * h->ap->n * h->ap->n;
+            if ((rc = ensure_k1e_ws(h, ((size_t)h->Nv + B) * SN * 8 + (size_t)B * h->ap->npw_h * 16))) return rc;
+            if (!h->slab_mode || !h->plan_ok) { bse_set_error("bse_apply_k1: the slab workspace did not fit"); return BSE_ENOMEM; }
+            h->mix_ce = ce; h->mix_cd = cd; h->mix_B = B;
+            h->mix_on = true;
+            rc = apply_pw(h, (const double2 *)a, (double2 *)out, B);
+            h->mix_on = false;
+            return rc;
+        }
+    }
+    const bool fly = pw && h->ap != &h->fft && batched;         // u on the apply grid is made on
     if (pw && (rc = ensure_u_pw(h))) return rc;                 // the fly from u(G), Pb orbitals at a time: no [Nv][Na] copy
     if (pw && !fly && (rc = ensure_u_apply(h))) return rc;
     if (fly && h->u_a) {                                        // a copy left by bse_apply_k1e: give its memory to the plan
@@ -1215,12 +1274,11 @@ extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, 
         h->plan_ok = false;
     }
     if ((rc = ensure_k1e_ws(h, (size_t)(B + (fly ? h->Pb : 0)) * h->ap->N * 8))) return rc;
-    if ((h->flags & BSE_TAU_MASK) == BSE_TAU_STREAM) {
+    if ((h->flags & BSE_TAU_MASK) == BSE_TAU_STREAM && !(pw && batched)) {
         if ((rc = ensure_tau_store(h, false))) return rc;
         if ((rc = fill_tau_store(h, false))) return rc;
     }
-    if (h->rows_set) { bse_set_error("bse_apply_k1 is not available on a row-sharded handle"); return BSE_EUNSUPPORTED; }
-    if ((rc = plan_apply_memory(h, B, false))) return rc;    // the combined call keeps the group / row-batch path
+    if ((rc = plan_apply_memory(h, B, false))) return rc;    // the slab did not fit (or REAL layout): group / row-batch path
     h->mix_ce = ce; h->mix_cd = cd; h->mix_B = B;
     h->mix_u = fly ? nullptr : ((pw && h->u_a) ? h->u_a : h->u);
     if (pw) {

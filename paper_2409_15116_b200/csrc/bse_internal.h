@@ -100,7 +100,7 @@ struct bse_handle {
     long long dbg_slab_rows = 0;                      // cap of the rows per chunk of the plane-slab apply; -1 = never use it
     // plane-slab streaming of the PW-layout apply: a_r = [B][Nv][SN], tau_batch = [P][SN],
     // acc_r = [B][slab_rc][SN], SN = R2 n_a^2 points of the slab { i1 = s + R1 k2 }
-    bool slab_mode = false, plan_allow_slab = true;
+    bool slab_mode = false, plan_allow_slab = true, plan_mix = false;
     int slab_rc = 0;                                  // rows per chunk
     int slab_S = 0, slab_M = 0;                       // the slab split n_a = S * M chosen by the plan (fewest slabs that fit)
     size_t a_r_elems = 0;                             // capacity of a_r in doubles
