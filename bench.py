@@ -359,6 +359,7 @@ def main():
         sampler.start()
     bse.bse_profile_reset(h)
     t_build, t_apply, t_fill = [], [], []
+    torch.cuda.profiler.start()          # `ncu --profile-from-start off` then lists the kernels of the timed steps only
     wall0 = time.perf_counter()
     for _ in range(args.steps):
         tb, ta, tf = step(True)
@@ -369,6 +370,7 @@ def main():
     if world > 1:
         dist.barrier()
     wall = time.perf_counter() - wall0
+    torch.cuda.profiler.stop()
     clocks = sampler.stop() if rank == 0 else None
     prof_counts = bse.bse_profile_get(h)
     P = bse.bse_num_pairs(h)

@@ -509,8 +509,23 @@ int plan_apply_memory(bse_handle *h, int B, bool allow_slab = true, bool mix = f
     cudaMemGetInfo(&free_b, &total_b);
     // Plane-slab streaming (PW layout, tau on H): the whole apply runs on one slab of R2 planes at a time, with a(r) of ALL B
     // blocks and tau(r) of ALL pairs resident for that slab, so every field is inverse-transformed exactly once per call (no
-    // trial-block groups, no pair shared between two row batches).  Taken whenever it fits.
-    if (pw && batched && allow_slab && h->dbg_max_group < 1 && h->dbg_max_batch < 1 && h->dbg_slab_rows >= 0) {
+    // trial-block groups, no pair shared between two row batches).  Every slab sweeps the coefficient arrays once, which costs
+    // more than it saves while the group path below holds ALL B blocks in one group (cfg 3-4: measured 43 vs 37 ms, 814 vs
+    // 735 ms), so the slab path is taken when that path would need several groups (cfg 5: 2.5 vs 3.3 s), on row-sharded
+    // handles, and when a slab knob asks for it.
+    bool one_group = false;
+    if (pw && batched) {
+        const double N8g = 8.0 * (double)h->ap->N, availg = 0.92 * (double)free_b - 512.0 * 1048576.0;
+        const double avgd = std::max(1.0, (double)h->nadj / h->Nv);
+        int maxd = 1;
+        for (int v = 0; v < h->Nv; ++v) maxd = std::max(maxd, h->adj_ptr_h[v + 1] - h->adj_ptr_h[v]);
+        const double want = (double)std::max<long long>(maxd, std::min<long long>(h->nadj, 256));
+        const double rest = availg - (double)B * h->Nv * N8g;
+        one_group = rest > 0 && rest / (N8g * (1.0 + 2.0 * B / avgd)) >= want;
+    }
+    const bool slab_forced = h->rows_set || h->dbg_slab_rows >= 1 || h->dbg_slab_planes >= 1;
+    if (pw && batched && allow_slab && h->dbg_max_group < 1 && h->dbg_max_batch < 1 && h->dbg_slab_rows >= 0 &&
+        (slab_forced || !one_group)) {
         const FftPlan &pl = *h->ap;
         const double avail_s = 0.92 * (double)free_b - 512.0 * 1048576.0;
         // the slab split n_a = S * M (any factorisation with M <= 32, fft_kernels.cuh): the fewest slabs whose working set fits,
@@ -1247,7 +1262,7 @@ extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, 
             h->u_a = nullptr; h->u_a_valid = false;
             h->plan_ok = false;
         }
-        if (!(h->plan_ok && h->slab_mode && h->plan_mix)) {      // the K1e scratch of another call would eat the slab's room
+        if (!h->plan_ok || (h->slab_mode && !h->plan_mix)) {     // about to plan: the K1e scratch of another call would eat the slab's room
             BSE_CUDA(cudaStreamSynchronize(h->stream));
             cudaFree(h->k1e_ws);
             h->k1e_ws = nullptr; h->k1e_bytes = 0;
@@ -1278,7 +1293,7 @@ extern "C" int bse_apply_k1(bse_handle *h, const double *a, double *out, int B, 
         if ((rc = ensure_tau_store(h, false))) return rc;
         if ((rc = fill_tau_store(h, false))) return rc;
     }
-    if ((rc = plan_apply_memory(h, B, false))) return rc;    // the slab did not fit (or REAL layout): group / row-batch path
+    if ((rc = plan_apply_memory(h, B, pw && batched, pw && batched))) return rc;   // group / row-batch path (same plan as above)
     h->mix_ce = ce; h->mix_cd = cd; h->mix_B = B;
     h->mix_u = fly ? nullptr : ((pw && h->u_a) ? h->u_a : h->u);
     if (pw) {
