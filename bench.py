@@ -260,6 +260,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-k1e", action="store_true")
+    ap.add_argument("--knob", action="append", default=[], help="key=value for bse_debug_set (tuning / A-B runs), repeatable")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -334,6 +335,9 @@ def main():
     flags |= bse.BSE_VEC_PW if args.vec == "pw" else bse.BSE_VEC_REAL
     stream = torch.cuda.current_stream().cuda_stream
     h = bse.bse_create([w.n] * 3, w.cell, w.ecut, Nv, u_d, n_pdep, phi_d, w.lam, w.eta, flags, stream)
+    for kv in args.knob:
+        key, val = kv.split("=")
+        bse.bse_debug_set(h, key, int(val))
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
     def step(timed):

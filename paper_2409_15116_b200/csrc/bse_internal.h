@@ -176,6 +176,7 @@ enum { EPI_PARTIAL = 0, EPI_TAU = 1, EPI_SUB = 2, EPI_STORE = 3 };
 int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb, int M, int N, long long K,
                  bool squareA, bool squareB, double *part, size_t part_bytes, double *C, long long ldc,
                  double alpha, const double *colscale, cudaStream_t s, bool accumulate = false);   // accumulate: C += instead of C =
+void bse_gemm_set_bm(int bm);      // test / tuning knob: force the CTA tile height (64 or 128; 0 = automatic)
 // NN form: acc = A[M][K] * B[K][N];  EPI_TAU: C = colscale2[n>>1] * (Xin + acc);  EPI_SUB: C = C - acc;  EPI_STORE: C = acc
 int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, int M, long long N, int K,
                 int epi, const double *Xin, const double *colscale2, double *C, long long ldc, cudaStream_t s);

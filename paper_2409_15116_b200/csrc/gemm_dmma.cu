@@ -9,10 +9,10 @@
 
 namespace {
 
-constexpr int BM = 64, BN = 64, BK = 16, STAGES = 3, THREADS = 128;
+constexpr int BN = 64, BK = 16, STAGES = 3;
+// CTA tile BMT x 64 x 16 with BMT = 64 (4 warps) or 128 (8 warps); every warp owns 32 x 32
 constexpr int LDK = BK + 4;    // K-major tile row stride (doubles): conflict-free fragment reads
 constexpr int LDN = BN + 4;    // N-major tile row stride
-constexpr int A_TILE = BM * LDK;
 constexpr int B_TILE_K = BN * LDK;
 constexpr int B_TILE_N = BK * LDN;
 
@@ -32,12 +32,13 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
 }
 
 // load a K-major tile: rows [r0, r0+64) of a [rows][K] matrix, k in [k0, k0+16) -> smem [64][LDK]
+template <int ROWS, int NT>
 __device__ __forceinline__ void load_tile_k(double *sm, const double *g, long long ld, int rows, int r0,
                                             long long k0, long long kend) {
-    // 64 rows x 8 chunks of 16 B = 512 chunks, 128 threads -> 4 each
+    // ROWS rows x 8 chunks of 16 B, NT threads
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int c = threadIdx.x + i * THREADS;
+    for (int i = 0; i < ROWS * 8 / NT; ++i) {
+        const int c = threadIdx.x + i * NT;
         const int r = c >> 3, kc = (c & 7) * 2;
         const long long left = kend - (k0 + kc);
         const bool ok = (r0 + r < rows) && (left > 0);
@@ -46,12 +47,13 @@ __device__ __forceinline__ void load_tile_k(double *sm, const double *g, long lo
     }
 }
 // load an N-major tile: k rows [k0,k0+16) of a [K][N] matrix, columns [c0, c0+64) -> smem [16][LDN]
+template <int NT>
 __device__ __forceinline__ void load_tile_n(double *sm, const double *g, long long ld, long long cols, long long c0,
                                             int k0, int kend) {
     // 16 rows x 32 chunks = 512 chunks
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int c = threadIdx.x + i * THREADS;
+    for (int i = 0; i < 512 / NT; ++i) {
+        const int c = threadIdx.x + i * NT;
         const int r = c >> 5, cc = (c & 31) * 2;
         const long long left = cols - (c0 + cc);
         const bool ok = (k0 + r < kend) && (left > 0);
@@ -65,12 +67,13 @@ __device__ __forceinline__ void load_tile_n(double *sm, const double *g, long lo
 // EPI_TAU    : C[m][n] = cs2[n>>1] * (Xin[m][n] + acc)
 // EPI_SUB    : C[m][n] = C[m][n] - acc
 // EPI_STORE  : C[m][n] = acc
-template <bool BN_MAJOR, int EPI, bool SQA, bool SQB>
-__global__ void __launch_bounds__(THREADS)
+template <int BM, bool BN_MAJOR, int EPI, bool SQA, bool SQB>
+__global__ void __launch_bounds__(2 * BM)
 dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restrict__ B, long long ldb, int M,
              long long Ntot, long long K, long long kchunk, double *__restrict__ C, long long ldc,
              const double *__restrict__ Xin, const double *__restrict__ cs2) {
     extern __shared__ __align__(16) double sm[];
+    constexpr int THREADS = 2 * BM, A_TILE = BM * LDK;
     double *As = sm;
     double *Bs = sm + STAGES * A_TILE;
     constexpr int B_TILE = BN_MAJOR ? B_TILE_N : B_TILE_K;
@@ -84,6 +87,7 @@ dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restri
     const long long kend = (kbeg + kchunk < K) ? kbeg + kchunk : K;
     const int nk = (int)((kend - kbeg + BK - 1) / BK);
     if (SQA && SQB && n0 + BN <= m0) return;      // screen SYRK: M is symmetric, only tiles touching v <= w are formed
+    (void)THREADS;
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int wm = (warp >> 1) * 32, wn = (warp & 1) * 32;
@@ -114,9 +118,9 @@ dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restri
         if (kt < nk) {
             const int st = kt % STAGES;
             const long long k0 = kbeg + (long long)kt * BK;
-            load_tile_k(As + st * A_TILE, A, lda, M, m0, k0, kend);
-            if (BN_MAJOR) load_tile_n(Bs + st * B_TILE, B, ldb, Ntot, n0, (int)k0, (int)kend);
-            else load_tile_k(Bs + st * B_TILE, B, ldb, (int)Ntot, (int)n0, k0, kend);
+            load_tile_k<BM, THREADS>(As + st * A_TILE, A, lda, M, m0, k0, kend);
+            if (BN_MAJOR) load_tile_n<THREADS>(Bs + st * B_TILE, B, ldb, Ntot, n0, (int)k0, (int)kend);
+            else load_tile_k<BN, THREADS>(Bs + st * B_TILE, B, ldb, (int)Ntot, (int)n0, k0, kend);
         }
         cp_commit();
     };
@@ -128,7 +132,7 @@ dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restri
         issue(kt + STAGES - 1);
         const double *as = As + (kt % STAGES) * A_TILE;
         const double *bs = Bs + (kt % STAGES) * B_TILE;
-        if (SQA && SQB && m0 == (int)n0 && wm > wn) continue;    // diagonal SYRK tile: the warp below the diagonal idles
+        if (SQA && SQB && m0 + wm >= (int)n0 + wn + 32) continue;   // SYRK: a warp tile entirely below the diagonal idles
 #pragma unroll
         for (int kk = 0; kk < BK; kk += 4) {
             double af[4], bf[4];
@@ -196,8 +200,14 @@ __global__ void splitk_reduce_kernel(const double *__restrict__ part, int splits
     C[m * ldc + n] = accumulate ? C[m * ldc + n] + s : s;
 }
 
-constexpr int SMEM_DOT = STAGES * (A_TILE + B_TILE_K) * 8;
-constexpr int SMEM_NN = STAGES * (A_TILE + B_TILE_N) * 8;
+constexpr int smem_dot(int bm) { return STAGES * (bm * LDK + B_TILE_K) * 8; }
+constexpr int smem_nn(int bm) { return STAGES * (bm * LDK + B_TILE_N) * 8; }
+
+// CTA tile height: 64 rows (4 warps).  The 128-row form (8 warps, the 64-column operand tile shared by twice as many warps) is
+// kept behind bse_debug_set("gemm_bm", 128) for A/B timing: it measured slower wherever it differed (cfg 5 pdep_project 468 vs
+// 354 ms, pdep_backproject 410 vs 337 ms, P_c equal): half as many CTAs to balance over 148 SMs and two CTAs per SM instead of 3-4.
+int g_bm_override = 0;
+inline int pick_bm(int) { return g_bm_override == 128 ? 128 : 64; }
 
 // Dynamic shared-memory opt-in of one kernel instantiation.  cudaFuncSetAttribute is thread-safe and idempotent, so it is
 // simply issued before every launch (a few hundred ns on the host) instead of remembering pointers in a shared table.
@@ -207,15 +217,34 @@ int prep(KernelT k, int smem) {
     return BSE_OK;
 }
 
+template <int BM, bool BN_MAJOR, int EPI, bool SQA, bool SQB>
+int launch(dim3 grid, int smem, cudaStream_t s, const double *A, long long lda, const double *B, long long ldb, int M,
+           long long N, long long K, long long kchunk, double *C, long long ldc, const double *Xin, const double *cs2) {
+    auto k = dgemm_kernel<BM, BN_MAJOR, EPI, SQA, SQB>;
+    int rc = prep(k, smem);
+    if (rc) return rc;
+    k<<<grid, 2 * BM, smem, s>>>(A, lda, B, ldb, M, N, K, kchunk, C, ldc, Xin, cs2);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
+
 }  // namespace
+
+void bse_gemm_set_bm(int bm) { g_bm_override = bm; }
 
 int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb, int M, int N, long long K,
                  bool squareA, bool squareB, double *part, size_t part_bytes, double *C, long long ldc,
                  double alpha, const double *colscale, cudaStream_t s, bool accumulate) {
     if (M <= 0 || N <= 0) return BSE_OK;
+    const int BM = pick_bm(M);
     const int tm = (M + BM - 1) / BM, tn = (N + BN - 1) / BN;
     const long long ksteps = (K + BK - 1) / BK;
-    const long long tiles = (squareA && squareB) ? (long long)tm * (tm + 1) / 2 : (long long)tm * tn;   // SYRK: v <= w tiles
+    long long tiles = (long long)tm * tn;
+    if (squareA && squareB) {                                   // SYRK: tiles that touch v <= w
+        tiles = 0;
+        for (int i = 0; i < tm; ++i)
+            for (int j = 0; j < tn; ++j) tiles += ((long long)(j + 1) * BN > (long long)i * BM) ? 1 : 0;
+    }
     // split K so that the CTAs come in whole waves of 148 (one per SM) and there are at least two per SM: the DMMA pipe
     // saturates at ~8 warps per SM, while a few CTAs over a multiple of 148 leave most SMs idle for a whole CTA time
     // (304 CTAs ran 1.5x longer than 288).  More, shorter CTAs only add prologue and partial-sum traffic.
@@ -227,27 +256,25 @@ int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb,
     if (smax < 1) smax = 1;
     long long splits = 1;
     double best = -1.0;
+    const long long per_sm = BM == 128 ? 1 : 2;                 // CTAs of 8 warps count double
     for (long long sp = 1; sp <= smax; ++sp) {
         const long long ctas = tiles * sp;
         double eff = (double)ctas / (double)(((ctas + sms - 1) / sms) * sms);
-        if (ctas < 2 * sms) eff *= 0.5 * (double)ctas / (double)sms;          // under two per SM: scaled down
+        if (ctas < per_sm * sms) eff *= (double)ctas / (double)(per_sm * sms);          // under two per SM: scaled down
         if (eff > best + 0.02) { best = eff; splits = sp; }
-        if (ctas >= 8 * sms) break;
+        if (ctas >= 4 * per_sm * sms) break;
     }
     long long kchunk = ((ksteps + splits - 1) / splits) * BK;
     splits = (K + kchunk - 1) / kchunk;
     dim3 grid(tn, tm, (unsigned)splits);
     int rc;
-    if (squareA && squareB) {
-        auto k = dgemm_kernel<false, EPI_PARTIAL, true, true>;
-        if ((rc = prep(k, SMEM_DOT))) return rc;
-        k<<<grid, THREADS, SMEM_DOT, s>>>(A, lda, B, ldb, M, N, K, kchunk, part, N, nullptr, nullptr);
-    } else {
-        auto k = dgemm_kernel<false, EPI_PARTIAL, false, false>;
-        if ((rc = prep(k, SMEM_DOT))) return rc;
-        k<<<grid, THREADS, SMEM_DOT, s>>>(A, lda, B, ldb, M, N, K, kchunk, part, N, nullptr, nullptr);
-    }
-    BSE_CUDA(cudaGetLastError());
+    if (squareA && squareB)
+        rc = BM == 128 ? launch<128, false, EPI_PARTIAL, true, true>(grid, smem_dot(128), s, A, lda, B, ldb, M, N, K, kchunk, part, N, nullptr, nullptr)
+                       : launch<64, false, EPI_PARTIAL, true, true>(grid, smem_dot(64), s, A, lda, B, ldb, M, N, K, kchunk, part, N, nullptr, nullptr);
+    else
+        rc = BM == 128 ? launch<128, false, EPI_PARTIAL, false, false>(grid, smem_dot(128), s, A, lda, B, ldb, M, N, K, kchunk, part, N, nullptr, nullptr)
+                       : launch<64, false, EPI_PARTIAL, false, false>(grid, smem_dot(64), s, A, lda, B, ldb, M, N, K, kchunk, part, N, nullptr, nullptr);
+    if (rc) return rc;
     const long long MN = (long long)M * N;
     splitk_reduce_kernel<<<(unsigned)((MN + 255) / 256), 256, 0, s>>>(part, (int)splits, MN, N, C, ldc, alpha, colscale,
                                                                        accumulate ? 1 : 0);
@@ -258,27 +285,18 @@ int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb,
 int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, int M, long long N, int K, int epi,
                 const double *Xin, const double *colscale2, double *C, long long ldc, cudaStream_t s) {
     if (M <= 0 || N <= 0) return BSE_OK;
+    const int BM = pick_bm(M);
     const int tm = (M + BM - 1) / BM;
     const long long tn = (N + BN - 1) / BN;
     if (tn * tm > 2147483647LL) { bse_set_error("bse_gemm_nn: too many tiles"); return BSE_EUNSUPPORTED; }
     dim3 grid((unsigned)(tn * tm), 1, 1);
-    int rc;
-    if (epi == EPI_TAU) {
-        auto k = dgemm_kernel<true, EPI_TAU, false, false>;
-        if ((rc = prep(k, SMEM_NN))) return rc;
-        k<<<grid, THREADS, SMEM_NN, s>>>(A, lda, B, ldb, M, N, K, K, C, ldc, Xin, colscale2);
-    } else if (epi == EPI_SUB) {
-        auto k = dgemm_kernel<true, EPI_SUB, false, false>;
-        if ((rc = prep(k, SMEM_NN))) return rc;
-        k<<<grid, THREADS, SMEM_NN, s>>>(A, lda, B, ldb, M, N, K, K, C, ldc, nullptr, nullptr);
-    } else if (epi == EPI_STORE) {
-        auto k = dgemm_kernel<true, EPI_STORE, false, false>;
-        if ((rc = prep(k, SMEM_NN))) return rc;
-        k<<<grid, THREADS, SMEM_NN, s>>>(A, lda, B, ldb, M, N, K, K, C, ldc, nullptr, nullptr);
-    } else {
-        bse_set_error("bse_gemm_nn: bad epilogue");
-        return BSE_EINVAL;
-    }
-    BSE_CUDA(cudaGetLastError());
-    return BSE_OK;
+#define BSE_NN(EPI, XIN, CS2)                                                                                                  \
+    (BM == 128 ? launch<128, true, EPI, false, false>(grid, smem_nn(128), s, A, lda, B, ldb, M, N, K, K, C, ldc, XIN, CS2)      \
+               : launch<64, true, EPI, false, false>(grid, smem_nn(64), s, A, lda, B, ldb, M, N, K, K, C, ldc, XIN, CS2))
+    if (epi == EPI_TAU) return BSE_NN(EPI_TAU, Xin, colscale2);
+    if (epi == EPI_SUB) return BSE_NN(EPI_SUB, nullptr, nullptr);
+    if (epi == EPI_STORE) return BSE_NN(EPI_STORE, nullptr, nullptr);
+#undef BSE_NN
+    bse_set_error("bse_gemm_nn: bad epilogue");
+    return BSE_EINVAL;
 }
