@@ -51,6 +51,11 @@ enum { BSE_OK = 0, BSE_EINVAL = -1, BSE_ENOMEM = -2, BSE_ECUDA = -3, BSE_ESTATE 
 #define BSE_VEC_PW     0x4u   /* a/out = [B][Nv][Npw_h] complex on H ("of length N_pw"); a(0) must be
                                  real; out = P_c of (sum_v' tau a) truncated to S.  With BSE_TAU_PW/STREAM the products
                                  are formed on the smallest supported grid n_a >= 3R+1 (alias-free inside S)     */
+#define BSE_TAU_F32    0x10u  /* with BSE_TAU_PW / BSE_TAU_STREAM: tau(G) is KEPT as complex64 (each pair integral is computed in fp64 and
+                                 rounded once); halves the store and the coefficient sweeps of the apply.  Mixed-precision variant
+                                 (PAPER.md:279); results then carry a relative error of about 2^-24 = 6e-8 instead of 1e-15, so the
+                                 1e-10 parity bar applies to the default (double) store only.  bse_get_tau returns the unrounded
+                                 double values (recomputed) */
 #define BSE_PTR_HOST   0x8u   /* u and phi passed to bse_create are HOST pointers (copied to the device)      */
 
 /* Create a problem instance.  Builds the sphere/stick tables, twiddles and v_c^{1/2} on the host and uploads

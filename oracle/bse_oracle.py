@@ -20,7 +20,8 @@ Conventions / readings (DESIGN.md "Readings of the paper", S1..S20):
 Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): P1 brute-force DFT, P2 Parseval, P3 analytic
 Gaussian Hartree potential at lambda = 0, P4 dense real-space operator on a tiny grid, P5 rank-1
 closed form, P6 complete-basis closed form, P7 W symmetric, P8 sum_r tau = 0, P9 P_c idempotent,
-P10 K symmetric, P11 analytic Gaussian overlap for eq. 16, P12 PW layout == gather(FFT(REAL)).
+P10 K symmetric, P11 analytic Gaussian overlap for eq. 16, P12 PW layout == gather(FFT(REAL)), P18 the single-precision
+store: every component representable in binary32 and within half an ulp (2^-24 relative) of the double value.
 No function here is "parity unpinned".
 """
 from __future__ import annotations
@@ -185,6 +186,13 @@ def tau_G(tab: Tables, uv: np.ndarray, uw: np.ndarray, phiS: np.ndarray, lam: np
     c = np.conj(phiS) @ x                           # O5: <phi_a | x>, full-sphere sum
     y = (f * c) @ phiS                              # O6: sum_a phi_a f_a c_a
     return tab.vc12 * (x + y)                       # O7: v_c rho + v_c^{1/2} chibar v_c^{1/2} rho
+
+
+def tau_G_f32(tab: Tables, uv, uw, phiS, lam) -> np.ndarray:
+    """Mixed-precision variant of the tau build ("experimenting with the use of single precision"; reading:
+    the pair integral is evaluated in fp64 and KEPT in single precision): tau_G rounded once, component by component, to
+    IEEE binary32 (round to nearest even), returned widened back to complex128."""
+    return tau_G(tab, uv, uw, phiS, lam).astype(np.complex64).astype(np.complex128)
 
 
 def tau_r(tab: Tables, uv, uw, phiS, lam) -> np.ndarray:

@@ -20,7 +20,7 @@ lib = C.CDLL(LIB_PATH)
 
 BSE_OK, BSE_EINVAL, BSE_ENOMEM, BSE_ECUDA, BSE_ESTATE, BSE_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 BSE_TAU_REAL, BSE_TAU_PW, BSE_TAU_STREAM = 0x0, 0x1, 0x2
-BSE_VEC_REAL, BSE_VEC_PW, BSE_PTR_HOST = 0x0, 0x4, 0x8
+BSE_VEC_REAL, BSE_VEC_PW, BSE_PTR_HOST, BSE_TAU_F32 = 0x0, 0x4, 0x8, 0x10
 STAGES = ["screen_syrk", "pair_list", "fwd_plane", "fwd_stick", "pdep_project", "pdep_backproject",
           "inv_stick", "inv_plane", "k1x_accumulate", "pc_overlap", "pc_update", "k1e_density", "k1e_product"]
 # kernels launched per stage invocation (bse_api.cu): split-K GEMMs launch GEMM + reduce, pair list 1 kernel

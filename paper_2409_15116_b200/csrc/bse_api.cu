@@ -385,10 +385,13 @@ int alloc_batch_ws(bse_handle *h, long long pb) {
 // tau store of the REAL / PW modes (grow-only); BSE_TAU_STREAM uses the PW store as a transient that is refilled inside
 // every apply call (tau(G) is 16 N / N_pw_h ~ 16x smaller than tau(r), which stays streamed in batches)
 int ensure_tau_store(bse_handle *h, bool real) {
-    const size_t need = real ? (size_t)h->Pa * h->N * 8 : (size_t)h->Pa * h->fft.npw_h * 16;
-    if (need <= h->tau_bytes && (real ? h->tau_r != nullptr : h->tau_g != nullptr)) return BSE_OK;
+    const bool f32 = !real && (h->flags & BSE_TAU_F32);         // tau(G) kept as complex64 (single precision)
+    const size_t need = real ? (size_t)h->Pa * h->N * 8 : (size_t)h->Pa * h->fft.npw_h * (f32 ? 8 : 16);
+    const bool have = real ? h->tau_r != nullptr : (f32 ? h->tau_g32 != nullptr : h->tau_g != nullptr);
+    if (need <= h->tau_bytes && have) return BSE_OK;
     cudaFree(h->tau_r); h->tau_r = nullptr;
     cudaFree(h->tau_g); h->tau_g = nullptr;
+    cudaFree(h->tau_g32); h->tau_g32 = nullptr;
     h->tau_bytes = 0;
     size_t free_b = 0, total_b = 0;
     cudaMemGetInfo(&free_b, &total_b);
@@ -400,6 +403,7 @@ int ensure_tau_store(bse_handle *h, bool real) {
         return BSE_ENOMEM;
     }
     if (real) BSE_CUDA(cudaMalloc(&h->tau_r, need));
+    else if (f32) BSE_CUDA(cudaMalloc(&h->tau_g32, need));
     else BSE_CUDA(cudaMalloc(&h->tau_g, need));
     h->tau_bytes = need;
     return BSE_OK;
@@ -412,7 +416,11 @@ int fill_tau_store(bse_handle *h, bool real) {
     for (long long p0 = 0; p0 < h->Pa; p0 += h->Pb) {
         const int cnt = (int)std::min<long long>(h->Pb, h->Pa - p0);
         if (real) rc = run_pair_batch(h, plist, p0, cnt, h->T, h->tau_r + p0 * h->N);
-        else rc = run_pair_batch(h, plist, p0, cnt, h->tau_g + p0 * h->fft.npw_h, nullptr);
+        else if (h->tau_g32) {                                   // the batch in double (workspace T), rounded once into the store
+            rc = run_pair_batch(h, plist, p0, cnt, h->T, nullptr);
+            if (!rc) rc = bse_launch_to_f32((const double *)h->T, (float *)(h->tau_g32 + p0 * h->fft.npw_h),
+                                            2 * (long long)cnt * h->fft.npw_h, h->stream);
+        } else rc = run_pair_batch(h, plist, p0, cnt, h->tau_g + p0 * h->fft.npw_h, nullptr);
         if (rc) return rc;
     }
     cudaEventRecord(h->ev_fill1, h->stream);
@@ -528,12 +536,14 @@ int plan_apply_memory(bse_handle *h, int B, bool allow_slab = true, bool mix = f
         (slab_forced || !one_group)) {
         const FftPlan &pl = *h->ap;
         const double avail_s = 0.92 * (double)free_b - 512.0 * 1048576.0;
-        // the slab split n_a = S * M (any factorisation with M <= 32, fft_kernels.cuh): the fewest slabs whose working set fits,
+        // the slab split n_a = S * M (any factorisation with M <= 16 and S <= 16, fft_slab.cuh): the fewest slabs whose working set fits,
         // because every slab sweeps all coefficient arrays once.  dbg_slab_planes caps M (tests: several slabs on small grids).
         long long rc = 0, pz = 0;
         int Ssel = 0, Msel = 0;
         double SN8 = 0.0;
-        for (int M = std::min(pl.n, 32); M >= 1; --M) {
+        // M <= 16: 32 M <= 512 threads per CTA keeps the slab stick kernels at two CTAs per SM with 128 registers; measured at
+        // cfg 5 (complex64 store, where memory would allow more): M = 20 costs 114 ms per sweep against 73 ms at M = 15
+        for (int M = std::min(pl.n, 16); M >= 1; --M) {
             if (pl.n % M || pl.n / M > 16) continue;           // the slab stick kernels keep <= 16 folded terms per thread
             if (h->dbg_slab_planes >= 1 && M > h->dbg_slab_planes) continue;
             SN8 = 8.0 * (double)M * pl.n * pl.n;
@@ -735,7 +745,7 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
         for (int c0 = 0; c0 < bt.nu; c0 += (int)h->Pb) {              // tau(G) -> tau(r) of the batch's pairs
             const int c = (int)std::min<long long>(h->Pb, bt.nu - c0);
             { StageTimer t(h, BSE_ST_INV_STICK, uniq * c * m.stick_flops, uniq * c * m.g, uniq * c * m.z);
-              if ((rc = bse_launch_inv_stick(pl, h->tau_g, c, h->Z, h->stream, h->batch_pairs, bt.u0 + c0))) return rc; }
+              if ((rc = bse_launch_inv_stick(pl, h->tau_g, c, h->Z, h->stream, h->batch_pairs, bt.u0 + c0, h->tau_g32))) return rc; }
             { StageTimer t(h, BSE_ST_INV_PLANE, uniq * c * m.plane_flops, uniq * c * m.N8, uniq * c * m.z);
               if ((rc = bse_launch_inv_plane(pl, h->Z, c, pl.N, h->tau_batch + (long long)c0 * pl.N, h->stream))) return rc; }
         }
@@ -779,11 +789,12 @@ int apply_pw_slab(bse_handle *h, const double2 *a, double2 *out, int B) {
     const double share = (double)M / pl.n;               // one slab's share of a whole-field pass
     const long long nloc = h->row1 - h->row0;            // out holds the owned rows only: [B][nloc][npw_h]
     int rc;
-    auto to_slab = [&](const double2 *src, long long fields, double *dst, int s) -> int {
+    auto to_slab = [&](const double2 *src, long long fields, double *dst, int s, const float2 *src32 = nullptr) -> int {
         for (long long f0 = 0; f0 < fields; f0 += h->slab_pz) {
             const int cnt = (int)std::min<long long>(h->slab_pz, fields - f0);
             { StageTimer t(h, BSE_ST_INV_STICK, cnt * m.stick_flops * share, cnt * m.g * share, cnt * m.z * share);
-              if (int r = bse_launch_inv_stick_slab(pl, S, M, src + f0 * npw_h, cnt, h->Z, h->stream, s)) return r; }
+              if (int r = bse_launch_inv_stick_slab(pl, S, M, src32 ? nullptr : src + f0 * npw_h, cnt, h->Z, h->stream, s, nullptr, 0,
+                                                    src32 ? src32 + f0 * npw_h : nullptr)) return r; }
             { StageTimer t(h, BSE_ST_INV_PLANE, cnt * m.plane_flops * share, cnt * m.N8 * share, cnt * m.z * share);
               if (int r = bse_launch_inv_plane(pl, h->Z, cnt, SN, dst + f0 * SN, h->stream, false, M)) return r; }
         }
@@ -808,7 +819,7 @@ int apply_pw_slab(bse_handle *h, const double2 *a, double2 *out, int B) {
     }
     for (int s = 0; s < S; ++s) {
         if ((rc = to_slab(a, (long long)B * Nv, h->a_r, s))) return rc;
-        if ((rc = to_slab(h->tau_g, h->Pa, h->tau_batch, s))) return rc;
+        if ((rc = to_slab(h->tau_g, h->Pa, h->tau_batch, s, h->tau_g32))) return rc;
         if (h->mix_on) {
             if ((rc = to_slab(h->uG, Nv, u_slab, s))) return rc;
             if ((rc = to_slab(vG, B, vH_slab, s))) return rc;
@@ -903,6 +914,10 @@ extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cel
     for (int a = 0; a < Npdep; ++a)
         if (!(lambda[a] < 1.0)) { bse_set_error("lambda >= 1"); return BSE_EINVAL; }
     if ((flags & BSE_TAU_MASK) == 3u) { bse_set_error("bad tau storage flag"); return BSE_EINVAL; }
+    if ((flags & BSE_TAU_F32) && (flags & BSE_TAU_MASK) == BSE_TAU_REAL) {
+        bse_set_error("BSE_TAU_F32 needs BSE_TAU_PW or BSE_TAU_STREAM");
+        return BSE_EINVAL;
+    }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         bse_set_error("no CUDA device: this library has no CPU fallback");
@@ -994,7 +1009,7 @@ extern "C" int bse_destroy(bse_handle *h) {
     free_plan(h->ffta);
     cudaFree(h->u_owned); cudaFree(h->phi_owned); cudaFree(h->f2); cudaFree(h->Mmat); cudaFree(h->rowcnt);
     cudaFree(h->rowptr); cudaFree(h->pid); cudaFree(h->pairs); cudaFree(h->adj_ptr); cudaFree(h->adj);
-    cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);
+    cudaFree(h->tau_r); cudaFree(h->tau_g); cudaFree(h->tau_g32); cudaFree(h->Z); cudaFree(h->X); cudaFree(h->T); cudaFree(h->Dm);
     cudaFree(h->part); cudaFree(h->Sov); cudaFree(h->tau_batch); cudaFree(h->a_dev); cudaFree(h->out_dev);
     cudaFree(h->uG); cudaFree(h->uGw); cudaFree(h->a_r); cudaFree(h->acc_r);
     cudaFree(h->batch_pairs); cudaFree(h->eslot); cudaFree(h->rowlist); cudaFree(h->rowid); cudaFree(h->pairs_act); cudaFree(h->eslot_act); cudaFree(h->k1e_ws); cudaFree(h->u_a); cudaFree(h->Ut); cudaFree(h->accG);
@@ -1391,7 +1406,7 @@ extern "C" int bse_get_tau(bse_handle *h, long long first, long long count, doub
         BSE_CUDA(cudaMemcpyAsync(dst, h->tau_r + first * h->N, (size_t)count * h->N * 8, cudaMemcpyDeviceToDevice, h->stream));
         return BSE_OK;
     }
-    if (layout == BSE_TAU_PW && mode == BSE_TAU_PW && !h->rows_set) {
+    if (layout == BSE_TAU_PW && mode == BSE_TAU_PW && !h->rows_set && !h->tau_g32) {
         BSE_CUDA(cudaMemcpyAsync(dst, h->tau_g + first * npw_h, (size_t)count * npw_h * 16, cudaMemcpyDeviceToDevice, h->stream));
         return BSE_OK;
     }

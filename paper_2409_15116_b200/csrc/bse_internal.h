@@ -76,6 +76,7 @@ struct bse_handle {
     // tau store
     double *tau_r = nullptr;         // [P][N]
     double2 *tau_g = nullptr;        // [P][npw_h]
+    float2 *tau_g32 = nullptr;       // [P][npw_h] single-precision store (BSE_TAU_F32) instead of tau_g
     size_t tau_bytes = 0;            // capacity of the store (grow-only)
     // workspaces (sized for a pair batch)
     long long Pb = 0;                // pair-batch capacity
@@ -158,15 +159,16 @@ int bse_launch_fwd_plane(const FftPlan &pl, const double *fields, const int2 *pa
 int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2 *X, const double *scale,
                          cudaStream_t s, const int *scatter = nullptr);
 // gather != nullptr: field p is read from T + gather[g0 + p] * npw_h (pair indices of a row batch)
+// T32 != nullptr: read the coefficients from this single-precision copy instead of T (BSE_TAU_F32)
 int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2 *Z, cudaStream_t s,
-                         const int *gather = nullptr, int g0 = 0);
+                         const int *gather = nullptr, int g0 = 0, const float2 *T32 = nullptr);
 // subtract: out <- out - transform instead of out <- transform (P_c update of the REAL layout)
 int bse_launch_inv_plane(const FftPlan &pl, const double2 *Z, int count, long long N, double *out, cudaStream_t s,
                          bool subtract = false, int np = 0);
 // slab forms of the stick passes (fft_kernels.cuh): the planes i1 = slab + S k, k < M, only (n = S M, M <= 32).  Zs[count][M][NS].
 // forward: field p goes to row (p / rc) * row_ld + row0 + p % rc of X; accumulate: X += (slabs 1 .. R1-1) instead of X =
 int bse_launch_inv_stick_slab(const FftPlan &pl, int S, int M, const double2 *T, int count, double2 *Zs, cudaStream_t s, int slab,
-                              const int *gather = nullptr, int g0 = 0);
+                              const int *gather = nullptr, int g0 = 0, const float2 *T32 = nullptr);
 int bse_launch_fwd_stick_slab(const FftPlan &pl, int S, int M, const double2 *Zs, int count, double2 *X, const double *scale,
                               cudaStream_t s, int slab, bool accumulate, int rc, long long row_ld, long long row0);
 
@@ -200,6 +202,8 @@ int bse_launch_k1_mix(const double *u, const double *vH, double *acc, const int 
 int bse_launch_row_sumsq(const double *x, const double *y, long long len, int rows, double *out, cudaStream_t s);
 // dst[j][i] = src[i][j], n x n, leading dimensions lds / ldd
 int bse_launch_transpose(const double *src, long long lds, double *dst, long long ldd, int n, cudaStream_t s);
+// dst[i] = (float) src[i], count doubles (tau(G) of a pair batch into the single-precision store)
+int bse_launch_to_f32(const double *src, float *dst, long long count, cudaStream_t s);
 // dst[w][k] = Omega * wt * src[w][k], wt = 2 for G != 0 and (1, 0) on (re, im) of G = 0 (entry 0 of H)
 int bse_launch_weight_pw(const double2 *src, double2 *dst, long long npw_h, long long rows, double Omega,
                          cudaStream_t s);

@@ -66,7 +66,7 @@ static int slab_per_cta(int groups, int count) {
     return std::max(1, (count + want - 1) / want);
 }
 int bse_launch_inv_stick_slab(const FftPlan &pl, int S, int M, const double2 *T, int count, double2 *Zs, cudaStream_t s, int slab,
-                              const int *gather, int g0) {
+                              const int *gather, int g0, const float2 *T32) {
     if (count <= 0) return BSE_OK;
     if (S * M != pl.n || M > 32 || M < 1 || S > 16) { bse_set_error("slab stick pass: bad factorisation"); return BSE_EINVAL; }
     const PlanDev P = to_dev(pl);
@@ -75,11 +75,11 @@ int bse_launch_inv_stick_slab(const FftPlan &pl, int S, int M, const double2 *T,
     const int per = slab_per_cta(groups, count);
     const dim3 grid(groups, (count + per - 1) / per);
     const bool small = TS * M <= 512;
-#define BSE_SLAB_PICK(name) \
-    (small ? (S <= 4 ? bsefft::name<4, 512> : (S <= 8 ? bsefft::name<8, 512> : (S <= 12 ? bsefft::name<12, 512> : bsefft::name<16, 512>))) \
-           : (S <= 4 ? bsefft::name<4, 1024> : (S <= 8 ? bsefft::name<8, 1024> : (S <= 12 ? bsefft::name<12, 1024> : bsefft::name<16, 1024>))))
-    auto kern = BSE_SLAB_PICK(inv_stick_slab_kernel);
-    kern<<<grid, TS * M, smem, s>>>(P, pl.n, S, M, A, T, pl.npw_h, Zs, gather, g0, slab, count, per);
+#define BSE_SLAB_PICK(name, ...) \
+    (small ? (S <= 4 ? bsefft::name<4, 512, ##__VA_ARGS__> : (S <= 8 ? bsefft::name<8, 512, ##__VA_ARGS__> : (S <= 12 ? bsefft::name<12, 512, ##__VA_ARGS__> : bsefft::name<16, 512, ##__VA_ARGS__>))) \
+           : (S <= 4 ? bsefft::name<4, 1024, ##__VA_ARGS__> : (S <= 8 ? bsefft::name<8, 1024, ##__VA_ARGS__> : (S <= 12 ? bsefft::name<12, 1024, ##__VA_ARGS__> : bsefft::name<16, 1024, ##__VA_ARGS__>))))
+    auto kern = T32 ? BSE_SLAB_PICK(inv_stick_slab_kernel, true) : BSE_SLAB_PICK(inv_stick_slab_kernel, false);
+    kern<<<grid, TS * M, smem, s>>>(P, pl.n, S, M, A, T, pl.npw_h, Zs, gather, g0, slab, count, per, T32);
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }
@@ -105,7 +105,7 @@ int bse_launch_fwd_stick(const FftPlan &pl, const double2 *Z, int count, double2
     return ((const FftOps *)pl.ops)->fwd_stick(to_dev(pl), Z, count, X, pl.npw_h, scale, s, scatter);
 }
 int bse_launch_inv_stick(const FftPlan &pl, const double2 *T, int count, double2 *Z, cudaStream_t s,
-                         const int *gather, int g0) {
+                         const int *gather, int g0, const float2 *T32) {
     if (count <= 0) return BSE_OK;
-    return ((const FftOps *)pl.ops)->inv_stick(to_dev(pl), T, count, pl.npw_h, Z, s, gather, g0);
+    return ((const FftOps *)pl.ops)->inv_stick(to_dev(pl), T, count, pl.npw_h, Z, s, gather, g0, T32);
 }

@@ -37,6 +37,12 @@ struct PlanDev {
     const int *hmapT;       // [n][NS] (t1 = m1 mod n, stick) -> h in H, -1 outside the sphere, -2-h: conj of entry h
 };
 
+// coefficient h of a field kept in double (t) or, when t32 != nullptr, in single precision
+__device__ __forceinline__ double2 ldcoef(const double2 *t, const float2 *t32, int h) {
+    if (t32) { const float2 f = t32[h]; return make_double2((double)f.x, (double)f.y); }
+    return t[h];
+}
+
 template <int R1, int R2>
 struct Geo {
     static constexpr int n = R1 * R2;
@@ -447,10 +453,10 @@ fwd_stick_kernel(PlanDev P, const double2 *__restrict__ Z, double2 *__restrict__
     }
 }
 
-template <int R1, int R2>
+template <int R1, int R2, bool F32>
 __global__ void __launch_bounds__(256)
 inv_stick_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, double2 *__restrict__ Z,
-                 const int *__restrict__ gather, int g0) {
+                 const int *__restrict__ gather, int g0, const float2 *__restrict__ T32) {
     using G = Geo<R1, R2>;
     constexpr int n = G::n, LDS = G::LDS, R2p = G::R2p, TS = G::TS;
     extern __shared__ __align__(16) unsigned char smem[];
@@ -459,7 +465,10 @@ inv_stick_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, doub
     const int NS = P.NS;
     const int s0 = blockIdx.x * TS;
     const long long p = blockIdx.y;
-    const double2 *tg = T + (gather ? (long long)gather[g0 + p] : p) * npw_h;
+    // T32 != nullptr: the coefficients are kept in single precision (BSE_TAU_F32) and widened on load
+    const long long toff = (gather ? (long long)gather[g0 + p] : p) * npw_h;
+    const double2 *tg = T + toff;
+    const float2 *tg32 = F32 ? T32 + toff : nullptr;
     for (int task = threadIdx.x; task < TS * R2; task += blockDim.x) {
         const int j = task / TS, sl = task - j * TS;
         const int s = s0 + sl;
@@ -469,8 +478,8 @@ inv_stick_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, doub
         for (int q = 0; q < R1; ++q) {
             const int code = P.hmapT[(j + q * R2) * NS + s];
             double2 v = make_double2(0.0, 0.0);
-            if (code >= 0) v = tg[code];
-            else if (code <= -2) { v = tg[-2 - code]; v.y = -v.y; }
+            if (code >= 0) v = F32 ? ldcoef(tg, tg32, code) : tg[code];
+            else if (code <= -2) { v = F32 ? ldcoef(tg, tg32, -2 - code) : tg[-2 - code]; v.y = -v.y; }
             x[q] = v;
         }
         Dft<R1, +1>::run(x);
@@ -501,7 +510,7 @@ struct FftOps {
     int (*fwd_plane)(const PlanDev &, const double *, const int2 *, long long, int, long long, double2 *, cudaStream_t);
     int (*inv_plane)(const PlanDev &, const double2 *, int, long long, double *, cudaStream_t, int, int);
     int (*fwd_stick)(const PlanDev &, const double2 *, int, double2 *, long long, const double *, cudaStream_t, const int *);
-    int (*inv_stick)(const PlanDev &, const double2 *, int, long long, double2 *, cudaStream_t, const int *, int);
+    int (*inv_stick)(const PlanDev &, const double2 *, int, long long, double2 *, cudaStream_t, const int *, int, const float2 *);
 };
 
 inline int plane_threads(int tasks) {
@@ -582,13 +591,15 @@ struct Launch {
         return BSE_OK;
     }
     static int inv_stick(const PlanDev &P, const double2 *T, int count, long long npw_h, double2 *Z, cudaStream_t s,
-                         const int *gather, int g0) {
-        int rc = set_smem((const void *)inv_stick_kernel<R1, R2>, G::stick_smem);
+                         const int *gather, int g0, const float2 *T32) {
+        auto kern = T32 ? inv_stick_kernel<R1, R2, true> : inv_stick_kernel<R1, R2, false>;
+        int rc = set_smem((const void *)kern, G::stick_smem);
         if (rc) return rc;
         for (int c0 = 0; c0 < count; c0 += 65535) {
             const int c = count - c0 < 65535 ? count - c0 : 65535;
-            inv_stick_kernel<R1, R2><<<dim3((P.NS + G::TS - 1) / G::TS, c), 256, G::stick_smem, s>>>(
-                P, gather ? T : T + (long long)c0 * npw_h, npw_h, Z + (long long)c0 * G::n * P.NS, gather, g0 + c0);
+            kern<<<dim3((P.NS + G::TS - 1) / G::TS, c), 256, G::stick_smem, s>>>(
+                P, gather ? T : T + (long long)c0 * npw_h, npw_h, Z + (long long)c0 * G::n * P.NS, gather, g0 + c0,
+                (T32 && !gather) ? T32 + (long long)c0 * npw_h : T32);
         }
         BSE_CUDA(cudaGetLastError());
         return BSE_OK;

@@ -74,10 +74,11 @@ __device__ __forceinline__ double2 slab_dft(const double2 *C, double2 *D, const 
 // costs one round of independent, stick-coalesced gathers (no index load in front of them).  S <= 16.
 // NQ = S rounded up to a multiple of 4 (template: the index registers are a compile-time array); MAXT = 512 or 1024 bounds the
 // CTA (32 M threads), so that slabs of <= 16 planes get 128 registers per thread.
-template <int NQ, int MAXT>
+template <int NQ, int MAXT, bool F32>
 __global__ void __launch_bounds__(MAXT)
 inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__restrict__ T, long long npw_h,
-                      double2 *__restrict__ Zs, const int *__restrict__ gather, int g0, int slab, int count, int per_cta) {
+                      double2 *__restrict__ Zs, const int *__restrict__ gather, int g0, int slab, int count, int per_cta,
+                      const float2 *__restrict__ T32) {
     constexpr int TS = SLAB_TS, LDT = TS + 1;
     extern __shared__ __align__(16) unsigned char smem[];
     double2 *C = reinterpret_cast<double2 *>(smem);
@@ -95,7 +96,9 @@ inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
     const int ti0 = (slab * j) % n, tstep = (slab * M) % n;     // (slab * t1) mod n for t1 = j + q M
     const int p_end = min(count, (int)(blockIdx.y + 1) * per_cta);
     for (int p = blockIdx.y * per_cta; p < p_end; ++p) {
-        const double2 *tg = T + (gather ? (long long)gather[g0 + p] : (long long)p) * npw_h;
+        const long long toff = (gather ? (long long)gather[g0 + p] : (long long)p) * npw_h;
+        const double2 *tg = T + toff;
+        const float2 *tg32 = F32 ? T32 + toff : nullptr;        // coefficients kept in single precision (BSE_TAU_F32)
         double2 y = make_double2(0.0, 0.0);
         int ti = ti0;
 #pragma unroll
@@ -105,8 +108,13 @@ inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
             for (int u = 0; u < 4; ++u) {
                 const int c = code[q0 + u];
                 v[u] = make_double2(0.0, 0.0);
-                if (c >= 0) v[u] = tg[c];
-                else if (c <= -2) { v[u] = tg[-2 - c]; v[u].y = -v[u].y; }
+                if (F32) {
+                    if (c >= 0) { const float2 f = tg32[c]; v[u] = make_double2((double)f.x, (double)f.y); }
+                    else if (c <= -2) { const float2 f = tg32[-2 - c]; v[u] = make_double2((double)f.x, -(double)f.y); }
+                } else {
+                    if (c >= 0) v[u] = tg[c];
+                    else if (c <= -2) { v[u] = tg[-2 - c]; v[u].y = -v[u].y; }
+                }
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {

@@ -290,7 +290,18 @@ __global__ void weight_pw_kernel(const double2 *__restrict__ src, double2 *__res
     dst[i] = (i % npw_h == 0) ? make_double2(Omega * c.x, 0.0) : make_double2(2.0 * Omega * c.x, 2.0 * Omega * c.y);
 }
 
+__global__ void to_f32_kernel(const double *__restrict__ src, float *__restrict__ dst, long long count) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < count) dst[i] = (float)src[i];
+}
+
 }  // namespace
+
+int bse_launch_to_f32(const double *src, float *dst, long long count, cudaStream_t s) {
+    to_f32_kernel<<<(unsigned)((count + 255) / 256), 256, 0, s>>>(src, dst, count);
+    BSE_CUDA(cudaGetLastError());
+    return BSE_OK;
+}
 
 int bse_launch_weight_pw(const double2 *src, double2 *dst, long long npw_h, long long rows, double Omega,
                          cudaStream_t s) {

@@ -653,3 +653,49 @@ def test_sharded_driver_single_rank():
             assert np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum()) <= TOL
     finally:
         sh.close()
+
+
+@pytest.mark.parametrize("tau", ["pw", "stream"])
+def test_single_precision_tau_store(tau):
+    """Mixed-precision variant (BSE_TAU_F32): tau(G) computed in fp64 and kept as complex64.  Against the oracle
+    with the same single rounding (tau_G_f32) the K1x output agrees to ~1e-9 (the two sides may round a coefficient that sits
+    on a binary32 tie differently: 2^-24 on that one coefficient); against the all-double oracle the error is the rounding
+    itself, 2^-24 = 6e-8 relative per coefficient, i.e. between 1e-9 and 2e-7 in the L2 norm - derived from the arithmetic, not
+    the 1e-10 bar of the double store.  Slab path and group path."""
+    bse = _bse()
+    flag = {"pw": bse.BSE_TAU_PW, "stream": bse.BSE_TAU_STREAM}[tau] | bse.BSE_TAU_F32 | bse.BSE_VEC_PW
+    cfg = wl.Config("f32", 10.0, 24, 9, 20, 8.0, 1.2, 0.8, 3.0, 0.02, 3, "random", seed=77)
+    w = wl.make(cfg=cfg)
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    pairs, _ = orc.screen_pairs(w.u, w.eta)
+    phiS = tab.expand_H_to_S(w.phi)
+    tau32 = np.array([tab.to_r(orc.tau_G_f32(tab, w.u[v], w.u[x], phiS, w.lam)) for v, x in pairs])
+    tau64 = orc.build_tau(tab, w.u, w.phi, w.lam, pairs, want="r")
+    ref32 = orc.apply_k1x_pw(tab, w.u, pairs, tau32, w.a_pw)
+    ref64 = orc.apply_k1x_pw(tab, w.u, pairs, tau64, w.a_pw)
+    wt = np.full(tab.npw_h, 2.0)
+    wt[0] = 1.0
+
+    def err(got, ref):
+        return float(np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum()))
+    assert 1e-9 < err(ref32, ref64) < 2e-7
+    for knobs in (None, {"slab_planes": 6, "slab_rows": 4}):
+        g = Gpu(w, flag, knobs)
+        try:
+            assert np.array_equal(g.build(), pairs)
+            a_d = torch.from_numpy(np.ascontiguousarray(w.a_pw).view(np.float64)).to("cuda:0")
+            out = torch.empty_like(a_d)
+            bse.bse_apply_k1x(g.h, a_d, out, w.a_pw.shape[0])
+            torch.cuda.synchronize()
+            got = out.cpu().numpy().view(np.complex128).reshape(ref32.shape)
+            assert err(got, ref32) <= 2e-9, err(got, ref32)
+            assert 1e-9 < err(got, ref64) < 2e-7
+            # bse_get_tau still hands out the double values
+            assert rel(g.tau_g(0, 3), orc.build_tau(tab, w.u, w.phi, w.lam, pairs[:3], want="G")) <= TOL
+        finally:
+            g.close()
+    u = torch.from_numpy(w.u).cuda()
+    phi = torch.from_numpy(np.ascontiguousarray(w.phi).view(np.float64)).cuda()
+    with pytest.raises(bse.BseError) as e:
+        bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u, w.phi.shape[0], phi, w.lam, w.eta, bse.BSE_TAU_REAL | bse.BSE_TAU_F32)
+    assert e.value.code == bse.BSE_EINVAL

@@ -368,3 +368,18 @@ def test_P17_rotation_covariance_of_k1x_and_k1e():
     e = orc.apply_k1e_real(tab, w.u, a)
     e2 = orc.apply_k1e_real(tab, u2, a2)
     assert np.linalg.norm(e2 - orc.rotate(U, e)) <= 1e-11 * np.linalg.norm(e)
+
+
+def test_p18_single_precision_store_is_one_rounding_of_the_double_value():
+    """tau_G_f32 (PAPER.md:279 reading): each component is an exactly representable binary32 number and differs from the fp64
+    pair integral by at most half a unit in the last place of binary32 (relative 2^-24)."""
+    w = wl.make(1)
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    phiS = tab.expand_H_to_S(w.phi)
+    t64 = orc.tau_G(tab, w.u[0], w.u[3], phiS, w.lam)
+    t32 = orc.tau_G_f32(tab, w.u[0], w.u[3], phiS, w.lam)
+    for a, b in ((t64.real, t32.real), (t64.imag, t32.imag)):
+        assert np.array_equal(b.astype(np.float32).astype(np.float64), b)
+        nz = np.abs(a) > 1e-30
+        assert np.all(np.abs(a[nz] - b[nz]) <= 2.0 ** -24 * np.abs(a[nz]) * (1 + 1e-12))
+        assert np.any(a[nz] != b[nz])
