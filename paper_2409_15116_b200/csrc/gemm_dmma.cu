@@ -35,11 +35,11 @@ __device__ __forceinline__ void dmma(double &c0, double &c1, double a, double b)
 template <int ROWS, int NT>
 __device__ __forceinline__ void load_tile_k(double *sm, const double *g, long long ld, int rows, int r0,
                                             long long k0, long long kend) {
-    // ROWS rows x 8 chunks of 16 B, NT threads
+    // ROWS rows x BK/2 chunks of 16 B, NT threads
 #pragma unroll
-    for (int i = 0; i < ROWS * 8 / NT; ++i) {
+    for (int i = 0; i < ROWS * (BK / 2) / NT; ++i) {
         const int c = threadIdx.x + i * NT;
-        const int r = c >> 3, kc = (c & 7) * 2;
+        const int r = c / (BK / 2), kc = (c % (BK / 2)) * 2;
         const long long left = kend - (k0 + kc);
         const bool ok = (r0 + r < rows) && (left > 0);
         const double *src = ok ? g + (long long)(r0 + r) * ld + k0 + kc : g;
@@ -50,9 +50,9 @@ __device__ __forceinline__ void load_tile_k(double *sm, const double *g, long lo
 template <int NT>
 __device__ __forceinline__ void load_tile_n(double *sm, const double *g, long long ld, long long cols, long long c0,
                                             int k0, int kend) {
-    // 16 rows x 32 chunks = 512 chunks
+    // BK rows x 32 chunks
 #pragma unroll
-    for (int i = 0; i < 512 / NT; ++i) {
+    for (int i = 0; i < BK * 32 / NT; ++i) {
         const int c = threadIdx.x + i * NT;
         const int r = c >> 5, cc = (c & 31) * 2;
         const long long left = cols - (c0 + cc);
@@ -124,8 +124,8 @@ dgemm_kernel(const double *__restrict__ A, long long lda, const double *__restri
         }
         cp_commit();
     };
-    issue(0);
-    issue(1);
+#pragma unroll
+    for (int i = 0; i < STAGES - 1; ++i) issue(i);
     for (int kt = 0; kt < nk; ++kt) {
         cp_wait<STAGES - 2>();
         __syncthreads();
