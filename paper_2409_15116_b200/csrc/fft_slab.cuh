@@ -13,7 +13,7 @@ namespace bsefft {
 // so every slab costs one fold over the (at most 2R+1) non-zero coefficients of a stick plus one M-point transform, all
 // slabs together S sweeps over the coefficients on H, and the forward pass ACCUMULATES its slab's contribution into X (slab 0
 // stores).  The host picks the smallest S whose slab fits the free memory (fewest sweeps).  Zs[p][k][NS].
-// CTA = TS sticks of one field, TS * M threads (M <= 32): thread (j, stick) folds residue class j (<= S stick-coalesced
+// CTA = TS sticks of one field, TS * M threads (the plan keeps M <= 16: 512 threads, two CTAs per SM): thread (j, stick) folds residue class j (<= S stick-coalesced
 // gathers, four in flight at a time).  The M-point transform runs out of shared memory as two passes of the split
 // M = A B (A + B terms per thread instead of M), input index j = j1 B + j2, output index k = k1 + A k2:
 //   z[k1][j2] = w_M^{k1 j2} sum_{j1 < A} y[j1 B + j2] w_A^{k1 j1},      x[k1 + A k2] = sum_{j2 < B} z[k1][j2] w_B^{k2 j2}

@@ -78,3 +78,25 @@ def test_jade_makes_the_screen_effective():
         finally:
             bse.bse_destroy(h)
     assert counts[1] < counts[0] and counts[1] <= len(orc.screen_pairs(w.u, w.eta)[0]) + 2
+
+
+def test_jade_many_orbitals_two_sweeps():
+    """N_v = 520 (> 512: the round kernels run over several CTAs, 519 rounds of 260 pairs per sweep): two sweeps from the
+    identity against the oracle's two sweeps, element by element (no sign freedom without the eigenvector start)."""
+    from paper_2409_15116_b200 import bse
+    Nv, n, L = 520, 24, 10.0
+    rng = np.random.default_rng(77)
+    Q, _ = np.linalg.qr(rng.normal(size=(n ** 3, Nv)))
+    psi = np.ascontiguousarray(Q.T) / np.sqrt(L ** 3 / n ** 3)            # orthonormal: dV sum_r psi_v psi_w = delta
+    A = jo.position_matrices(psi, n, L)
+    V, Ad = jo.jade(A, init="identity", tol=0.0, max_sweeps=2)
+    psi_d = torch.from_numpy(psi).cuda()
+    U_d = torch.empty((Nv, Nv), dtype=torch.float64, device="cuda:0")
+    sweeps, s0, s1 = bse.bse_jade([n] * 3, np.eye(3) * L, Nv, psi_d, U_d, None, tol=0.0, max_sweeps=2, init_eig=False)
+    torch.cuda.synchronize()
+    U = U_d.cpu().numpy()
+    assert sweeps == 2
+    assert np.abs(U - V.T).max() < 1e-10
+    assert np.abs(U @ U.T - np.eye(Nv)).max() < 1e-12
+    const = 3.0 * Nv - sum((a * a).sum() for a in A)
+    assert abs(s0 - (const + jo.off_sum(A))) < 1e-8 and abs(s1 - (const + jo.off_sum(Ad))) < 1e-8 and s1 < s0
