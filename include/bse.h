@@ -136,12 +136,18 @@ int bse_k1e_from_hartree(bse_handle *h, const double *vG, int v0, int v1, int B,
 
 /* Same with HOST pointers: copies a to the device, applies, copies out back, synchronises (the end-to-end
  * call bench.py times as `e2e`).  With BSE_TAU_REAL the blocks are pipelined: block b+1 is copied in and block b-1
- * copied out (two copy streams) while block b is applied.  Pinned host memory is needed for the overlap. */
+ * copied out (two copy streams) while block b is applied.  In the other storage modes the copy of a runs on a copy
+ * stream while tau is rebuilt (BSE_TAU_STREAM), and every row chunk that P_c has finished is copied out on the second copy
+ * stream while the next chunk is projected.  Pinned host memory is needed for the overlap. */
 int bse_apply_k1x_host(bse_handle *h, const double *a_host, double *out_host, int B);
 
 /* Replace u and/or phi (either may be NULL) of a handle created with BSE_PTR_HOST by new HOST arrays of the same sizes:
- * host-to-device copy into the buffers the handle owns, enqueued on its stream, nothing reallocated.  tau is invalidated
- * (call bse_build_tau again).  BSE_ESTATE if the handle borrows device arrays. */
+ * host-to-device copy into the buffers the handle owns, nothing reallocated.  The copy is ENQUEUED (a copy stream of the
+ * handle, ordered after the work already on its stream) and the call returns: with pinned host memory the arrays must stay
+ * unchanged until the next call on this handle that synchronises (bse_build_tau + bse_get_pairs, bse_apply_k1x_host, ...).
+ * u goes in column slabs (all orbitals on a range of grid points), and the bse_build_tau that follows screens each slab as
+ * it arrives (a1 is a sum over grid points), so the copy hides the screen.  tau is invalidated (call bse_build_tau again).
+ * BSE_ESTATE if the handle borrows device arrays. */
 int bse_set_inputs_host(bse_handle *h, const double *u_host, const double *phi_host);
 
 int bse_destroy(bse_handle *h);
@@ -162,7 +168,9 @@ int bse_get_tau(bse_handle *h, long long first, long long count, double *dst, un
  * layout, "max_batch" caps the pairs of one row batch (so that small cases exercise the multi-group / multi-batch paths of
  * the large configurations; 0 = no cap);  "compact_inv" = k forces the compact inverse plane kernel sized for k CTAs per SM
  * (0 = never, -1 = automatic);  "slab_rows" = k caps the rows per chunk of the plane-slab apply (PW layout with tau on H; -1 = never
- * take that path, 0 = no cap), "slab_planes" = k the planes per slab; setting "max_group" or "max_batch" also keeps the apply on the group / row-batch path.
+ * take that path, 0 = no cap), "slab_planes" = k the planes per slab; setting "max_group" or "max_batch" also keeps the apply on the group / row-batch path;
+ * "pc_rows" = k caps the rows P_c projects per chunk (0 = no cap); "in_chunks" = k makes bse_set_inputs_host copy u in k
+ * column slabs (0 = automatic: 8 from 256 MB on, else 1).
  * BSE_EINVAL for an unknown key. */
 int bse_debug_set(bse_handle *h, const char *key, long long value);
 /* Per-stage device time (CUDA events on the library's stream).  enable != 0 switches recording on (adds a

@@ -191,11 +191,11 @@ int st_inv_plane(bse_handle *h, const FftPlan &pl, int cnt, double *out) {
 }
 // C[M][Nn] = alpha colscale[n] sum_k A[m][k] B[n][k]   (split-K DMMA)
 int st_gemm_dot(bse_handle *h, int stage, const double *A, long long lda, const double *B, long long ldb, int M, int Nn,
-                long long K, bool sq, double *C, long long ldc, double alpha, const double *colscale) {
+                long long K, bool sq, double *C, long long ldc, double alpha, const double *colscale, bool accumulate = false) {
     const double flops = sq ? (double)M * (Nn + 1) * (double)K : 2.0 * M * Nn * (double)K;
     const double bytes = sq ? 8.0 * M * (double)K : 8.0 * ((double)M * K + (double)Nn * K);
     StageTimer t(h, stage, flops, bytes);
-    return bse_gemm_dot(A, lda, B, ldb, M, Nn, K, sq, sq, h->part, h->part_bytes, C, ldc, alpha, colscale, h->stream);
+    return bse_gemm_dot(A, lda, B, ldb, M, Nn, K, sq, sq, h->part, h->part_bytes, C, ldc, alpha, colscale, h->stream, accumulate);
 }
 // NN form with the EPI_TAU / EPI_SUB epilogue: reads A [M][K], B [K][Nn], one [M][Nn] operand, writes [M][Nn]
 int st_gemm_nn(bse_handle *h, int stage, const double *A, long long lda, const double *B, long long ldb, int M,
@@ -253,12 +253,19 @@ int p_c_rows(bse_handle *h, double *x, long long rows, long long K, const double
     long long mc = rows;
     const long long per_row = (long long)h->Nv * 8 * 2;
     if (rows * per_row > (long long)h->part_bytes) mc = std::max<long long>(64, (long long)(h->part_bytes / per_row) / 64 * 64);
+    if (h->dbg_pc_rows >= 1) mc = std::min(mc, h->dbg_pc_rows);
     for (long long r0 = 0; r0 < rows; r0 += mc) {
         const int m = (int)std::min(mc, rows - r0);
         if ((rc = st_gemm_dot(h, BSE_ST_PC_OVERLAP, x + r0 * K, K, ub, K, m, h->Nv, K, false, h->Sov + r0 * lds, lds,
                               alpha, nullptr))) return rc;
         if ((rc = st_gemm_nn(h, BSE_ST_PC_UPDATE, h->Sov + r0 * lds, lds, uk, K, m, K, h->Nv, EPI_SUB, nullptr, nullptr,
                              x + r0 * K, K))) return rc;
+        if (h->d2h_host && x == h->out_dev && r0 == h->d2h_rows_done) {      // rows [r0, r0 + m) are final: send them off
+            BSE_CUDA(cudaEventRecord(h->ev_d2h, h->stream));
+            BSE_CUDA(cudaStreamWaitEvent(h->s_out, h->ev_d2h, 0));
+            BSE_CUDA(cudaMemcpyAsync(h->d2h_host + r0 * K, x + r0 * K, (size_t)m * K * 8, cudaMemcpyDeviceToHost, h->s_out));
+            h->d2h_rows_done = r0 + m;
+        }
     }
     return BSE_OK;
 }
@@ -1005,6 +1012,8 @@ extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cel
 extern "C" int bse_destroy(bse_handle *h) {
     if (!h) return BSE_OK;
     cudaStreamSynchronize(h->stream);
+    if (h->s_in) cudaStreamSynchronize(h->s_in);
+    if (h->s_out) cudaStreamSynchronize(h->s_out);
     free_plan(h->fft);
     free_plan(h->ffta);
     cudaFree(h->u_owned); cudaFree(h->phi_owned); cudaFree(h->f2); cudaFree(h->Mmat); cudaFree(h->rowcnt);
@@ -1016,6 +1025,9 @@ extern "C" int bse_destroy(bse_handle *h) {
     for (cudaEvent_t e : h->ev_pipe) cudaEventDestroy(e);
     if (h->s_in) cudaStreamDestroy(h->s_in);
     if (h->s_out) cudaStreamDestroy(h->s_out);
+    if (h->ev_d2h) cudaEventDestroy(h->ev_d2h);
+    if (h->ev_in_done) cudaEventDestroy(h->ev_in_done);
+    for (cudaEvent_t e : h->ev_in) cudaEventDestroy(e);
     if (h->ev0) cudaEventDestroy(h->ev0);
     if (h->ev1) cudaEventDestroy(h->ev1);
     if (h->ev_fill0) cudaEventDestroy(h->ev_fill0);
@@ -1041,13 +1053,36 @@ extern "C" int bse_set_rows(bse_handle *h, int v0, int v1) {
     return BSE_OK;
 }
 
+// the library's stream waits for whatever bse_set_inputs_host left in flight on the copy stream
+static int wait_inputs(bse_handle *h) {
+    if (h->inputs_pending) {
+        BSE_CUDA(cudaStreamWaitEvent(h->stream, h->ev_in_done, 0));
+        h->inputs_pending = false;
+    }
+    h->in_chunks = 0;
+    return BSE_OK;
+}
+
 extern "C" int bse_build_tau(bse_handle *h) {
     if (!h) { bse_set_error("null handle"); return BSE_EINVAL; }
     int rc;
     h->built = false;
     // a1: M = (u^2)(u^2)^T, then the threshold decision and the list, all on the device
-    if ((rc = st_gemm_dot(h, BSE_ST_SCREEN, h->u, h->N, h->u, h->N, h->Nv, h->Nv, h->N, true, h->Mmat, h->Nv, 1.0,
-                          nullptr))) return rc;
+    if (h->inputs_pending && h->in_chunks > 1) {
+        // u is still arriving from the host in column slabs: M accumulates slab after slab (the sum over grid points in
+        // slab order), so the copy hides the screen
+        for (int c = 0; c < h->in_chunks; ++c) {
+            const long long k0 = c * h->in_kc, kc = std::min<long long>(h->in_kc, h->N - k0);
+            BSE_CUDA(cudaStreamWaitEvent(h->stream, h->ev_in[c], 0));
+            if ((rc = st_gemm_dot(h, BSE_ST_SCREEN, h->u + k0, h->N, h->u + k0, h->N, h->Nv, h->Nv, kc, true, h->Mmat, h->Nv,
+                                  1.0, nullptr, c > 0))) return rc;
+        }
+    } else {
+        if ((rc = wait_inputs(h))) return rc;
+        if ((rc = st_gemm_dot(h, BSE_ST_SCREEN, h->u, h->N, h->u, h->N, h->Nv, h->Nv, h->N, true, h->Mmat, h->Nv, 1.0,
+                              nullptr))) return rc;
+    }
+    if ((rc = wait_inputs(h))) return rc;
     { StageTimer t(h, BSE_ST_PAIRLIST, 0.0, 8.0 * h->Nv * (double)h->Nv);
       if ((rc = bse_launch_pairlist(h))) return rc; }
     const unsigned mode = h->flags & BSE_TAU_MASK;
@@ -1065,8 +1100,11 @@ extern "C" int bse_apply_k1x(bse_handle *h, const double *a, double *out, int B)
     if (a == out) { bse_set_error("out must not alias a"); return BSE_EINVAL; }
     int rc;
     if ((h->flags & BSE_TAU_MASK) == BSE_TAU_STREAM) {       // tau rebuilt inside every apply: tau(G) transient, tau(r) streamed
-        if ((rc = ensure_tau_store(h, false))) return rc;
-        if ((rc = fill_tau_store(h, false))) return rc;
+        if (!h->tau_prefilled) {
+            if ((rc = ensure_tau_store(h, false))) return rc;
+            if ((rc = fill_tau_store(h, false))) return rc;
+        }
+        h->tau_prefilled = false;
     }
     if ((rc = plan_apply_memory(h, B))) return rc;
     if (h->flags & BSE_VEC_PW) return apply_pw(h, (const double2 *)a, (double2 *)out, B);
@@ -1115,11 +1153,35 @@ extern "C" int bse_apply_k1x_host(bse_handle *h, const double *a_host, double *o
         BSE_CUDA(cudaStreamSynchronize(h->stream));
         return BSE_OK;
     }
-    BSE_CUDA(cudaMemcpyAsync(h->a_dev, a_host, bytes, cudaMemcpyHostToDevice, h->stream));
-    const int rc = bse_apply_k1x(h, h->a_dev, h->out_dev, B);
-    if (rc) return rc;
-    BSE_CUDA(cudaMemcpyAsync(out_host, h->out_dev, bytes, cudaMemcpyDeviceToHost, h->stream));
+    // one apply over all blocks: a arrives on the copy stream while tau is rebuilt (STREAM), and every row chunk P_c has
+    // finished leaves on the other copy stream while the next one is projected (p_c_rows)
+    if (!h->s_in) {
+        BSE_CUDA(cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
+        BSE_CUDA(cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
+    }
+    if (!h->ev_d2h) BSE_CUDA(cudaEventCreateWithFlags(&h->ev_d2h, cudaEventDisableTiming));
+    BSE_CUDA(cudaEventRecord(h->ev_d2h, h->stream));                         // earlier work on the library's stream first
+    BSE_CUDA(cudaStreamWaitEvent(h->s_in, h->ev_d2h, 0));
+    BSE_CUDA(cudaMemcpyAsync(h->a_dev, a_host, bytes, cudaMemcpyHostToDevice, h->s_in));
+    BSE_CUDA(cudaEventRecord(h->ev_d2h, h->s_in));
+    int rc = BSE_OK;
+    if (h->built && (h->flags & BSE_TAU_MASK) == BSE_TAU_STREAM) {
+        if ((rc = ensure_tau_store(h, false)) == BSE_OK && (rc = fill_tau_store(h, false)) == BSE_OK) h->tau_prefilled = true;
+    }
+    BSE_CUDA(cudaStreamWaitEvent(h->stream, h->ev_d2h, 0));
+    if (rc == BSE_OK) {
+        h->d2h_host = out_host;
+        h->d2h_rows_done = 0;
+        rc = bse_apply_k1x(h, h->a_dev, h->out_dev, B);
+        h->d2h_host = nullptr;
+    }
+    h->tau_prefilled = false;
+    if (rc) { cudaStreamSynchronize(h->s_in); cudaStreamSynchronize(h->s_out); return rc; }
+    const size_t done = (size_t)h->d2h_rows_done * (bytes / ((size_t)B * h->Nv));   // bytes per row: the vector length * 8
+    if (done < bytes)
+        BSE_CUDA(cudaMemcpyAsync((char *)out_host + done, (char *)h->out_dev + done, bytes - done, cudaMemcpyDeviceToHost, h->stream));
     BSE_CUDA(cudaStreamSynchronize(h->stream));
+    BSE_CUDA(cudaStreamSynchronize(h->s_out));
     return BSE_OK;
 }
 
@@ -1128,8 +1190,38 @@ extern "C" int bse_apply_k1x_host(bse_handle *h, const double *a_host, double *o
 extern "C" int bse_set_inputs_host(bse_handle *h, const double *u_host, const double *phi_host) {
     if (!h || (!u_host && !phi_host)) { bse_set_error("null pointer"); return BSE_EINVAL; }
     if (!h->u_owned || !h->phi_owned) { bse_set_error("bse_set_inputs_host needs a handle created with BSE_PTR_HOST"); return BSE_ESTATE; }
-    if (u_host) BSE_CUDA(cudaMemcpyAsync(h->u_owned, u_host, (size_t)h->Nv * h->N * 8, cudaMemcpyHostToDevice, h->stream));
-    if (phi_host) BSE_CUDA(cudaMemcpyAsync(h->phi_owned, phi_host, (size_t)h->Npdep * h->fft.npw_h * 16, cudaMemcpyHostToDevice, h->stream));
+    if (!h->s_in) {
+        BSE_CUDA(cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
+        BSE_CUDA(cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
+    }
+    if (!h->ev_in_done) BSE_CUDA(cudaEventCreateWithFlags(&h->ev_in_done, cudaEventDisableTiming));
+    BSE_CUDA(cudaEventRecord(h->ev_in_done, h->stream));                     // readers of the old arrays first
+    BSE_CUDA(cudaStreamWaitEvent(h->s_in, h->ev_in_done, 0));
+    h->in_chunks = 0;
+    if (u_host) {
+        // column slabs (all orbitals on a range of grid points): the screen of bse_build_tau is a sum over grid points and
+        // starts on slab 0 while the others are on their way.  Small arrays go in one piece.
+        const size_t ub = (size_t)h->Nv * h->N * 8;
+        const int nch = h->dbg_in_chunks >= 1 ? (int)h->dbg_in_chunks : (ub >= ((size_t)256 << 20) ? 8 : 1);
+        const long long kc = nch == 1 ? h->N : ((h->N + nch - 1) / nch + 1023) / 1024 * 1024;
+        const int used = (int)((h->N + kc - 1) / kc);
+        while ((int)h->ev_in.size() < used) {
+            cudaEvent_t e;
+            BSE_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            h->ev_in.push_back(e);
+        }
+        for (int c = 0; c < used; ++c) {
+            const long long k0 = c * kc, kw = std::min<long long>(kc, h->N - k0);
+            BSE_CUDA(cudaMemcpy2DAsync(h->u_owned + k0, (size_t)h->N * 8, u_host + k0, (size_t)h->N * 8, (size_t)kw * 8, h->Nv,
+                                       cudaMemcpyHostToDevice, h->s_in));
+            BSE_CUDA(cudaEventRecord(h->ev_in[c], h->s_in));
+        }
+        h->in_chunks = used;
+        h->in_kc = kc;
+    }
+    if (phi_host) BSE_CUDA(cudaMemcpyAsync(h->phi_owned, phi_host, (size_t)h->Npdep * h->fft.npw_h * 16, cudaMemcpyHostToDevice, h->s_in));
+    BSE_CUDA(cudaEventRecord(h->ev_in_done, h->s_in));
+    h->inputs_pending = true;
     h->built = false;
     if (u_host) { h->uG_valid = false; h->u_a_valid = false; h->u_bl = -1; }     // derived copies are refilled in place, lazily
     return BSE_OK;
@@ -1140,6 +1232,7 @@ extern "C" int bse_apply_k1e(bse_handle *h, const double *a, double *out, int B)
     if (!h || !a || !out || B <= 0) { bse_set_error("null pointer or B <= 0"); return BSE_EINVAL; }
     if (a == out) { bse_set_error("out must not alias a"); return BSE_EINVAL; }
     int rc;
+    if ((rc = wait_inputs(h))) return rc;
     const long long Nv = h->Nv;
     if (!(h->flags & BSE_VEC_PW)) {
         const FftPlan &pl = h->fft;
@@ -1207,6 +1300,7 @@ extern "C" int bse_k1e_hartree_partial(bse_handle *h, const double *a_rows, int 
     const long long npw_h = pl.npw_h, nloc = v1 - v0;
     const double N8 = 8.0 * (double)pl.N;
     int rc;
+    if ((rc = wait_inputs(h))) return rc;
     if ((rc = ensure_u_pw(h))) return rc;
     if ((rc = ensure_u_apply(h))) return rc;
     const double *ua = h->u_a ? h->u_a : h->u;
@@ -1235,6 +1329,7 @@ extern "C" int bse_k1e_from_hartree(bse_handle *h, const double *vG, int v0, int
     const long long npw_h = pl.npw_h, nloc = v1 - v0;
     const double N8 = 8.0 * (double)pl.N;
     int rc;
+    if ((rc = wait_inputs(h))) return rc;
     if ((rc = ensure_u_pw(h))) return rc;
     if ((rc = ensure_u_apply(h))) return rc;
     const double *ua = h->u_a ? h->u_a : h->u;
@@ -1432,6 +1527,8 @@ extern "C" int bse_debug_set(bse_handle *h, const char *key, long long value) {
     else if (k == "slab_rows") { h->dbg_slab_rows = value; h->plan_ok = false; }
     else if (k == "gemm_bm") { bse_gemm_set_bm((int)value); }       // process-wide: CTA tile height of the DMMA GEMMs
     else if (k == "slab_planes") { h->dbg_slab_planes = value; h->plan_ok = false; }
+    else if (k == "pc_rows") { h->dbg_pc_rows = value; }
+    else if (k == "in_chunks") { h->dbg_in_chunks = value; }
     else { bse_set_error("bse_debug_set: unknown key " + k); return BSE_EINVAL; }
     return BSE_OK;
 }

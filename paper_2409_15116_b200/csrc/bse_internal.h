@@ -97,6 +97,8 @@ struct bse_handle {
     std::vector<int> plan_adj_h, plan_adj_ptr_h;   // the adjacency the row batches were planned for (exact comparison)
     // debug / test knobs (bse_debug_set; never read from the environment): caps that only ever lower a limit
     long long dbg_max_group = 0, dbg_max_batch = 0;   // 0 = no cap; either one set keeps the apply on the group / row-batch path
+    long long dbg_in_chunks = 0;                      // column slabs bse_set_inputs_host copies u in (0 = automatic)
+    long long dbg_pc_rows = 0;                        // cap of the rows per chunk of P_c (0 = no cap)
     long long dbg_slab_planes = 0;                    // cap of the planes per slab (0 = no cap)
     long long dbg_slab_rows = 0;                      // cap of the rows per chunk of the plane-slab apply; -1 = never use it
     // plane-slab streaming of the PW-layout apply: a_r = [B][Nv][SN], tau_batch = [P][SN],
@@ -128,6 +130,18 @@ struct bse_handle {
     size_t a_dev_bytes = 0;
     cudaStream_t s_in = nullptr, s_out = nullptr;  // copy streams of the pipelined host-pointer apply
     std::vector<cudaEvent_t> ev_pipe;
+    // host-pointer apply, non-pipelined form: the copy of a overlaps the tau rebuild (STREAM), finished row chunks of P_c
+    // leave for the host while the next chunk is projected
+    bool tau_prefilled = false;                    // bse_apply_k1x_host has rebuilt tau for the apply that follows
+    double *d2h_host = nullptr;                    // host image of out_dev (non-null only inside bse_apply_k1x_host)
+    long long d2h_rows_done = 0;                   // leading rows of out_dev already on their way to d2h_host
+    cudaEvent_t ev_d2h = nullptr;
+    // bse_set_inputs_host copies on s_in, u in column slabs: bse_build_tau screens slab c as soon as it has arrived
+    bool inputs_pending = false;                   // a copy is in flight that the library's stream has not yet waited for
+    int in_chunks = 0;                             // column slabs of the last copy of u (0: u was not copied)
+    long long in_kc = 0;                           // grid points per slab
+    std::vector<cudaEvent_t> ev_in;                // [c] slab c of u is on the device
+    cudaEvent_t ev_in_done = nullptr;              // everything bse_set_inputs_host enqueued is on the device
     // profiling
     bool prof = false;
     double st_ms[BSE_ST_COUNT] = {0};

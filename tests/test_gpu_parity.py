@@ -699,3 +699,40 @@ def test_single_precision_tau_store(tau):
     with pytest.raises(bse.BseError) as e:
         bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, u, w.phi.shape[0], phi, w.lam, w.eta, bse.BSE_TAU_REAL | bse.BSE_TAU_F32)
     assert e.value.code == bse.BSE_EINVAL
+
+
+@pytest.mark.parametrize("tau", ["stream", "pw"])
+def test_host_pointer_apply_with_overlapped_copies(tau):
+    """bse_apply_k1x_host in the non-pipelined form: a is copied in while tau is rebuilt (STREAM), and P_c's row chunks
+    (capped at 64 rows here: 3 chunks, the last one ragged) leave for the host one by one.  Same result as the device call."""
+    bse = _bse()
+    cfg = wl.Config("h2", 10.0, 24, 40, 20, 8.0, 1.2, 0.8, 3.0, 0.05, 4, "random", seed=93)
+    w = wl.make(cfg=cfg)
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    phi = np.ascontiguousarray(w.phi).view(np.float64)
+    flag = {"stream": bse.BSE_TAU_STREAM, "pw": bse.BSE_TAU_PW}[tau]
+    h = bse.bse_create([w.n] * 3, w.cell, w.ecut, w.Nv, np.ascontiguousarray(w.u), w.phi.shape[0], phi, w.lam, w.eta,
+                       bse.BSE_PTR_HOST | flag | bse.BSE_VEC_PW)
+    try:
+        bse.bse_debug_set(h, "pc_rows", 64)
+        bse.bse_debug_set(h, "in_chunks", 8)                     # u arrives in 7 column slabs (the last one ragged): the screen
+        u_pin = torch.from_numpy(np.ascontiguousarray(w.u)).pin_memory()         # accumulates slab after slab behind the copy
+        phi_pin = torch.from_numpy(phi).pin_memory()
+        bse.bse_set_inputs_host(h, u_pin, phi_pin)
+        bse.bse_build_tau(h)
+        pairs = bse.bse_get_pairs(h)
+        assert np.array_equal(pairs, orc.screen_pairs(w.u, w.eta)[0])
+        a = torch.from_numpy(np.ascontiguousarray(w.a_pw).view(np.float64)).pin_memory()
+        out = torch.full(a.shape, float("nan"), dtype=torch.float64).pin_memory()
+        for _ in range(2):                                       # the second call reuses streams, events and staging
+            out.fill_(float("nan"))
+            bse.bse_apply_k1x_host(h, a, out, w.a_pw.shape[0])
+            tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs, want="r")
+            ref = orc.apply_k1x_pw(tab, w.u, pairs, tau_ref, w.a_pw)
+            got = out.numpy().view(np.complex128).reshape(ref.shape)
+            wt = np.full(tab.npw_h, 2.0)
+            wt[0] = 1.0
+            err = np.sqrt((wt * np.abs(got - ref) ** 2).sum() / (wt * np.abs(ref) ** 2).sum())
+            assert err <= TOL, err
+    finally:
+        bse.bse_destroy(h)
