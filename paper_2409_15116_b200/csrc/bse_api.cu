@@ -34,8 +34,12 @@ int upload(T *&dst, const std::vector<T> &src) {
     return BSE_OK;
 }
 
+// the accumulate launchers handle the trial blocks 8, 4, 2 or 1 at a time
+static int acc_launches(int nb) { return nb / 8 + ((nb & 4) ? 1 : 0) + ((nb & 2) ? 1 : 0) + (nb & 1); }
+
 struct StageTimer {
     bse_handle *h; int st;
+    int launches = 1;                              // kernels the stage call launches (set by the caller when not one)
     // bytes: algorithmic HBM bytes by SURVEY 8(d) (fields, coefficients on H, GEMM operands); handoff: bytes of the stick-plane
     // intermediate Z, which exists only because the 3-D transform is split into two kernels (implementation traffic)
     StageTimer(bse_handle *h_, int st_, double flops, double bytes, double handoff = 0.0) : h(h_), st(st_) {
@@ -45,7 +49,7 @@ struct StageTimer {
         if (h->prof) cudaEventRecord(h->ev0, h->stream);
     }
     ~StageTimer() {
-        h->st_launch[st] += 1;
+        h->st_launch[st] += launches;
         if (h->prof) {
             cudaEventRecord(h->ev1, h->stream);
             cudaEventSynchronize(h->ev1);
@@ -211,6 +215,7 @@ int st_accumulate(bse_handle *h, const double *tau, long long p0, long long cnt,
     const double directed = (double)h->nadj * (double)cnt / (double)std::max<long long>(h->P, 1);
     StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)h->N * directed,
                  m.N8 * ((double)cnt + (first ? 2.0 * nb * h->Nv : 0.0)));
+    t.launches = acc_launches(nb);
     return bse_launch_accumulate(h, tau, p0, cnt, a, acc, nb, first);
 }
 
@@ -758,6 +763,7 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
         }
         { StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)pl.N * (double)h->nadj * rows / h->Nv,
                        m.N8 * (uniq * bt.nu + nb * rows + (r0 == 0 ? (double)nb * h->Nv : 0.0)));
+          t.launches = acc_launches(nb);
           if (acc_real) rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, h->rowlist + r0, rows, a, acc_real, h->Nv, false, nb);
           else rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, h->rowlist + r0, rows, a, h->acc_r, h->rows_cap, true, nb);
           if (rc) return rc; }
@@ -836,6 +842,7 @@ int apply_pw_slab(bse_handle *h, const double2 *a, double2 *out, int B) {
             const double directed = (double)(h->adj_ptr_h[v0 + rows] - h->adj_ptr_h[v0]);
             { StageTimer t(h, BSE_ST_ACCUM, 2.0 * B * (double)SN * directed,
                            8.0 * SN * ((double)h->Pa * rows / nloc + (double)B * rows + (v0 == h->row0 ? (double)B * Nv : 0.0)));
+              t.launches = acc_launches(B);
               if ((rc = bse_launch_accumulate_rows(h, SN, h->tau_batch, h->eslot_act, h->rowid + v0, rows, h->a_r, h->acc_r, rows,
                                                    true, B))) return rc; }
             if (h->mix_on) {
