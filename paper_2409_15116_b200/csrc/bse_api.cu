@@ -390,7 +390,8 @@ int alloc_batch_ws(bse_handle *h, long long pb) {
         bse_set_error("out of device memory (pair-batch workspaces)");
         return BSE_ENOMEM;
     }
-    h->Pb = pb;
+    h->Pb_alloc = pb;
+    h->Pb = pb >= 64 ? pb / 64 * 64 : pb;          // whole 64-row CTA tiles in the PDEP GEMMs (297 pairs cost as much as 320)
     return BSE_OK;
 }
 
@@ -561,7 +562,7 @@ int plan_apply_memory(bse_handle *h, int B, bool allow_slab = true, bool mix = f
             SN8 = 8.0 * (double)M * pl.n * pl.n;
             // a(r) of all blocks + tau(r) of all (owned) pairs; the combined call also keeps u and v_H of the slab (k1e_ws)
             const double fixed = ((double)B * h->Nv + (double)h->Pa + (mix ? (double)h->Nv + 2.0 * B : 0.0)) * SN8;
-            pz = (long long)(((double)h->Pb * h->n * h->fft.NS) / ((double)M * pl.NS));
+            pz = (long long)(((double)h->Pb_alloc * h->n * h->fft.NS) / ((double)M * pl.NS));
             rc = (long long)((avail_s - fixed) / ((double)B * SN8));
             rc = std::min<long long>(rc, std::min<long long>(pz / B, 65535 / B));
             rc = std::min<long long>(rc, std::min<long long>(h->Nv, 256));

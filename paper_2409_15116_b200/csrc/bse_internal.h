@@ -79,8 +79,9 @@ struct bse_handle {
     float2 *tau_g32 = nullptr;       // [P][npw_h] single-precision store (BSE_TAU_F32) instead of tau_g
     size_t tau_bytes = 0;            // capacity of the store (grow-only)
     // workspaces (sized for a pair batch)
-    long long Pb = 0;                // pair-batch capacity
-    double2 *Z = nullptr;            // [Pb][n][NS]
+    long long Pb = 0;                // pairs per batch (Pb_alloc rounded down to whole 64-row GEMM tiles)
+    long long Pb_alloc = 0;          // fields the batch workspaces hold
+    double2 *Z = nullptr;            // [Pb_alloc][n][NS]
     double2 *X = nullptr;            // [Pb][npw_h]
     double2 *T = nullptr;            // [Pb][npw_h]
     double *Dm = nullptr;            // [Pb][Npdep]

@@ -245,9 +245,14 @@ int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb,
         for (int i = 0; i < tm; ++i)
             for (int j = 0; j < tn; ++j) tiles += ((long long)(j + 1) * BN > (long long)i * BM) ? 1 : 0;
     }
-    // split K so that the CTAs come in whole waves of 148 (one per SM) and there are at least two per SM: the DMMA pipe
-    // saturates at ~8 warps per SM, while a few CTAs over a multiple of 148 leave most SMs idle for a whole CTA time
-    // (304 CTAs ran 1.5x longer than 288).  More, shorter CTAs only add prologue and partial-sum traffic.
+    // split K so that the CTAs fill the machine in whole waves.  A CTA of 64 rows (4 warps, 60 KB of shared memory) is
+    // resident 3 to an SM, so a wave is 444 CTAs and costs 3 units (one unit = one CTA on an SM whose DMMA pipe is saturated,
+    // which takes ~8 warps); the last, partial wave puts c = ceil(r / 148) CTAs on an SM and costs c units, or ~1.7 when
+    // c = 1 (4 warps do not saturate the pipe).  Measured: 304 CTAs ran 1.5x longer than 288; cfg 4's projection at 576 CTAs
+    // (one wave + 132) reached 0.69 of the DMMA peak, at 288 (two per SM) 0.86.  The SYRK squares its operands on the way to
+    // the fragments and needs all three resident CTAs to hide that: two per SM ran at 0.44 against 0.66 with three, so there a
+    // partial wave costs as much as a full one.  More, shorter CTAs only add prologue and partial-sum traffic, so a larger
+    // split must win by 2 %.
     const long long sms = 148;
     long long smax = ksteps / 8;
     const long long cap = (long long)(part_bytes / ((size_t)M * N * 8));
@@ -256,13 +261,18 @@ int bse_gemm_dot(const double *A, long long lda, const double *B, long long ldb,
     if (smax < 1) smax = 1;
     long long splits = 1;
     double best = -1.0;
-    const long long per_sm = BM == 128 ? 1 : 2;                 // CTAs of 8 warps count double
+    const long long res = BM == 128 ? 2 : 3;                    // resident CTAs per SM
     for (long long sp = 1; sp <= smax; ++sp) {
         const long long ctas = tiles * sp;
-        double eff = (double)ctas / (double)(((ctas + sms - 1) / sms) * sms);
-        if (ctas < per_sm * sms) eff *= (double)ctas / (double)(per_sm * sms);          // under two per SM: scaled down
+        const long long full = ctas / (res * sms), r = ctas % (res * sms);
+        double t = (double)(full * res);
+        if (r) {
+            const long long c = (r + sms - 1) / sms;
+            t += (squareA && squareB) ? (double)res : (c == 1 && BM == 64) ? 1.7 : (double)c;
+        }
+        const double eff = ((double)ctas / (double)sms) / t;
         if (eff > best + 0.02) { best = eff; splits = sp; }
-        if (ctas >= 4 * per_sm * sms) break;
+        if (ctas >= 5 * res * sms) break;
     }
     long long kchunk = ((ksteps + splits - 1) / splits) * BK;
     splits = (K + kchunk - 1) / kchunk;
