@@ -257,7 +257,8 @@ int p_c_rows(bse_handle *h, double *x, long long rows, long long K, const double
     if ((rc = ensure_sov(h, rows))) return rc;
     long long mc = rows;
     const long long per_row = (long long)h->Nv * 8 * 2;
-    if (rows * per_row > (long long)h->part_bytes) mc = std::max<long long>(64, (long long)(h->part_bytes / per_row) / 64 * 64);
+    const long long chunk_bytes = (long long)std::min<size_t>(h->part_bytes, (size_t)64 << 20);
+    if (rows * per_row > chunk_bytes) mc = std::max<long long>(64, (chunk_bytes / per_row) / 64 * 64);
     if (h->dbg_pc_rows >= 1) mc = std::min(mc, h->dbg_pc_rows);
     for (long long r0 = 0; r0 < rows; r0 += mc) {
         const int m = (int)std::min(mc, rows - r0);
@@ -1002,7 +1003,7 @@ extern "C" int bse_create(bse_handle **hout, const int grid[3], const double cel
     size_t budget = std::min<size_t>((size_t)12 << 30, free_b / 4);
     long long Pb = (long long)(budget / (per_pair + per_pair_r));
     Pb = std::max<long long>(1, std::min<long long>(Pb, 512));
-    h->part_bytes = std::max<size_t>((size_t)64 << 20, nv2 * 8 * 2);
+    h->part_bytes = std::max<size_t>((size_t)128 << 20, nv2 * 8 * 2);    // split-K partial sums: room for 13 splits of the screen at N_v = 1024
     if ((rc = alloc_batch_ws(h, Pb))) return fail(rc);
     if (cudaMalloc(&h->part, h->part_bytes)) {
         bse_set_error("out of device memory (workspaces)");
