@@ -162,6 +162,27 @@ int bse_get_overlap(const bse_handle *h, double *O /* HOST [Nv][Nv], eq. 16 */);
  * BSE_TAU_PW ([count][Npw_h] complex).  Works in every storage mode (recomputes if needed). */
 int bse_get_tau(bse_handle *h, long long first, long long count, double *dst, unsigned layout);
 
+/* ---- allocation-free screen (a1, eq. 16) ----
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ *   M[v][w] = sum_r u_v(r)^2 u_w(r)^2   for v <= w   (the matrix whose normalised form bse_get_overlap returns and
+ *   bse_build_tau thresholds against eta), by the same split-K FP64 tensor-core SYRK + reduction as bse_build_tau.
+ * It needs no handle and calls no cudaMalloc / cudaFree / allocating library routine: the split-K partial sums go to a
+ * fixed array of BSE_SCREEN_STATIC_BYTES (8 MiB) that is part of the library image, so EVERY GPU that loads the library
+ * holds those 8 MiB until the process exits, and Nv is limited to BSE_SCREEN_STATIC_MAX_NV = 1024 (8 Nv^2 bytes must fit;
+ * the split-K factor is at most floor(8 MiB / (8 Nv^2)), so near the limit the call is correct but slower than the
+ * handle's path).  Larger Nv: BSE_EINVAL with a message naming the limit.
+ *   u      DEVICE [Nv][N] doubles, 16-byte aligned, N even (BSE_EINVAL otherwise); read only
+ *   M      DEVICE [Nv][Nv] doubles, written; entries with v <= w are defined (raw sums, no dV, not normalised), entries
+ *          below the diagonal are unspecified (zero, or the symmetric value inside a diagonal 64 x 64 tile)
+ *   stream the CUDA stream (cudaStream_t) everything is enqueued on; the call does not synchronise
+ * The array is shared by every call of the process on that GPU and keeps the last call's contents: each call clears it first
+ * (on `stream`), so calls on the same stream are safe back to back, while calls that overlap on the GPU (different streams,
+ * or several host threads) RACE on it: serialise them.  The first call on a device resolves the array's device address
+ * (cudaGetSymbolAddress, once per device, with that device current): make that call outside stream capture. */
+#define BSE_SCREEN_STATIC_BYTES  (8u << 20)
+#define BSE_SCREEN_STATIC_MAX_NV 1024
+int bse_screen_overlap_static(const double *u, int Nv, long long N, double *M, void *stream);
+
 /* ---- measurement helpers ---- */
 /* Debug / test knobs of one handle (nothing is read from the environment).  They only lower a limit or choose between
  * equivalent kernels, never change a result:  "max_group" caps the number of trial blocks processed together in the PW

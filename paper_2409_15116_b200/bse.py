@@ -55,6 +55,7 @@ _sig = {
     "bse_profile_model": [_vp, C.POINTER(_d), C.POINTER(_d)],
     "bse_profile_handoff": [_vp, C.POINTER(_d)],
     "bse_probe_fp64_peak": [C.POINTER(_d), C.POINTER(_d), _vp],
+    "bse_screen_overlap_static": [_vp, _i, _ll, _vp, _vp],
 }
 for _name, _args in _sig.items():
     getattr(lib, _name).argtypes = _args
@@ -169,6 +170,14 @@ def bse_get_overlap(h, Nv):
     o = np.empty((Nv, Nv), dtype=np.float64)
     _check(lib.bse_get_overlap(h, o.ctypes.data), "bse_get_overlap")
     return o
+
+
+BSE_SCREEN_STATIC_BYTES, BSE_SCREEN_STATIC_MAX_NV = 8 << 20, 1024
+
+
+def bse_screen_overlap_static(u, Nv, N, M, stream=None):
+    """Allocation-free screen (include/bse.h): u DEVICE [Nv][N], M DEVICE [Nv][Nv] (v <= w defined); enqueued on `stream`."""
+    _check(lib.bse_screen_overlap_static(_ptr(u), int(Nv), int(N), _ptr(M), _ptr(stream)), "bse_screen_overlap_static")
 
 
 def bse_get_tau(h, first, count, dst, layout=BSE_TAU_REAL):

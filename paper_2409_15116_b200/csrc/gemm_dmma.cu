@@ -310,3 +310,58 @@ int bse_gemm_nn(const double *A, long long lda, const double *B, long long ldb, 
     bse_set_error("bse_gemm_nn: bad epilogue");
     return BSE_EINVAL;
 }
+
+// ---------------------------------------------------------------------------------------------------------
+// Allocation-free screen (include/bse.h: bse_screen_overlap_static).  The split-K partial sums of the SYRK above normally
+// live in the handle's cudaMalloc'ed workspace; callers that may not allocate (CUDA graph capture, serving loops) get the
+// same kernels with the partial sums in a fixed array that is part of the library image: every GPU that loads the library
+// holds these 8 MiB until the process exits.  In HOST code the name g_screen_scratch is only a stand-in of the symbol, not a
+// device address: the address comes from cudaGetSymbolAddress, once per device, with that device current.
+#include <mutex>
+
+constexpr size_t SCREEN_SCRATCH_BYTES = (size_t)BSE_SCREEN_STATIC_BYTES;
+static __device__ __align__(256) double g_screen_scratch[SCREEN_SCRATCH_BYTES / 8];
+
+namespace {
+constexpr int MAX_DEVICES = 64;
+double *g_screen_scratch_addr[MAX_DEVICES] = {nullptr};         // device address of g_screen_scratch on device d
+std::mutex g_screen_scratch_mutex;
+
+int screen_scratch_address(double **out) {
+    int dev = -1;
+    BSE_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) { bse_set_error("bse_screen_overlap_static: device ordinal out of range"); return BSE_EUNSUPPORTED; }
+    std::lock_guard<std::mutex> lock(g_screen_scratch_mutex);
+    if (!g_screen_scratch_addr[dev]) {
+        double *p = nullptr;
+        BSE_CUDA(cudaGetSymbolAddress((void **)&p, g_screen_scratch));
+        if (!p) { bse_set_error("bse_screen_overlap_static: cudaGetSymbolAddress returned a null address"); return BSE_ECUDA; }
+        g_screen_scratch_addr[dev] = p;
+    }
+    *out = g_screen_scratch_addr[dev];
+    return BSE_OK;
+}
+}  // namespace
+
+extern "C" int bse_screen_overlap_static(const double *u, int Nv, long long N, double *M, void *stream) {
+    if (!u || !M || Nv <= 0 || N <= 0) { bse_set_error("bse_screen_overlap_static: null pointer or empty size"); return BSE_EINVAL; }
+    if ((N & 1) || ((uintptr_t)u & 15)) {
+        bse_set_error("bse_screen_overlap_static: N must be even and u 16-byte aligned (16-byte operand loads)");
+        return BSE_EINVAL;
+    }
+    const size_t need = (size_t)Nv * (size_t)Nv * 8;              // one set of partial sums (split-K factor 1)
+    if (need > SCREEN_SCRATCH_BYTES) {
+        bse_set_error("bse_screen_overlap_static: Nv = " + std::to_string(Nv) + " needs " + std::to_string(need) +
+                      " bytes of split-K scratch, the static array holds " + std::to_string(SCREEN_SCRATCH_BYTES) +
+                      " (Nv <= " + std::to_string(BSE_SCREEN_STATIC_MAX_NV) + ")");
+        return BSE_EINVAL;
+    }
+    double *part = nullptr;
+    int rc;
+    if ((rc = screen_scratch_address(&part))) return rc;
+    cudaStream_t s = (cudaStream_t)stream;
+    // the array keeps the previous call's partial sums, and the SYRK writes only the tiles that touch v <= w: clear it, so that
+    // the tiles below the diagonal reduce to zero instead of to whatever an earlier call left there
+    BSE_CUDA(cudaMemsetAsync(part, 0, SCREEN_SCRATCH_BYTES, s));
+    return bse_gemm_dot(u, N, u, N, Nv, Nv, N, true, true, part, SCREEN_SCRATCH_BYTES, M, Nv, 1.0, nullptr, s, false);
+}
