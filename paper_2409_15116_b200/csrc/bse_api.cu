@@ -1533,6 +1533,8 @@ extern "C" int bse_debug_set(bse_handle *h, const char *key, long long value) {
     if (k == "max_group") { h->dbg_max_group = value; h->plan_ok = false; }
     else if (k == "max_batch") { h->dbg_max_batch = value; h->plan_ok = false; }
     else if (k == "compact_inv") { h->fft.compact_inv = h->ffta.compact_inv = (int)value; }
+    else if (k == "pipe") { h->fft.pipe = h->ffta.pipe = (int)value; }
+    else if (k == "pipe_lc") { h->fft.pipe_lc = h->ffta.pipe_lc = (int)value; }
     else if (k == "slab_rows") { h->dbg_slab_rows = value; h->plan_ok = false; }
     else if (k == "gemm_bm") { bse_gemm_set_bm((int)value); }       // process-wide: CTA tile height of the DMMA GEMMs
     else if (k == "slab_planes") { h->dbg_slab_planes = value; h->plan_ok = false; }

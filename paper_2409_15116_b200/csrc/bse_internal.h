@@ -20,6 +20,8 @@ struct FftPlan {
     long long npw_h = 0;
     const void *ops = nullptr;    // bsefft::FftOps of this n
     int compact_inv = -1;         // inverse plane kernel: -1 automatic, 0 never compact, k > 1 compact sized for k CTAs / SM
+    int pipe = -1;                // plane passes: -1 automatic, 0 one-plane-per-CTA kernels, 1 pipelined kernels (fft_pipe.cuh)
+    int pipe_lc = 0;              // > 0: cap on the lines per slab of the pipelined kernels (test knob)
     // device tables
     double2 *tw = nullptr;        // [n]   exp(-2 pi i t / n)
     int *soff = nullptr;          // [n]   stick index of (t2 = m2 mod n, m3) is soff[t2] + m3

@@ -39,6 +39,7 @@ static PlanDev to_dev(const FftPlan &pl, int np = 0) {
     PlanDev d;
     d.R = pl.R; d.W = pl.W; d.NS = pl.NS;
     d.np = np > 0 ? np : pl.n;
+    d.pipe = pl.pipe; d.pipe_lc = pl.pipe_lc;
     d.tw = pl.tw; d.soff = pl.soff; d.wmax = pl.wmax; d.wmin = pl.wmin; d.hmapT = pl.hmapT;
     return d;
 }

@@ -35,6 +35,8 @@ struct PlanDev {
     const int *wmax;        // [n] largest m3 of a stick at t2 = m2 mod n, -1 if none
     const int *wmin;        // [n] smallest m3 stored (1 for m2 < 0: the (m2<0, m3=0) sticks are mirrors)
     const int *hmapT;       // [n][NS] (t1 = m1 mod n, stick) -> h in H, -1 outside the sphere, -2-h: conj of entry h
+    int pipe;               // plane passes: -1 automatic, 0 the one-plane-per-CTA kernels, 1 the pipelined kernels (fft_pipe.cuh)
+    int pipe_lc;            // > 0: at most this many packed lines per slab of the pipelined kernels (test knob)
 };
 
 // coefficient h of a field kept in double (t) or, when t32 != nullptr, in single precision
@@ -503,6 +505,10 @@ inv_stick_kernel(PlanDev P, const double2 *__restrict__ T, long long npw_h, doub
 }
 
 
+}  // namespace bsefft
+#include "fft_pipe.cuh"
+namespace bsefft {
+
 // ---------------------------------------------------------------------------------------------------------
 // host launchers for one factorisation; collected in a table by fft_kernels.cu
 struct FftOps {
@@ -528,8 +534,68 @@ struct Launch {
             BSE_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         return BSE_OK;
     }
+    // ---- pipelined plane passes (fft_pipe.cuh) ----
+    using PG = PipeGeo<R1, R2>;
+    static constexpr int SMEM_MAX = 232448;                     // opt-in limit of one CTA on sm_100
+    // automatic choice: planes so large that at most two one-plane CTAs fit an SM (n >= 100), where the load, butterfly and
+    // store phases of the one-plane kernels do not overlap
+    static bool use_pipe(const PlanDev &P) { return P.pipe > 0 || (P.pipe < 0 && G::smem_ctas <= 2); }
+    // lines per slab: as many as fit beside the fixed buffers, at most one rows-pass task per thread, slabs of equal size
+    static int pick_lc(int fixed, int per_line, int knob) {
+        int lc = (SMEM_MAX - fixed) / per_line;
+        const int cap = (PIPE_THREADS + R2 - 1) / R2;
+        if (lc > cap) lc = cap;
+        if (lc > G::n / 2) lc = G::n / 2;
+        if (lc < 2) return 0;
+        const int ns = (G::n / 2 + lc - 1) / lc;
+        lc = (G::n / 2 + ns - 1) / ns;
+        if (knob > 0 && lc > knob) lc = knob;
+        return lc;
+    }
+    static int persistent_grid(const void *kern, int smem, long long total, int *grid) {
+        int dev = 0, sms = 0, occ = 0;
+        BSE_CUDA(cudaGetDevice(&dev));
+        BSE_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        BSE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        BSE_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        BSE_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, PIPE_THREADS, smem));
+        if (occ < 1) return BSE_EUNSUPPORTED;
+        const long long g = (long long)occ * sms;
+        *grid = (int)(total < g ? total : g);
+        return BSE_OK;
+    }
+    static int inv_plane_pipe(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s) {
+        const int LC = pick_lc(PG::inv_smem(P.W, P.NS, 0), G::LD * 16 + 2 * G::n * 8, P.pipe_lc);
+        if (LC < 2) return BSE_EUNSUPPORTED;
+        const int smem = PG::inv_smem(P.W, P.NS, LC);
+        const long long total = (long long)count * P.np;
+        int grid = 0;
+        const int rc = persistent_grid((const void *)inv_plane_pipe_kernel<R1, R2>, smem, total, &grid);
+        if (rc) return rc;
+        inv_plane_pipe_kernel<R1, R2><<<grid, PIPE_THREADS, smem, s>>>(P, Z, N, out, total, LC);
+        BSE_CUDA(cudaGetLastError());
+        return BSE_OK;
+    }
+    static int fwd_plane_pipe(const PlanDev &P, const double *fields, const int2 *pairs, long long p0, int count, long long N,
+                              double2 *Z, cudaStream_t s) {
+        const int nf = pairs ? 2 : 1, NST = 2;
+        const int LC = pick_lc(PG::fwd_smem(P.W, 0, NST, nf), G::LD * 16 + NST * nf * 2 * G::n * 8, P.pipe_lc);
+        if (LC < 2) return BSE_EUNSUPPORTED;
+        const int smem = PG::fwd_smem(P.W, LC, NST, nf);
+        const long long total = (long long)count * P.np;
+        int grid = 0;
+        const int rc = persistent_grid((const void *)fwd_plane_pipe_kernel<R1, R2>, smem, total, &grid);
+        if (rc) return rc;
+        fwd_plane_pipe_kernel<R1, R2><<<grid, PIPE_THREADS, smem, s>>>(P, fields, pairs, p0, N, Z, total, LC, NST);
+        BSE_CUDA(cudaGetLastError());
+        return BSE_OK;
+    }
     static int fwd_plane(const PlanDev &P, const double *fields, const int2 *pairs, long long p0, int count, long long N,
                          double2 *Z, cudaStream_t s) {
+        if (use_pipe(P)) {
+            int rc = fwd_plane_pipe(P, fields, pairs, p0, count, N, Z, s);
+            if (rc != BSE_EUNSUPPORTED) return rc;
+        }
         int rc = set_smem((const void *)fwd_plane_kernel<R1, R2>, G::plane_smem, true);
         if (rc) return rc;
         const int threads = G::plane_thr;
@@ -543,6 +609,10 @@ struct Launch {
     }
     static int inv_plane(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s, int sub,
                          int force) {
+        if (!sub && force < 0 && use_pipe(P)) {
+            int rc = inv_plane_pipe(P, Z, count, N, out, s);
+            if (rc != BSE_EUNSUPPORTED) return rc;
+        }
         // large planes (one full-plane CTA per SM): the compact form, if two of its CTAs fit an SM
         // force = k (test / tuning knob of the plan, bse_debug_set): the compact form sized for k CTAs per SM (0: never, -1: auto)
         const int tables = G::n * 16 + 3 * G::n * 4;

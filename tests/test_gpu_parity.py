@@ -522,6 +522,29 @@ def test_every_supported_grid_edge(n):
     _check_pw(w, bse.BSE_TAU_PW)
 
 
+@pytest.mark.parametrize("n", [12, 16, 20, 24, 30, 32, 36, 40, 48, 60, 64, 72, 80, 96, 100, 108, 120, 128, 144, 160])
+def test_pipelined_plane_passes_every_grid_edge(n):
+    """The pipelined plane passes (fft_pipe.cuh: persistent CTAs, cp.async.bulk staging on mbarriers, compact columns; the
+    default only from n = 100 on) forced on every supported grid edge: pair densities + inverse pass in the REAL layout,
+    single-field forward / slab inverse in the PW layout, with the slab height the launcher picks and with 3 lines per
+    slab (several slabs, the last one ragged where 3 does not divide n / 2)."""
+    bse = _bse()
+    R = max(2, min(n // 5, 12))
+    L = 10.0
+    ecut = 0.5 * (2.0 * np.pi / L) ** 2 * (R * R + 0.5)
+    cfg = wl.Config(f"p{n}", L, n, 3, 5, ecut, 1.6, 0.8, 3.0, 0.0, 2, "random", seed=700 + n)
+    w = wl.make(cfg=cfg)
+    tab = orc.Tables(w.n, w.L, w.ecut)
+    pairs_ref, _ = orc.screen_pairs(w.u, w.eta)
+    tau_ref = orc.build_tau(tab, w.u, w.phi, w.lam, pairs_ref, want="r")
+    o1 = _check_full(w, check_g=True, knobs={"pipe": 1}, tau_ref=tau_ref)
+    o2 = _check_full(w, check_g=False, knobs={"pipe": 1, "pipe_lc": 3}, tau_ref=tau_ref)
+    o0 = _check_full(w, check_g=False, knobs={"pipe": 0}, tau_ref=tau_ref)
+    assert rel(o1, o0) < 1e-12 and rel(o2, o0) < 1e-12
+    _check_pw(w, bse.BSE_TAU_PW, {"pipe": 1})
+    _check_pw(w, bse.BSE_TAU_STREAM, {"pipe": 1, "pipe_lc": 3, "slab_planes": 2})
+
+
 def test_compact_inverse_kernel_subtract_epilogue():
     """the SUB epilogue of the compact inverse plane kernel (P_c update of the REAL layout, taken from N_v >= 48
     with band-limited orbitals) forced on a small grid."""
