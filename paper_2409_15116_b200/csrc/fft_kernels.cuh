@@ -537,9 +537,12 @@ struct Launch {
     // ---- pipelined plane passes (fft_pipe.cuh) ----
     using PG = PipeGeo<R1, R2>;
     static constexpr int SMEM_MAX = 232448;                     // opt-in limit of one CTA on sm_100
-    // automatic choice: planes so large that at most two one-plane CTAs fit an SM (n >= 100), where the load, butterfly and
-    // store phases of the one-plane kernels do not overlap
-    static bool use_pipe(const PlanDev &P) { return P.pipe > 0 || (P.pipe < 0 && G::smem_ctas <= 2); }
+    // automatic choice (measured): where one full plane fills the SM (n >= 120), the inverse pass
+    // (cfg 5: 230 -> 210 ms) and the single-field forward pass (-11 %); the pair-density forward pass stages two fields, which
+    // leaves it 9 lines per slab at n = 160 (slower), and on smaller planes the one-plane kernels run more warps per SM
+    static bool use_pipe(const PlanDev &P, bool inverse, bool pair) {
+        return P.pipe > 0 || (P.pipe < 0 && G::smem_ctas == 1 && (inverse || !pair));
+    }
     // lines per slab: as many as fit beside the fixed buffers, at most one rows-pass task per thread, slabs of equal size
     static int pick_lc(int fixed, int per_line, int knob) {
         int lc = (SMEM_MAX - fixed) / per_line;
@@ -592,7 +595,7 @@ struct Launch {
     }
     static int fwd_plane(const PlanDev &P, const double *fields, const int2 *pairs, long long p0, int count, long long N,
                          double2 *Z, cudaStream_t s) {
-        if (use_pipe(P)) {
+        if (use_pipe(P, false, pairs != nullptr)) {
             int rc = fwd_plane_pipe(P, fields, pairs, p0, count, N, Z, s);
             if (rc != BSE_EUNSUPPORTED) return rc;
         }
@@ -609,7 +612,7 @@ struct Launch {
     }
     static int inv_plane(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s, int sub,
                          int force) {
-        if (!sub && force < 0 && use_pipe(P)) {
+        if (!sub && force < 0 && use_pipe(P, true, false)) {
             int rc = inv_plane_pipe(P, Z, count, N, out, s);
             if (rc != BSE_EUNSUPPORTED) return rc;
         }
