@@ -262,6 +262,10 @@ def main():
     ap.add_argument("--no-k1e", action="store_true")
     ap.add_argument("--tau-f32", action="store_true", help="mixed-precision variant: tau(G) kept as complex64 (BSE_TAU_F32); "
                     "not the headline (the 1e-10 parity bar applies to the double store)")
+    ap.add_argument("--reduce", default=None, metavar="Nv,Npdep,B",
+                    help="profiling only: the chosen config's grid, cell and sphere with fewer orbitals / PDEP vectors / blocks "
+                         "(cfg 3-5; ncu --set full saves and restores the whole device memory around every replay); the line "
+                         "is marked REDUCED and is not a bench value")
     ap.add_argument("--knob", action="append", default=[], help="key=value for bse_debug_set (tuning / A-B runs), repeatable")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -275,6 +279,8 @@ def main():
         sharded.bench_main(args, rank, local_rank, world)
         return
     args.warmup = max(args.warmup, 3)
+    if args.reduce:
+        args.no_e2e = args.no_cpu_baseline = True
 
     import psutil
     import torch
@@ -305,7 +311,11 @@ def main():
     t_gen0 = time.perf_counter()
     u_host = phi_host = a_host = out_host = None
     if large:
-        w = wl.make_device(args.config, dev)
+        if args.reduce:
+            r_nv, r_npdep, r_b = (int(x) for x in args.reduce.split(","))
+            w = wl.make_device(args.config, dev, Nv=r_nv, Npdep=r_npdep, B=r_b)
+        else:
+            w = wl.make_device(args.config, dev)
         B = w.a_pw.shape[0]
         u_d = w.u
         phi_d = torch.view_as_real(w.phi).contiguous()
@@ -551,7 +561,8 @@ def main():
         "metric": METRIC, "value": world * P / (t_pairs_ms * 1e-3), "unit": "pairs/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": tb_ms + ta_ms, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_string(args.config, w.n, Nv, n_pdep, npw_h, w.eta, P, B),
+        "config": {"workload": ("REDUCED for profiling, not a bench value: " if args.reduce else "")
+                               + workload_string(args.config, w.n, Nv, n_pdep, npw_h, w.eta, P, B),
                    "tau_storage": args.tau + (" (kept as complex64: mixed-precision variant)" if args.tau_f32 else ""),
                    "vec_layout": args.vec, "parallelism": "replicas" if world > 1 else "1gpu",
                    "l2": "512 MB buffer written between timed steps (L2 flush); inputs also exceed L2",

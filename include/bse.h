@@ -191,7 +191,9 @@ int bse_screen_overlap_static(const double *u, int Nv, long long N, double *M, v
  * (0 = never, -1 = automatic);  "slab_rows" = k caps the rows per chunk of the plane-slab apply (PW layout with tau on H; -1 = never
  * take that path, 0 = no cap), "slab_planes" = k the planes per slab; setting "max_group" or "max_batch" also keeps the apply on the group / row-batch path;
  * "pc_rows" = k caps the rows P_c projects per chunk (0 = no cap); "in_chunks" = k makes bse_set_inputs_host copy u in k
- * column slabs (0 = automatic: 8 from 256 MB on, else 1).
+ * column slabs (0 = automatic: 8 from 256 MB on, else 1);  "pipe" picks the plane-pass kernels (1 = the pipelined,
+ * bulk-copy staged ones wherever they fit, 0 = the one-plane-per-CTA ones, -1 = automatic: pipelined for the inverse and the
+ * single-field forward pass from n = 120 on), "pipe_lc" = k caps the packed lines per slab of the pipelined kernels (0 = no cap).
  * BSE_EINVAL for an unknown key. */
 int bse_debug_set(bse_handle *h, const char *key, long long value);
 /* Per-stage device time (CUDA events on the library's stream).  enable != 0 switches recording on (adds a
