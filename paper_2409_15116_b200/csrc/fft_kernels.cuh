@@ -22,6 +22,8 @@
 // Stick pass (one CTA = TS sticks of one pair, all i1): S1 from global, S2 to global with the v_c^{1/2}/N scaling and the
 // gather to the half sphere H (forward) / scatter from H (inverse) fused.
 #pragma once
+#include <cstdint>
+
 #include "bse_internal.h"
 #include "fft_codelets.cuh"
 
@@ -568,6 +570,8 @@ struct Launch {
         return BSE_OK;
     }
     static int inv_plane_pipe(const PlanDev &P, const double2 *Z, int count, long long N, double *out, cudaStream_t s) {
+        // bulk copies move 16-byte aligned pieces: a caller's buffer at an odd multiple of 8 bytes takes the one-plane kernels
+        if ((((uintptr_t)out | (uintptr_t)Z) & 15) || (N & 1)) return BSE_EUNSUPPORTED;
         const int LC = pick_lc(PG::inv_smem(P.W, P.NS, 0), G::LD * 16 + 2 * G::n * 8, P.pipe_lc);
         if (LC < 2) return BSE_EUNSUPPORTED;
         const int smem = PG::inv_smem(P.W, P.NS, LC);
@@ -581,6 +585,7 @@ struct Launch {
     }
     static int fwd_plane_pipe(const PlanDev &P, const double *fields, const int2 *pairs, long long p0, int count, long long N,
                               double2 *Z, cudaStream_t s) {
+        if (((uintptr_t)fields & 15) || (N & 1)) return BSE_EUNSUPPORTED;      // see inv_plane_pipe
         const int nf = pairs ? 2 : 1, NST = 2;
         const int LC = pick_lc(PG::fwd_smem(P.W, 0, NST, nf), G::LD * 16 + NST * nf * 2 * G::n * 8, P.pipe_lc);
         if (LC < 2) return BSE_EUNSUPPORTED;
