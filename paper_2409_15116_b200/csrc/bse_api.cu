@@ -36,6 +36,8 @@ int upload(T *&dst, const std::vector<T> &src) {
 
 // the accumulate launchers handle the trial blocks 8, 4, 2 or 1 at a time
 static int acc_launches(int nb) { return nb / 8 + ((nb & 4) ? 1 : 0) + ((nb & 2) ? 1 : 0) + (nb & 1); }
+// accumulate_rows: all whole groups of 8 blocks in ONE launch
+static int acc_rows_launches(int nb) { return (nb >= 8 ? 1 : 0) + ((nb & 4) ? 1 : 0) + ((nb & 2) ? 1 : 0) + (nb & 1); }
 
 struct StageTimer {
     bse_handle *h; int st;
@@ -765,7 +767,7 @@ int accumulate_all(bse_handle *h, const double *a, int nb, double *acc_real, dou
         }
         { StageTimer t(h, BSE_ST_ACCUM, 2.0 * nb * (double)pl.N * (double)h->nadj * rows / h->Nv,
                        m.N8 * (uniq * bt.nu + nb * rows + (r0 == 0 ? (double)nb * h->Nv : 0.0)));
-          t.launches = acc_launches(nb);
+          t.launches = acc_rows_launches(nb);
           if (acc_real) rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, h->rowlist + r0, rows, a, acc_real, h->Nv, false, nb);
           else rc = bse_launch_accumulate_rows(h, pl.N, h->tau_batch, h->eslot, h->rowlist + r0, rows, a, h->acc_r, h->rows_cap, true, nb);
           if (rc) return rc; }
@@ -844,7 +846,7 @@ int apply_pw_slab(bse_handle *h, const double2 *a, double2 *out, int B) {
             const double directed = (double)(h->adj_ptr_h[v0 + rows] - h->adj_ptr_h[v0]);
             { StageTimer t(h, BSE_ST_ACCUM, 2.0 * B * (double)SN * directed,
                            8.0 * SN * ((double)h->Pa * rows / nloc + (double)B * rows + (v0 == h->row0 ? (double)B * Nv : 0.0)));
-              t.launches = acc_launches(B);
+              t.launches = acc_rows_launches(B);
               if ((rc = bse_launch_accumulate_rows(h, SN, h->tau_batch, h->eslot_act, h->rowid + v0, rows, h->a_r, h->acc_r, rows,
                                                    true, B))) return rc; }
             if (h->mix_on) {
