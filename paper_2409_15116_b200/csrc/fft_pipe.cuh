@@ -67,12 +67,15 @@ struct PipeGeo {
     static constexpr int tables = n * 16 + 3 * n * 4;
     static __host__ __device__ int pad16(int b) { return (b + 15) & ~15; }
     // inverse: Cc[W*LDC] | Wk[LC*LD] | Os[2 LC n] | Zs[NS] | tables | mbar
+    // (one extra compact column and one extra stick that stay zero: what the predicates of the one-plane kernels skip is
+    // read from there, so the field loop has no divergent branches)
     static __host__ __device__ int inv_smem(int W, int NS, int LC) {
-        return W * G::LDC * 16 + LC * G::LD * 16 + 2 * LC * n * 8 + NS * 16 + pad16(tables) + 16;
+        return (W + 1) * G::LDC * 16 + LC * G::LD * 16 + 2 * LC * n * 8 + (NS + 1) * 16 + pad16(tables) + 16;
     }
     // forward: Cc[2W*LDL] | Wk[LC*LD] | raw[NST][nf][2 LC n] | tables | mbar[NST]
+    // (column 2W of the compact store takes the pruned frequencies |m3| > R: the rows pass stores without branching)
     static __host__ __device__ int fwd_smem(int W, int LC, int nst, int nf) {
-        return 2 * W * LDL * 16 + LC * G::LD * 16 + nst * nf * 2 * LC * n * 8 + pad16(tables) + 16 * nst;
+        return (2 * W + 1) * LDL * 16 + LC * G::LD * 16 + nst * nf * 2 * LC * n * 8 + pad16(tables) + 16 * nst;
     }
 };
 
@@ -87,11 +90,11 @@ inv_plane_pipe_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, dou
     constexpr int n = G::n, LD = G::LD, R2p = G::R2p, LDC = G::LDC;
     extern __shared__ __align__(16) unsigned char smem[];
     const int R = P.R, W = P.W, NS = P.NS;
-    double2 *Cc = reinterpret_cast<double2 *>(smem);
-    double2 *Wk = Cc + (size_t)W * LDC;
+    double2 *Cc = reinterpret_cast<double2 *>(smem);                 // [W + 1][LDC], column W stays zero
+    double2 *Wk = Cc + (size_t)(W + 1) * LDC;
     double *Os = reinterpret_cast<double *>(Wk + (size_t)LC * LD);
-    double2 *Zs = reinterpret_cast<double2 *>(Os + (size_t)2 * LC * n);
-    double2 *tw = Zs + NS;
+    double2 *Zs = reinterpret_cast<double2 *>(Os + (size_t)2 * LC * n);   // [NS + 1], stick NS stays zero
+    double2 *tw = Zs + NS + 1;
     int *soff = reinterpret_cast<int *>(tw + n);
     int *wmax = soff + n, *wmin = wmax + n;
     unsigned long long *mbar = reinterpret_cast<unsigned long long *>(reinterpret_cast<unsigned char *>(tw) + PG::pad16(PG::tables));
@@ -100,7 +103,8 @@ inv_plane_pipe_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, dou
     for (int i = tid; i < n; i += blockDim.x) {
         tw[i] = P.tw[i]; soff[i] = P.soff[i]; wmax[i] = P.wmax[i]; wmin[i] = P.wmin[i];
     }
-    if (tid == 0) { mbar_init(bar, 1); mbar_fence_init(); }
+    for (int i = tid; i < LDC; i += blockDim.x) Cc[(size_t)W * LDC + i] = make_double2(0.0, 0.0);
+    if (tid == 0) { Zs[NS] = make_double2(0.0, 0.0); mbar_init(bar, 1); mbar_fence_init(); }
     __syncthreads();
     long long it = blockIdx.x;
     const uint32_t zbytes = (uint32_t)NS * 16u;
@@ -118,11 +122,10 @@ inv_plane_pipe_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, dou
 #pragma unroll
             for (int q = 0; q < R1; ++q) {
                 const int t2 = j + q * R2;
-                double2 v = make_double2(0.0, 0.0);
-                if (m3 <= wmax[t2]) {
-                    if (m3 >= wmin[t2]) v = Zs[soff[t2] + m3];
-                    else { v = Zs[soff[n - t2]]; v.y = -v.y; }
-                }
+                const bool in = m3 <= wmax[t2], own = m3 >= wmin[t2];        // own: stored; else the mirror (-m2, 0), conjugated
+                const int idx = in ? soff[own ? t2 : n - t2] + (own ? m3 : 0) : NS;     // NS: the zero stick
+                double2 v = Zs[idx];
+                if (in && !own) v.y = -v.y;
                 x[q] = v;
             }
             Dft<R1, +1>::run(x);
@@ -144,8 +147,9 @@ inv_plane_pipe_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, dou
 #pragma unroll
             for (int q = 0; q < R2; ++q) x[q] = c[q];
             Dft<R2, +1>::run(x);
+            // column m3 = 0 is the transform of a Hermitian column: real up to rounding; the rows pass uses its real parts
 #pragma unroll
-            for (int q = 0; q < R2; ++q) c[q] = x[q];
+            for (int q = 0; q < R2; ++q) c[q] = m3 ? x[q] : make_double2(x[q].x, 0.0);
         }
         __syncthreads();
         double *o = out + p * N + (long long)i1 * n * n;
@@ -160,15 +164,11 @@ inv_plane_pipe_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, dou
 #pragma unroll
                 for (int q = 0; q < R1; ++q) {
                     const int e = j + q * R2;
-                    double2 v = make_double2(0.0, 0.0);
-                    if (e <= R) {
-                        const double2 a = Cc[e * LDC + sa], b = Cc[e * LDC + sb];
-                        v = e ? make_double2(a.x - b.y, a.y + b.x) : make_double2(a.x, b.x);
-                    } else if (e >= n - R) {
-                        const double2 a = Cc[(n - e) * LDC + sa], b = Cc[(n - e) * LDC + sb];
-                        v = make_double2(a.x + b.y, b.x - a.y);
-                    }
-                    x[q] = v;
+                    const bool lo = e <= R;
+                    const int col = lo ? e : (e >= n - R ? n - e : W);       // W: the zero column
+                    const double sg = lo ? 1.0 : -1.0;
+                    const double2 a = Cc[col * LDC + sa], b = Cc[col * LDC + sb];
+                    x[q] = make_double2(fma(-sg, b.y, a.x), fma(sg, a.y, b.x));
                 }
                 Dft<R1, +1>::run(x);
                 twiddle_powers<R1>(x, cconj(tw[j]));
@@ -210,8 +210,8 @@ fwd_plane_pipe_kernel(PlanDev P, const double *__restrict__ fields, const int2 *
     extern __shared__ __align__(16) unsigned char smem[];
     const int R = P.R, W = P.W;
     const int nf = pairs ? 2 : 1;
-    double2 *Cc = reinterpret_cast<double2 *>(smem);                 // [2W][LDL]: column m3 and, at W + m3, column n - m3
-    double2 *Wk = Cc + (size_t)2 * W * LDL;
+    double2 *Cc = reinterpret_cast<double2 *>(smem);                 // [2W + 1][LDL]: column m3 and, at W + m3, column n - m3
+    double2 *Wk = Cc + (size_t)(2 * W + 1) * LDL;
     double *raw = reinterpret_cast<double *>(Wk + (size_t)LC * LD);
     const int stage_dbl = nf * 2 * LC * n;
     double2 *tw = reinterpret_cast<double2 *>(raw + (size_t)NST * stage_dbl);
@@ -292,8 +292,8 @@ fwd_plane_pipe_kernel(PlanDev P, const double *__restrict__ fields, const int2 *
 #pragma unroll
                 for (int k2 = 0; k2 < R2; ++k2) {
                     const int k = blk + R1 * k2;
-                    if (k <= R) Cc[k * LDL + l0 + ll] = x[k2];
-                    else if (k >= n - R) Cc[(W + n - k) * LDL + l0 + ll] = x[k2];
+                    const int col = k <= R ? k : (k >= n - R ? W + n - k : 2 * W);      // 2W: pruned, never read
+                    Cc[col * LDL + l0 + ll] = x[k2];
                 }
             }
             __syncthreads();

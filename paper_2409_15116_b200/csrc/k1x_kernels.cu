@@ -156,7 +156,7 @@ accumulate_kernel(const double *__restrict__ tau, long long p_first, long long p
 // directed entry e in the batch.  Each output row is written once, never re-read:
 //   acc[b * acc_ld + (local ? i : v)][r] = sum_{e in row v} tau_b[eslot[e]][r] * a[b][adj[e].x][r],  v = rows[i]
 // grid = (rows, ceil(N / (2*blockDim))); rows vary fastest across resident CTAs, so they share the r-tile of a in L2.
-template <int BB>
+template <int BB, bool GROUPS>
 __global__ void __launch_bounds__(256)
 accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict__ eslot,
                        const int *__restrict__ rows, const int *__restrict__ adj_ptr,
@@ -164,8 +164,8 @@ accumulate_rows_kernel(const double *__restrict__ tau_dir, const int *__restrict
                        long long N, int b0, long long acc_ld, int local, int ngroups) {
     // ngroups > 1: blockIdx.x = row * ngroups + g, the CTA takes the blocks b0 + g BB .. of its row.  The CTAs of one row and
     // tile then run side by side, so tau(r) of the row's pairs comes from HBM once and from L2 for the other groups
-    const int ri = blockIdx.x / ngroups;
-    b0 += (blockIdx.x - ri * ngroups) * BB;
+    const int ri = GROUPS ? blockIdx.x / ngroups : blockIdx.x;
+    if (GROUPS) b0 += (blockIdx.x - ri * ngroups) * BB;
     const int v = rows[ri];                          // the batch is a cluster of rows, not a range
     const int arow = local ? ri : v;                 // acc_r of the PW layout holds the batch's rows in batch order
     const long long r = 2 * ((long long)blockIdx.y * blockDim.x + threadIdx.x);
@@ -398,12 +398,12 @@ int bse_launch_accumulate_rows(bse_handle *h, long long N, const double *tau_dir
     int b0 = 0;
     const int ng = B / 8;                            // whole groups of 8 blocks: one launch, the groups of a row side by side
     if (ng > 1) {
-        accumulate_rows_kernel<8><<<dim3(nrows * ng, (unsigned)tiles), threads, 0, h->stream>>>(
+        accumulate_rows_kernel<8, true><<<dim3(nrows * ng, (unsigned)tiles), threads, 0, h->stream>>>(
             tau_dir, eslot, rows, h->adj_ptr, h->adj, a, acc, h->Nv, N, 0, acc_ld, local ? 1 : 0, ng);
         b0 = 8 * ng;
     }
 #define BSE_ROWS(BB)                                                                                              \
-    accumulate_rows_kernel<BB><<<grid, threads, 0, h->stream>>>(tau_dir, eslot, rows, h->adj_ptr, h->adj, a, acc, h->Nv, \
+    accumulate_rows_kernel<BB, false><<<grid, threads, 0, h->stream>>>(tau_dir, eslot, rows, h->adj_ptr, h->adj, a, acc, h->Nv, \
                                                                 N, b0, acc_ld, local ? 1 : 0, 1)
     while (b0 < B) {
         const int left = B - b0;
