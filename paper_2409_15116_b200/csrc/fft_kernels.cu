@@ -80,7 +80,8 @@ int bse_launch_inv_stick_slab(const FftPlan &pl, int S, int M, const double2 *T,
     (small ? (S <= 4 ? bsefft::name<4, 512, ##__VA_ARGS__> : (S <= 8 ? bsefft::name<8, 512, ##__VA_ARGS__> : (S <= 12 ? bsefft::name<12, 512, ##__VA_ARGS__> : bsefft::name<16, 512, ##__VA_ARGS__>))) \
            : (S <= 4 ? bsefft::name<4, 1024, ##__VA_ARGS__> : (S <= 8 ? bsefft::name<8, 1024, ##__VA_ARGS__> : (S <= 12 ? bsefft::name<12, 1024, ##__VA_ARGS__> : bsefft::name<16, 1024, ##__VA_ARGS__>))))
     auto kern = T32 ? BSE_SLAB_PICK(inv_stick_slab_kernel, true) : BSE_SLAB_PICK(inv_stick_slab_kernel, false);
-    kern<<<grid, TS * M, smem, s>>>(P, pl.n, S, M, A, T, pl.npw_h, Zs, gather, g0, slab, count, per, T32);
+    kern<<<grid, TS * M, smem, s>>>(P, pl.n, S, M, A, T, pl.npw_h, Zs, gather, g0, slab, count, per, T32,
+                                    bsefft::slab_const(pl.n, M, A));
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }
@@ -96,7 +97,7 @@ int bse_launch_fwd_stick_slab(const FftPlan &pl, int S, int M, const double2 *Zs
     const bool small = TS * M <= 512;
     auto kern = BSE_SLAB_PICK(fwd_stick_slab_kernel);
     kern<<<grid, TS * M, smem, s>>>(P, pl.n, S, M, A, Zs, X, pl.npw_h, scale, slab, accumulate ? 1 : 0, rc_rows, row_ld, row0,
-                                    count, per);
+                                    count, per, bsefft::slab_const(pl.n, M, A));
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }

@@ -31,15 +31,25 @@ __device__ __forceinline__ double2 cmul_s(double2 v, double2 w) {
 // M-point transform of the TS sticks held in C[j][stick]; thread t (< M) of lane sl returns the value of index
 // k = k1 + A k2, k1 = t / B, k2 = t % B.  D is the second buffer; contains one __syncthreads (every thread must call) and
 // expects C complete (a barrier) on entry.
+// Host-computed constants of one split n = S M, M = A B (no integer division in the kernels): the root strides n/A, n/B, n/M
+// and the multiplier that turns t / B into a multiply-shift (exact for t < 64, B <= 32).
+struct SlabConst {
+    int B, nA, nB, nM, magicB;
+};
+inline SlabConst slab_const(int n, int M, int A) {
+    const int B = M / A;
+    return SlabConst{B, n / A, n / B, n / M, (65536 + B - 1) / B};
+}
+
 template <int SIGN>
 __device__ __forceinline__ double2 slab_dft(const double2 *C, double2 *D, const double2 *__restrict__ tw, int n, int M, int A,
-                                            int B, int t, int sl, int &k_out) {
+                                            int B, int t, int sl, int &k_out, const SlabConst sc) {
     constexpr int LDT = SLAB_TS + 1;
-    const int k1 = t / B, r2 = t - k1 * B;                      // pass 1: (k1, j2 = r2); pass 2: (k1, k2 = r2)
+    const int k1 = (t * sc.magicB) >> 16, r2 = t - k1 * B;      // t / B, t % B.  pass 1: (k1, j2 = r2); pass 2: (k1, k2 = r2)
     double2 z = make_double2(0.0, 0.0);
     {
         int wi = 0;                                             // (k1 j1 mod A) * (n / A)
-        const int wstep = k1 * (n / A);
+        const int wstep = k1 * sc.nA;
         const double2 *c = C + r2 * LDT + sl;
         for (int j1 = 0; j1 < A; ++j1) {
             const double2 p = cmul_s<SIGN>(c[j1 * B * LDT], tw[wi]);
@@ -48,14 +58,14 @@ __device__ __forceinline__ double2 slab_dft(const double2 *C, double2 *D, const 
             wi += wstep;
             if (wi >= n) wi -= n;
         }
-        z = cmul_s<SIGN>(z, tw[k1 * r2 * (n / M)]);             // w_M^{k1 j2}, k1 j2 < M
+        z = cmul_s<SIGN>(z, tw[k1 * r2 * sc.nM]);               // w_M^{k1 j2}, k1 j2 < M
     }
     D[t * LDT + sl] = z;                                        // D[k1 B + j2]
     __syncthreads();
     double2 x = make_double2(0.0, 0.0);
     {
         int wi = 0;                                             // (k2 j2 mod B) * (n / B)
-        const int wstep = r2 * (n / B);
+        const int wstep = r2 * sc.nB;
         const double2 *d = D + k1 * B * LDT + sl;
         for (int j2 = 0; j2 < B; ++j2) {
             const double2 p = cmul_s<SIGN>(d[j2 * LDT], tw[wi]);
@@ -75,10 +85,10 @@ __device__ __forceinline__ double2 slab_dft(const double2 *C, double2 *D, const 
 // NQ = S rounded up to a multiple of 4 (template: the index registers are a compile-time array); MAXT = 512 or 1024 bounds the
 // CTA (32 M threads), so that slabs of <= 16 planes get 128 registers per thread.
 template <int NQ, int MAXT, bool F32>
-__global__ void __launch_bounds__(MAXT)
+__global__ void __launch_bounds__(MAXT, MAXT <= 512 ? 2 : 1)
 inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__restrict__ T, long long npw_h,
                       double2 *__restrict__ Zs, const int *__restrict__ gather, int g0, int slab, int count, int per_cta,
-                      const float2 *__restrict__ T32) {
+                      const float2 *__restrict__ T32, const SlabConst sc) {
     constexpr int TS = SLAB_TS, LDT = TS + 1;
     extern __shared__ __align__(16) unsigned char smem[];
     double2 *C = reinterpret_cast<double2 *>(smem);
@@ -87,13 +97,14 @@ inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
     const int NS = P.NS, R = P.R;
     const int sl = threadIdx.x % TS, j = threadIdx.x / TS;      // lanes run over sticks: coalesced gathers
     const int sidx = blockIdx.x * TS + sl;
+    const int Bm = sc.B;                                        // M / A
     int code[NQ];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
         const int t1 = j + q * M;
         code[q] = (q < S && sidx < NS && (t1 <= R || t1 >= n - R)) ? P.hmapT[(long long)t1 * NS + sidx] : -1;   // |m1| <= R
     }
-    const int ti0 = (slab * j) % n, tstep = (slab * M) % n;     // (slab * t1) mod n for t1 = j + q M
+    const int ti0 = slab * j, tstep = slab * M;                 // (slab * t1) mod n for t1 = j + q M; slab j, slab M < S M = n
     const int p_end = min(count, (int)(blockIdx.y + 1) * per_cta);
     for (int p = blockIdx.y * per_cta; p < p_end; ++p) {
         const long long toff = (gather ? (long long)gather[g0 + p] : (long long)p) * npw_h;
@@ -129,17 +140,17 @@ inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
         C[j * LDT + sl] = y;
         __syncthreads();
         int k;
-        const double2 x = slab_dft<+1>(C, D, tw, n, M, A, M / A, j, sl, k);
+        const double2 x = slab_dft<+1>(C, D, tw, n, M, A, Bm, j, sl, k, sc);
         if (sidx < NS) Zs[((long long)p * M + k) * NS + sidx] = x;
     }
 }
 
 // field p of the launch goes to row  (p / rc) * row_ld + row0 + (p % rc)  of X (the rows of a chunk, block after block)
 template <int NQ, int MAXT>
-__global__ void __launch_bounds__(MAXT)
+__global__ void __launch_bounds__(MAXT, MAXT <= 512 ? 2 : 1)
 fwd_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__restrict__ Zs, double2 *__restrict__ X,
                       long long npw_h, const double *__restrict__ scale, int slab, int accumulate, int rc, long long row_ld,
-                      long long row0, int count, int per_cta) {
+                      long long row0, int count, int per_cta, const SlabConst sc) {
     constexpr int TS = SLAB_TS, LDT = TS + 1;
     extern __shared__ __align__(16) unsigned char smem[];
     double2 *C = reinterpret_cast<double2 *>(smem);
@@ -149,14 +160,14 @@ fwd_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
     const int sl = threadIdx.x % TS, t = threadIdx.x / TS;
     const int sidx = blockIdx.x * TS + sl;
     // this thread's output residue j = k1 + A k2 (what slab_dft returns for thread t) and its targets on H, with their scale
-    const int Bf = M / A, j = t / Bf + A * (t % Bf);
+    const int Bf = sc.B, tq = (t * sc.magicB) >> 16, j = tq + A * (t - tq * Bf);     // Bf = M / A; j = t / Bf + A (t % Bf)
     int hh[NQ];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
         const int t1 = j + q * M;
         hh[q] = (q < S && sidx < NS && (t1 <= R || t1 >= n - R)) ? P.hmapT[(long long)t1 * NS + sidx] : -1;
     }
-    const int ti0 = (slab * j) % n, tstep = (slab * M) % n;
+    const int ti0 = slab * j, tstep = slab * M;                 // both < S M = n
     const int p_end = min(count, (int)(blockIdx.y + 1) * per_cta);
     for (int p = blockIdx.y * per_cta; p < p_end; ++p) {
         const double2 zin = sidx < NS ? Zs[((long long)p * M + t) * NS + sidx] : make_double2(0.0, 0.0);   // plane k = t of the slab
@@ -165,7 +176,7 @@ fwd_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
         C[t * LDT + sl] = zin;
         __syncthreads();
         int jj;                                                 // Y[j] = sum_k x[k] e^{-2 pi i k j / M}
-        const double2 y = slab_dft<-1>(C, D, tw, n, M, A, Bf, t, sl, jj);
+        const double2 y = slab_dft<-1>(C, D, tw, n, M, A, Bf, t, sl, jj, sc);
         int ti = ti0;
         // one read-modify-write after the other (measured: a batch of reads followed by a batch of writes is slower)
 #pragma unroll
