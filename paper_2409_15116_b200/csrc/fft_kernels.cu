@@ -72,7 +72,8 @@ int bse_launch_inv_stick_slab(const FftPlan &pl, int S, int M, const double2 *T,
     if (S * M != pl.n || M > 32 || M < 1 || S > 16) { bse_set_error("slab stick pass: bad factorisation"); return BSE_EINVAL; }
     const PlanDev P = to_dev(pl);
     const int TS = bsefft::SLAB_TS, A = slab_split(M), groups = (pl.NS + TS - 1) / TS;
-    const int smem = 2 * M * (TS + 1) * 16;
+    const int NQt = S <= 4 ? 4 : (S <= 8 ? 8 : (S <= 12 ? 12 : 16)), Bt = M / A;
+    const int smem = (2 * M * (TS + 1) + NQt * M + A * A + M + Bt * Bt) * 16;     // C | D | root tables (fft_slab.cuh)
     const int per = slab_per_cta(groups, count);
     const dim3 grid(groups, (count + per - 1) / per);
     const bool small = TS * M <= 512;
@@ -91,8 +92,10 @@ int bse_launch_fwd_stick_slab(const FftPlan &pl, int S, int M, const double2 *Zs
     if (S * M != pl.n || M > 32 || M < 1 || S > 16) { bse_set_error("slab stick pass: bad factorisation"); return BSE_EINVAL; }
     const PlanDev P = to_dev(pl);
     const int TS = bsefft::SLAB_TS, A = slab_split(M), groups = (pl.NS + TS - 1) / TS;
-    const int smem = 2 * M * (TS + 1) * 16;
-    const int per = 1;          // one field per CTA: the read-modify-writes of many short CTAs overlap better than a walk
+    const int NQt = S <= 4 ? 4 : (S <= 8 ? 8 : (S <= 12 ? 12 : 16)), Bt = M / A;
+    const int smem = (2 * M * (TS + 1) + NQt * M + A * A + M + Bt * Bt) * 16;     // C | D | root tables (fft_slab.cuh)
+    const int per = count >= 1024 ? 4 : 1;     // few fields per CTA: the read-modify-writes of many short CTAs overlap better than
+                                               // a long walk; four amortise the index map (11.4 -> 11.0 ms on the reduced cfg 5)
     const dim3 grid(groups, (count + per - 1) / per);
     const bool small = TS * M <= 512;
     auto kern = BSE_SLAB_PICK(fwd_stick_slab_kernel);

@@ -41,38 +41,47 @@ inline SlabConst slab_const(int n, int M, int A) {
     return SlabConst{B, n / A, n / B, n / M, (65536 + B - 1) / B};
 }
 
+// Root tables of one CTA in shared memory (every entry is read by all lanes of a warp at once: broadcasts), filled once by
+// slab_tables:  Wf[q M + j] = tw[slab (j + q M) mod n]  (the fold),  W1[k1 A + j1] = w_A^{k1 j1},  Wm[t] = w_M^{k1 j2} (t = k1 B + j2),
+// W2[k2 B + j2] = w_B^{k2 j2};  all as tw[.] = e^{-2 pi i ./n}, conjugated by cmul_s for the inverse.
+struct SlabTables {
+    const double2 *Wf, *W1, *Wm, *W2;
+};
+__device__ __forceinline__ int slab_table_size(int NQ, int M, int A, int B) { return NQ * M + A * A + M + B * B; }
+__device__ __forceinline__ SlabTables slab_tables(double2 *base, const double2 *__restrict__ tw, int n, int NQ, int M, int A,
+                                                  int B, int slab, const SlabConst sc) {
+    double2 *Wf = base, *W1 = Wf + NQ * M, *Wm = W1 + A * A, *W2 = Wm + M;
+    for (int i = threadIdx.x; i < NQ * M; i += blockDim.x) Wf[i] = tw[(int)(((long long)slab * i) % n)];   // i = q M + j = t1
+    for (int i = threadIdx.x; i < A * A; i += blockDim.x) W1[i] = tw[(((i / A) * (i % A)) % A) * sc.nA];
+    for (int i = threadIdx.x; i < M; i += blockDim.x) Wm[i] = tw[(i / B) * (i % B) * sc.nM];
+    for (int i = threadIdx.x; i < B * B; i += blockDim.x) W2[i] = tw[(((i / B) * (i % B)) % B) * sc.nB];
+    return SlabTables{Wf, W1, Wm, W2};
+}
+
 template <int SIGN>
-__device__ __forceinline__ double2 slab_dft(const double2 *C, double2 *D, const double2 *__restrict__ tw, int n, int M, int A,
-                                            int B, int t, int sl, int &k_out, const SlabConst sc) {
+__device__ __forceinline__ double2 slab_dft(const double2 *C, double2 *D, const SlabTables &tb, int A, int B, int t, int sl,
+                                            int &k_out, const SlabConst sc) {
     constexpr int LDT = SLAB_TS + 1;
     const int k1 = (t * sc.magicB) >> 16, r2 = t - k1 * B;      // t / B, t % B.  pass 1: (k1, j2 = r2); pass 2: (k1, k2 = r2)
     double2 z = make_double2(0.0, 0.0);
     {
-        int wi = 0;                                             // (k1 j1 mod A) * (n / A)
-        const int wstep = k1 * sc.nA;
-        const double2 *c = C + r2 * LDT + sl;
+        const double2 *c = C + r2 * LDT + sl, *w = tb.W1 + k1 * A;
         for (int j1 = 0; j1 < A; ++j1) {
-            const double2 p = cmul_s<SIGN>(c[j1 * B * LDT], tw[wi]);
+            const double2 p = cmul_s<SIGN>(c[j1 * B * LDT], w[j1]);
             z.x += p.x;
             z.y += p.y;
-            wi += wstep;
-            if (wi >= n) wi -= n;
         }
-        z = cmul_s<SIGN>(z, tw[k1 * r2 * sc.nM]);               // w_M^{k1 j2}, k1 j2 < M
+        z = cmul_s<SIGN>(z, tb.Wm[t]);                          // w_M^{k1 j2}
     }
     D[t * LDT + sl] = z;                                        // D[k1 B + j2]
     __syncthreads();
     double2 x = make_double2(0.0, 0.0);
     {
-        int wi = 0;                                             // (k2 j2 mod B) * (n / B)
-        const int wstep = r2 * sc.nB;
-        const double2 *d = D + k1 * B * LDT + sl;
+        const double2 *d = D + k1 * B * LDT + sl, *w = tb.W2 + r2 * B;
         for (int j2 = 0; j2 < B; ++j2) {
-            const double2 p = cmul_s<SIGN>(d[j2 * LDT], tw[wi]);
+            const double2 p = cmul_s<SIGN>(d[j2 * LDT], w[j2]);
             x.x += p.x;
             x.y += p.y;
-            wi += wstep;
-            if (wi >= n) wi -= n;
         }
     }
     k_out = k1 + A * r2;
@@ -93,25 +102,25 @@ inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
     extern __shared__ __align__(16) unsigned char smem[];
     double2 *C = reinterpret_cast<double2 *>(smem);
     double2 *D = C + M * LDT;
-    const double2 *__restrict__ tw = P.tw;                      // small table, read through L1
     const int NS = P.NS, R = P.R;
     const int sl = threadIdx.x % TS, j = threadIdx.x / TS;      // lanes run over sticks: coalesced gathers
     const int sidx = blockIdx.x * TS + sl;
     const int Bm = sc.B;                                        // M / A
+    const SlabTables tb = slab_tables(D + M * LDT, P.tw, n, NQ, M, A, Bm, slab, sc);
+    __syncthreads();
     int code[NQ];
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
         const int t1 = j + q * M;
         code[q] = (q < S && sidx < NS && (t1 <= R || t1 >= n - R)) ? P.hmapT[(long long)t1 * NS + sidx] : -1;   // |m1| <= R
     }
-    const int ti0 = slab * j, tstep = slab * M;                 // (slab * t1) mod n for t1 = j + q M; slab j, slab M < S M = n
+    const double2 *wf = tb.Wf + j;                              // wf[q M] = e^{-2 pi i slab t1 / n} for t1 = j + q M
     const int p_end = min(count, (int)(blockIdx.y + 1) * per_cta);
     for (int p = blockIdx.y * per_cta; p < p_end; ++p) {
         const long long toff = (gather ? (long long)gather[g0 + p] : (long long)p) * npw_h;
         const double2 *tg = T + toff;
         const float2 *tg32 = F32 ? T32 + toff : nullptr;        // coefficients kept in single precision (BSE_TAU_F32)
         double2 y = make_double2(0.0, 0.0);
-        int ti = ti0;
 #pragma unroll
         for (int q0 = 0; q0 < NQ; q0 += 4) {
             double2 v[4];
@@ -129,18 +138,16 @@ inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
             }
 #pragma unroll
             for (int u = 0; u < 4; ++u) {
-                const double2 pr = cmul_s<+1>(v[u], tw[ti]);    // times e^{+2 pi i slab t1 / n}
+                const double2 pr = cmul_s<+1>(v[u], wf[(q0 + u) * M]);    // times e^{+2 pi i slab t1 / n}
                 y.x += pr.x;
                 y.y += pr.y;
-                ti += tstep;
-                if (ti >= n) ti -= n;
             }
         }
         __syncthreads();                                        // the previous field's transform has left C and D
         C[j * LDT + sl] = y;
         __syncthreads();
         int k;
-        const double2 x = slab_dft<+1>(C, D, tw, n, M, A, Bm, j, sl, k, sc);
+        const double2 x = slab_dft<+1>(C, D, tb, A, Bm, j, sl, k, sc);
         if (sidx < NS) Zs[((long long)p * M + k) * NS + sidx] = x;
     }
 }
@@ -155,10 +162,10 @@ fwd_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
     extern __shared__ __align__(16) unsigned char smem[];
     double2 *C = reinterpret_cast<double2 *>(smem);
     double2 *D = C + M * LDT;
-    const double2 *__restrict__ tw = P.tw;
     const int NS = P.NS, R = P.R;
     const int sl = threadIdx.x % TS, t = threadIdx.x / TS;
     const int sidx = blockIdx.x * TS + sl;
+    const SlabTables tb = slab_tables(D + M * LDT, P.tw, n, NQ, M, A, sc.B, slab, sc);   // first used after the barriers below
     // this thread's output residue j = k1 + A k2 (what slab_dft returns for thread t) and its targets on H, with their scale
     const int Bf = sc.B, tq = (t * sc.magicB) >> 16, j = tq + A * (t - tq * Bf);     // Bf = M / A; j = t / Bf + A (t % Bf)
     int hh[NQ];
@@ -167,7 +174,7 @@ fwd_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
         const int t1 = j + q * M;
         hh[q] = (q < S && sidx < NS && (t1 <= R || t1 >= n - R)) ? P.hmapT[(long long)t1 * NS + sidx] : -1;
     }
-    const int ti0 = slab * j, tstep = slab * M;                 // both < S M = n
+    const double2 *wf = tb.Wf + j;
     const int p_end = min(count, (int)(blockIdx.y + 1) * per_cta);
     for (int p = blockIdx.y * per_cta; p < p_end; ++p) {
         const double2 zin = sidx < NS ? Zs[((long long)p * M + t) * NS + sidx] : make_double2(0.0, 0.0);   // plane k = t of the slab
@@ -176,20 +183,17 @@ fwd_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
         C[t * LDT + sl] = zin;
         __syncthreads();
         int jj;                                                 // Y[j] = sum_k x[k] e^{-2 pi i k j / M}
-        const double2 y = slab_dft<-1>(C, D, tw, n, M, A, Bf, t, sl, jj, sc);
-        int ti = ti0;
+        const double2 y = slab_dft<-1>(C, D, tb, A, Bf, t, sl, jj, sc);
         // one read-modify-write after the other (measured: a batch of reads followed by a batch of writes is slower)
 #pragma unroll
         for (int q = 0; q < NQ; ++q) {
             if (hh[q] >= 0) {
-                const double2 pr = cmul_s<-1>(y, tw[ti]);       // times e^{-2 pi i slab t1 / n}
+                const double2 pr = cmul_s<-1>(y, wf[q * M]);    // times e^{-2 pi i slab t1 / n}
                 const double sc = scale[hh[q]];
                 double2 v = make_double2(pr.x * sc, pr.y * sc);
                 if (accumulate) { const double2 o = xo[hh[q]]; v.x += o.x; v.y += o.y; }
                 xo[hh[q]] = v;
             }
-            ti += tstep;
-            if (ti >= n) ti -= n;
         }
     }
 }
