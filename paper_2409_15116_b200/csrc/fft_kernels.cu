@@ -61,9 +61,11 @@ static int slab_split(int M) {
         if (M % a == 0) A = a;
     return A;
 }
-// the fields of a launch are spread over the CTAs of a stick group so that the grid holds ~8 CTAs per SM
+// the fields of a launch are spread over the CTAs of a stick group
 static int slab_per_cta(int groups, int count) {
-    const int want = std::max(1, (148 * 8 + groups - 1) / groups);      // field chunks per stick group
+    // two CTAs are resident per SM (64 registers, 480 threads): ~16 waves of 296 CTAs, so that the last, partial wave costs
+    // little (with 4 waves of CTAs that walk over 250 fields each, the tail was a sixth of the launch)
+    const int want = std::max(1, (148 * 2 * 16 + groups - 1) / groups);   // field chunks per stick group
     return std::max(1, (count + want - 1) / want);
 }
 int bse_launch_inv_stick_slab(const FftPlan &pl, int S, int M, const double2 *T, int count, double2 *Zs, cudaStream_t s, int slab,
@@ -94,8 +96,8 @@ int bse_launch_fwd_stick_slab(const FftPlan &pl, int S, int M, const double2 *Zs
     const int TS = bsefft::SLAB_TS, A = slab_split(M), groups = (pl.NS + TS - 1) / TS;
     const int NQt = S <= 4 ? 4 : (S <= 8 ? 8 : (S <= 12 ? 12 : 16)), Bt = M / A;
     const int smem = (2 * M * (TS + 1) + NQt * M + A * A + M + Bt * Bt) * 16;     // C | D | root tables (fft_slab.cuh)
-    const int per = count >= 1024 ? 4 : 1;     // few fields per CTA: the read-modify-writes of many short CTAs overlap better than
-                                               // a long walk; four amortise the index map (11.4 -> 11.0 ms on the reduced cfg 5)
+    const int per = count >= 2048 ? 8 : (count >= 1024 ? 4 : 1);     // few fields per CTA: the read-modify-writes of many short CTAs overlap better than
+                                               // a long walk; a few amortise the index map and the root tables (cfg 5: 1 / 4 / 8 / 16 fields: 245 / 224 / 220 / 218 ms)
     const dim3 grid(groups, (count + per - 1) / per);
     const bool small = TS * M <= 512;
     auto kern = BSE_SLAB_PICK(fwd_stick_slab_kernel);
