@@ -82,9 +82,15 @@ int bse_launch_inv_stick_slab(const FftPlan &pl, int S, int M, const double2 *T,
 #define BSE_SLAB_PICK(name, ...) \
     (small ? (S <= 4 ? bsefft::name<4, 512, ##__VA_ARGS__> : (S <= 8 ? bsefft::name<8, 512, ##__VA_ARGS__> : (S <= 12 ? bsefft::name<12, 512, ##__VA_ARGS__> : bsefft::name<16, 512, ##__VA_ARGS__>))) \
            : (S <= 4 ? bsefft::name<4, 1024, ##__VA_ARGS__> : (S <= 8 ? bsefft::name<8, 1024, ##__VA_ARGS__> : (S <= 12 ? bsefft::name<12, 1024, ##__VA_ARGS__> : bsefft::name<16, 1024, ##__VA_ARGS__>))))
-    auto kern = T32 ? BSE_SLAB_PICK(inv_stick_slab_kernel, true) : BSE_SLAB_PICK(inv_stick_slab_kernel, false);
-    kern<<<grid, TS * M, smem, s>>>(P, pl.n, S, M, A, T, pl.npw_h, Zs, gather, g0, slab, count, per, T32,
-                                    bsefft::slab_const(pl.n, M, A));
+    // staged gathers (cp.async, one field ahead) where two CTAs per SM still fit beside the staging area
+    const int stage_bytes = NQt * TS * M * 16;
+    const bool staged = !T32 && small && per > 1 && 2 * (smem + stage_bytes + 1024) <= 232448;
+    const int smem_all = smem + (staged ? stage_bytes : 0);
+    auto kern = T32 ? BSE_SLAB_PICK(inv_stick_slab_kernel, true, false)
+                    : (staged ? BSE_SLAB_PICK(inv_stick_slab_kernel, false, true) : BSE_SLAB_PICK(inv_stick_slab_kernel, false, false));
+    if (smem_all > 48 * 1024) BSE_CUDA(cudaFuncSetAttribute((const void *)kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_all));
+    kern<<<grid, TS * M, smem_all, s>>>(P, pl.n, S, M, A, T, pl.npw_h, Zs, gather, g0, slab, count, per, T32,
+                                        bsefft::slab_const(pl.n, M, A));
     BSE_CUDA(cudaGetLastError());
     return BSE_OK;
 }

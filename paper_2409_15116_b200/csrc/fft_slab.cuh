@@ -93,7 +93,9 @@ __device__ __forceinline__ double2 slab_dft(const double2 *C, double2 *D, const 
 // costs one round of independent, stick-coalesced gathers (no index load in front of them).  S <= 16.
 // NQ = S rounded up to a multiple of 4 (template: the index registers are a compile-time array); MAXT = 512 or 1024 bounds the
 // CTA (32 M threads), so that slabs of <= 16 planes get 128 registers per thread.
-template <int NQ, int MAXT, bool F32>
+// STAGED (double coefficients, where the staging area fits beside two CTAs per SM): the NQ gathers of the NEXT field go to
+// G[q][thread] by cp.async while this field's M-point transform runs; a thread reads back only what it copied itself.
+template <int NQ, int MAXT, bool F32, bool STAGED>
 __global__ void __launch_bounds__(MAXT, MAXT <= 512 ? 2 : 1)
 inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__restrict__ T, long long npw_h,
                       double2 *__restrict__ Zs, const int *__restrict__ gather, int g0, int slab, int count, int per_cta,
@@ -107,6 +109,7 @@ inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
     const int sidx = blockIdx.x * TS + sl;
     const int Bm = sc.B;                                        // M / A
     const SlabTables tb = slab_tables(D + M * LDT, P.tw, n, NQ, M, A, Bm, slab, sc);
+    double2 *G = D + M * LDT + slab_table_size(NQ, M, A, Bm);
     __syncthreads();
     int code[NQ];
 #pragma unroll
@@ -116,11 +119,35 @@ inv_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
     }
     const double2 *wf = tb.Wf + j;                              // wf[q M] = e^{-2 pi i slab t1 / n} for t1 = j + q M
     const int p_end = min(count, (int)(blockIdx.y + 1) * per_cta);
+    auto stage_field = [&](int p) {
+        const double2 *tg = T + (gather ? (long long)gather[g0 + p] : (long long)p) * npw_h;
+#pragma unroll
+        for (int q = 0; q < NQ; ++q) {
+            const int c = code[q];
+            const double2 *src = c >= 0 ? tg + c : (c <= -2 ? tg + (-2 - c) : tg);
+            const unsigned dst = (unsigned)__cvta_generic_to_shared(G + q * blockDim.x + threadIdx.x);
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(dst), "l"(src), "r"(c == -1 ? 0 : 16));
+        }
+        asm volatile("cp.async.commit_group;\n" ::);
+    };
+    if (STAGED && (int)(blockIdx.y * per_cta) < p_end) stage_field(blockIdx.y * per_cta);
     for (int p = blockIdx.y * per_cta; p < p_end; ++p) {
         const long long toff = (gather ? (long long)gather[g0 + p] : (long long)p) * npw_h;
         const double2 *tg = T + toff;
         const float2 *tg32 = F32 ? T32 + toff : nullptr;        // coefficients kept in single precision (BSE_TAU_F32)
         double2 y = make_double2(0.0, 0.0);
+        if (STAGED) {
+            asm volatile("cp.async.wait_group 0;\n" ::: "memory");
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
+                double2 v = G[q * blockDim.x + threadIdx.x];
+                if (code[q] <= -2) v.y = -v.y;
+                const double2 pr = cmul_s<+1>(v, wf[q * M]);
+                y.x += pr.x;
+                y.y += pr.y;
+            }
+            if (p + 1 < p_end) stage_field(p + 1);
+        } else
 #pragma unroll
         for (int q0 = 0; q0 < NQ; q0 += 4) {
             double2 v[4];
