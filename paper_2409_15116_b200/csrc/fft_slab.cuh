@@ -203,8 +203,12 @@ fwd_stick_slab_kernel(PlanDev P, int n, int S, int M, int A, const double2 *__re
     }
     const double2 *wf = tb.Wf + j;
     const int p_end = min(count, (int)(blockIdx.y + 1) * per_cta);
+    const double2 *zp = Zs + ((long long)blockIdx.y * per_cta * M + t) * NS + sidx;     // plane k = t of the slab
+    double2 znext = (sidx < NS && (int)(blockIdx.y * per_cta) < p_end) ? *zp : make_double2(0.0, 0.0);
     for (int p = blockIdx.y * per_cta; p < p_end; ++p) {
-        const double2 zin = sidx < NS ? Zs[((long long)p * M + t) * NS + sidx] : make_double2(0.0, 0.0);   // plane k = t of the slab
+        const double2 zin = znext;
+        zp += (long long)M * NS;
+        if (sidx < NS && p + 1 < p_end) znext = *zp;            // the next field's value travels behind this field's transform
         double2 *xo = X + ((p / rc) * row_ld + row0 + (p % rc)) * npw_h;
         __syncthreads();
         C[t * LDT + sl] = zin;
