@@ -40,6 +40,7 @@ static PlanDev to_dev(const FftPlan &pl, int np = 0) {
     d.R = pl.R; d.W = pl.W; d.NS = pl.NS;
     d.np = np > 0 ? np : pl.n;
     d.pipe = pl.pipe; d.pipe_lc = pl.pipe_lc;
+    d.magicW = (1 << 20) / (pl.W > 0 ? pl.W : 1) + 1;
     d.tw = pl.tw; d.soff = pl.soff; d.wmax = pl.wmax; d.wmin = pl.wmin; d.hmapT = pl.hmapT;
     return d;
 }

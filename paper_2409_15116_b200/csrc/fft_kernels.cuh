@@ -39,6 +39,7 @@ struct PlanDev {
     const int *hmapT;       // [n][NS] (t1 = m1 mod n, stick) -> h in H, -1 outside the sphere, -2-h: conj of entry h
     int pipe;               // plane passes: -1 automatic, 0 the one-plane-per-CTA kernels, 1 the pipelined kernels (fft_pipe.cuh)
     int pipe_lc;            // > 0: at most this many packed lines per slab of the pipelined kernels (test knob)
+    int magicW;             // 2^20 / W + 1: task / W == (task * magicW) >> 20 for task < 4096, W <= 160 (no integer division)
 };
 
 // coefficient h of a field kept in double (t) or, when t32 != nullptr, in single precision
@@ -442,16 +443,18 @@ fwd_stick_kernel(PlanDev P, const double2 *__restrict__ Z, double2 *__restrict__
         const int blk = task / TS, sl = task - blk * TS;
         const int s = s0 + sl;
         if (s >= NS) continue;
+        int hh[R2];                           // the targets on H: fetched before the butterfly, their latency hides behind it
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) hh[k2] = P.hmapT[(blk + R1 * k2) * NS + s];
         double2 x[R2];
 #pragma unroll
         for (int q = 0; q < R2; ++q) x[q] = C[sl * LDS + blk * R2p + q];
         Dft<R2, -1>::run(x);
 #pragma unroll
         for (int k2 = 0; k2 < R2; ++k2) {
-            const int hh = P.hmapT[(blk + R1 * k2) * NS + s];
-            if (hh >= 0) {
-                const double sc = scale[hh];
-                xo[hh] = make_double2(x[k2].x * sc, x[k2].y * sc);
+            if (hh[k2] >= 0) {
+                const double sc = scale[hh[k2]];
+                xo[hh[k2]] = make_double2(x[k2].x * sc, x[k2].y * sc);
             }
         }
     }

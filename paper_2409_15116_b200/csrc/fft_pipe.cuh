@@ -117,7 +117,7 @@ inv_plane_pipe_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, dou
         parity ^= 1u;
         // I1 (columns pass 1 from the staged sticks; (m2<0, m3=0) is the conjugate of (-m2, 0))
         for (int task = tid; task < W * R2; task += blockDim.x) {
-            const int j = task / W, m3 = task - j * W;
+            const int j = (task * P.magicW) >> 20, m3 = task - j * W;                  // task / W
             double2 x[R1];
 #pragma unroll
             for (int q = 0; q < R1; ++q) {
@@ -141,7 +141,7 @@ inv_plane_pipe_kernel(PlanDev P, const double2 *__restrict__ Z, long long N, dou
         }
         // I2 (columns pass 2, in place): slot blk * R2p + k2 = fwdslot(row) then holds row blk + R1 k2 of column m3
         for (int task = tid; task < W * R1; task += blockDim.x) {
-            const int blk = task / W, m3 = task - blk * W;
+            const int blk = (task * P.magicW) >> 20, m3 = task - blk * W;              // task / W
             double2 *c = Cc + m3 * LDC + blk * R2p;
             double2 x[R2];
 #pragma unroll
@@ -300,7 +300,7 @@ fwd_plane_pipe_kernel(PlanDev P, const double *__restrict__ fields, const int2 *
         }
         // P3 (untangle rows 2l / 2l+1 + columns pass 1), columns m3 = 0..R; two DFTs per thread (rows j = 2jp, 2jp+1)
         for (int task = tid; task < W * (R2 / 2); task += blockDim.x) {
-            const int jp = task / W, m3 = task - jp * W;
+            const int jp = (task * P.magicW) >> 20, m3 = task - jp * W;                // task / W
             double2 *ca = Cc + m3 * LDL, *cb = Cc + (W + m3) * LDL;
             double2 xa[R1], xb[R1];
 #pragma unroll
@@ -331,7 +331,7 @@ fwd_plane_pipe_kernel(PlanDev P, const double *__restrict__ fields, const int2 *
         // P4 (columns pass 2): only sticks inside the disk leave the SM
         double2 *z = Z + it * (long long)P.NS;
         for (int task = tid; task < W * R1; task += blockDim.x) {
-            const int blk = task / W, m3 = task - blk * W;
+            const int blk = (task * P.magicW) >> 20, m3 = task - blk * W;              // task / W
             const double2 *ca = Cc + m3 * LDL + blk * (R2 / 2), *cb = Cc + (W + m3) * LDL + blk * (R2 / 2);
             double2 x[R2];
 #pragma unroll
