@@ -153,6 +153,19 @@ def test_several_groups_and_row_batches():
     assert rel(o3, o1) < 1e-12
 
 
+def test_seventeen_trial_blocks():
+    """B = 17: the accumulate stage takes the two whole groups of 8 blocks side by side in one launch (the grouped kernel
+    variant, otherwise only reached by cfg 5's B = 16) and the last block through the row kernel; slab path, group /
+    row-batch path and the REAL layout with tau on H."""
+    bse = _bse()
+    w = wl.make(cfg=wl.Config("b17", 10.0, 20, 7, 10, 6.0, 1.2, 0.8, 3.0, 0.02, 17, "random", seed=1717))
+    for tau in (bse.BSE_TAU_PW, bse.BSE_TAU_STREAM):
+        o_slab = _check_pw(w, tau, {"slab_rows": 3, "slab_planes": 5})
+        o_grp = _check_pw(w, tau, {"slab_rows": -1, "max_batch": 6})
+        assert rel(o_grp, o_slab) < 1e-12
+    _check_full(w, bse.BSE_TAU_PW, check_g=False, knobs={"max_batch": 5})
+
+
 def test_cfg1_full_all_modes():
     w = wl.make(1)
     bse = _bse()
