@@ -152,18 +152,13 @@ fwd_plane_kernel(PlanDev P, const double *__restrict__ fields, const int2 *__res
         const int jp = task / W, m3 = task - jp * W;
         const int sa = G::fwdslot(m3), sb = G::fwdslot(m3 ? n - m3 : n / 2);
         double2 xa[R1], xb[R1];
+        const int sbr = m3 ? sb : sa;          // m3 = 0: with zb := za the formulas below give (2 za.x, 0) and (2 za.y, 0): no branch
 #pragma unroll
         for (int q = 0; q < R1; ++q) {
             const int l = jp + q * (R2 / 2);
-            const double2 za = C[l * LD + sa];
-            if (m3 == 0) {
-                xa[q] = make_double2(2.0 * za.x, 0.0);
-                xb[q] = make_double2(2.0 * za.y, 0.0);
-            } else {
-                const double2 zb = C[l * LD + sb];
-                xa[q] = make_double2(za.x + zb.x, za.y - zb.y);       // za + conj(zb)      = 2 A[m3]
-                xb[q] = make_double2(za.y + zb.y, zb.x - za.x);       // (za - conj(zb))/i  = 2 B[m3]
-            }
+            const double2 za = C[l * LD + sa], zb = C[l * LD + sbr];
+            xa[q] = make_double2(za.x + zb.x, za.y - zb.y);           // za + conj(zb)      = 2 A[m3]
+            xb[q] = make_double2(za.y + zb.y, zb.x - za.x);           // (za - conj(zb))/i  = 2 B[m3]
         }
         Dft<R1, -1>::run(xa);
         Dft<R1, -1>::run(xb);

@@ -303,18 +303,13 @@ fwd_plane_pipe_kernel(PlanDev P, const double *__restrict__ fields, const int2 *
             const int jp = (task * P.magicW) >> 20, m3 = task - jp * W;                // task / W
             double2 *ca = Cc + m3 * LDL, *cb = Cc + (W + m3) * LDL;
             double2 xa[R1], xb[R1];
+            const double2 *cbr = m3 ? cb : ca;   // m3 = 0: with zb := za the formulas give (2 za.x, 0) and (2 za.y, 0): no branch
 #pragma unroll
             for (int q = 0; q < R1; ++q) {
                 const int l = jp + q * (R2 / 2);
-                const double2 za = ca[l];
-                if (m3 == 0) {
-                    xa[q] = make_double2(2.0 * za.x, 0.0);
-                    xb[q] = make_double2(2.0 * za.y, 0.0);
-                } else {
-                    const double2 zb = cb[l];
-                    xa[q] = make_double2(za.x + zb.x, za.y - zb.y);       // za + conj(zb)      = 2 A[m3]
-                    xb[q] = make_double2(za.y + zb.y, zb.x - za.x);       // (za - conj(zb))/i  = 2 B[m3]
-                }
+                const double2 za = ca[l], zb = cbr[l];
+                xa[q] = make_double2(za.x + zb.x, za.y - zb.y);           // za + conj(zb)      = 2 A[m3]
+                xb[q] = make_double2(za.y + zb.y, zb.x - za.x);           // (za - conj(zb))/i  = 2 B[m3]
             }
             Dft<R1, -1>::run(xa);
             Dft<R1, -1>::run(xb);
